@@ -1,0 +1,252 @@
+"""ctypes front end of the CPU oracle -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+legs may import this package.  It never imports paper_1407_7595_b200.
+All arithmetic lives in mem_oracle.cpp; this file only marshals arguments.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "mem_oracle.cpp")
+_HDR = os.path.join(_HERE, "mem_oracle.h")
+_LIB = os.path.join(_HERE, "libmem_oracle.so")
+
+W_ENU, Z_BB, TT_LJETS, TT_DILEP = 1, 2, 3, 4
+
+
+def build(force: bool = False) -> str:
+    """g++ -O2, no FMA contraction, platform libm (reading A16)."""
+    stale = (not os.path.exists(_LIB)) or any(
+        os.path.getmtime(s) > os.path.getmtime(_LIB) for s in (_SRC, _HDR))
+    if force or stale:
+        tmp = _LIB + ".%d.tmp" % os.getpid()
+        subprocess.check_call(["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fPIC", "-shared",
+                               "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+class Params(C.Structure):
+    _fields_ = [(n, C.c_double) for n in (
+        "sqrt_s", "G_F", "alpha_s", "sin2_thw", "m_W", "Gam_W", "m_Z", "Gam_Z", "m_t", "Gam_t",
+        "V_ud", "V_tb", "pdf_A_q", "pdf_A_g", "pdf_pow_x", "pdf_pow_1mx",
+        "tf_w_tail", "tf_mu1", "tf_sig1", "tf_mu2", "tf_sig2",
+        "jetE_rlo", "jetE_rhi", "bw_nwidths", "nu_pz_max", "nu_eta_max", "met_sigma", "met_nsigma",
+        "vegas_alpha")] + [("vegas_points", C.c_int64), ("vegas_iters", C.c_int32),
+                           ("vegas_bins", C.c_int32), ("n_flav", C.c_int32), ("reserved", C.c_int32)]
+
+
+_lib = None
+_dp = C.POINTER(C.c_double)
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(build())
+        L.orc_params_default.argtypes = [C.c_int, C.POINTER(Params)]
+        L.orc_n_fields.argtypes = [C.c_int]
+        L.orc_n_dims.argtypes = [C.c_int]
+        L.orc_philox4x32_10.argtypes = [C.POINTER(C.c_uint32)] * 3
+        L.orc_philox4x32_10.restype = None
+        L.orc_u52.argtypes = [C.c_uint32, C.c_uint32]
+        L.orc_u52.restype = C.c_double
+        L.orc_uniforms.argtypes = [C.c_uint64, C.c_uint64, C.c_uint64, C.c_uint32, C.c_int, _dp]
+        L.orc_uniforms.restype = None
+        L.orc_pdf_shape.argtypes = [C.POINTER(Params), C.c_double]
+        L.orc_pdf_shape.restype = C.c_double
+        L.orc_tf_jet.argtypes = [C.POINTER(Params), C.c_double, C.c_double]
+        L.orc_tf_jet.restype = C.c_double
+        L.orc_bw_window.argtypes = [C.c_double] * 4 + [_dp, _dp]
+        L.orc_bw_window.restype = None
+        L.orc_bw_point.argtypes = [C.c_double] * 3 + [_dp, _dp, _dp]
+        L.orc_bw_point.restype = None
+        L.orc_me_w.argtypes = [C.POINTER(Params)] + [_dp] * 4
+        L.orc_me_w.restype = C.c_double
+        L.orc_me_z.argtypes = [C.POINTER(Params), C.c_int] + [_dp] * 4
+        L.orc_me_z.restype = C.c_double
+        for f in (L.orc_me_tt_qq, L.orc_me_tt_gg):
+            f.argtypes = [C.POINTER(Params)] + [_dp] * 4
+            f.restype = C.c_double
+        L.orc_me_top_decay.argtypes = [C.POINTER(Params), C.c_double] + [_dp] * 4
+        L.orc_me_top_decay.restype = C.c_double
+        L.orc_boost_transverse.argtypes = [_dp, C.c_int, _dp]
+        L.orc_boost_transverse.restype = None
+        L.orc_weight.argtypes = [C.c_int, C.POINTER(Params), _dp, _dp, _dp]
+        L.orc_weight.restype = C.c_double
+        L.orc_eval_points.argtypes = [C.c_int, C.POINTER(Params), _dp, C.c_int64, C.c_int64, C.c_uint64,
+                                      C.c_int64, C.c_int64, C.c_uint64, C.c_int32, _dp, _dp]
+        L.orc_integrate.argtypes = [C.c_int, C.POINTER(Params), _dp, C.c_int64, C.c_uint64, C.c_int64,
+                                    C.c_uint64, _dp, _dp]
+        L.orc_vegas_map.argtypes = [_dp, C.c_int, C.c_int, _dp, _dp, C.POINTER(C.c_int), _dp]
+        L.orc_vegas_map.restype = None
+        L.orc_vegas_refine.argtypes = [_dp, _dp, C.c_int, C.c_double]
+        L.orc_vegas_refine.restype = None
+        L.orc_vegas_integrate.argtypes = [C.c_int, C.POINTER(Params), _dp, C.c_int64, C.c_uint64, C.c_int64,
+                                          C.c_uint64, _dp, _dp, _dp]
+        _lib = L
+    return _lib
+
+
+def _p(a):
+    return a.ctypes.data_as(_dp)
+
+
+def _f64(a):
+    return np.ascontiguousarray(np.asarray(a, dtype=np.float64))
+
+
+def params_default(process: int) -> Params:
+    p = Params()
+    if lib().orc_params_default(process, C.byref(p)) != 0:
+        raise ValueError("unknown process %r" % process)
+    return p
+
+
+def n_fields(process):
+    return lib().orc_n_fields(process)
+
+
+def n_dims(process):
+    return lib().orc_n_dims(process)
+
+
+def philox4x32_10(ctr, key):
+    c = (C.c_uint32 * 4)(*ctr)
+    k = (C.c_uint32 * 2)(*key)
+    o = (C.c_uint32 * 4)()
+    lib().orc_philox4x32_10(c, k, o)
+    return [int(x) for x in o]
+
+
+def u52(a, b):
+    return lib().orc_u52(a, b)
+
+
+def uniforms(seed, event, point, iteration, n):
+    u = np.empty(n, dtype=np.float64)
+    lib().orc_uniforms(seed, event, point, iteration, n, _p(u))
+    return u
+
+
+def pdf_shape(p, x):
+    return lib().orc_pdf_shape(C.byref(p), x)
+
+
+def tf_jet(p, e_jet, e_parton):
+    return lib().orc_tf_jet(C.byref(p), e_jet, e_parton)
+
+
+def bw_window(m, gam, s_lo, s_hi):
+    a, b = C.c_double(), C.c_double()
+    lib().orc_bw_window(m, gam, s_lo, s_hi, C.byref(a), C.byref(b))
+    return a.value, b.value
+
+
+def bw_point(m, gam, t):
+    a, b, c = C.c_double(), C.c_double(), C.c_double()
+    lib().orc_bw_point(m, gam, t, C.byref(a), C.byref(b), C.byref(c))
+    return a.value, b.value, c.value
+
+
+def _v4(*vs):
+    return [_f64(v) for v in vs]
+
+
+def me_w(p, qa, qb, lep, nu):
+    a = _v4(qa, qb, lep, nu)
+    return lib().orc_me_w(C.byref(p), *[_p(x) for x in a])
+
+
+def me_z(p, up_type, qa, qb, p1, p2):
+    a = _v4(qa, qb, p1, p2)
+    return lib().orc_me_z(C.byref(p), int(up_type), *[_p(x) for x in a])
+
+
+def me_tt_qq(p, q1, q2, pt, ptb):
+    a = _v4(q1, q2, pt, ptb)
+    return lib().orc_me_tt_qq(C.byref(p), *[_p(x) for x in a])
+
+
+def me_tt_gg(p, q1, q2, pt, ptb):
+    a = _v4(q1, q2, pt, ptb)
+    return lib().orc_me_tt_gg(C.byref(p), *[_p(x) for x in a])
+
+
+def me_top_decay(p, n_c, pt, pb, pf_down, pf_up):
+    a = _v4(pt, pb, pf_down, pf_up)
+    return lib().orc_me_top_decay(C.byref(p), float(n_c), *[_p(x) for x in a])
+
+
+def boost_transverse(P, mom):
+    P = _f64(P)
+    m = _f64(mom).copy()
+    lib().orc_boost_transverse(_p(P), m.shape[0], _p(m))
+    return m
+
+
+def weight(process, p, rec, u, debug=False):
+    rec, u = _f64(rec), _f64(u)
+    if debug:
+        dbg = np.zeros(1 + 4 * (2 + 4 * 6), dtype=np.float64)
+        w = lib().orc_weight(process, C.byref(p), _p(rec), _p(u), _p(dbg))
+        return w, dbg
+    return lib().orc_weight(process, C.byref(p), _p(rec), _p(u), None)
+
+
+def eval_points(process, p, events, event, first_point, n, seed, iteration=0, grid=None, event_offset=0):
+    ev = _f64(events)
+    out = np.empty(n, dtype=np.float64)
+    g = None if grid is None else _f64(grid)
+    rc = lib().orc_eval_points(process, C.byref(p), _p(ev), ev.shape[1], event, event_offset, first_point, n,
+                               seed, iteration, None if g is None else _p(g), _p(out))
+    if rc != 0:
+        raise ValueError("orc_eval_points failed")
+    return out
+
+
+def integrate(process, p, events, n_points, seed, event_offset=0):
+    ev = _f64(events)
+    ne = ev.shape[1]
+    op, oe = np.empty(ne), np.empty(ne)
+    rc = lib().orc_integrate(process, C.byref(p), _p(ev), ne, event_offset, n_points, seed, _p(op), _p(oe))
+    if rc != 0:
+        raise ValueError("orc_integrate failed")
+    return op, oe
+
+
+def vegas_map(edges, u):
+    e = _f64(edges)
+    D, B1 = e.shape
+    u = _f64(u)
+    z = np.empty(D)
+    k = (C.c_int * D)()
+    jac = C.c_double()
+    lib().orc_vegas_map(_p(e), B1 - 1, D, _p(u), _p(z), k, C.byref(jac))
+    return z, np.array(list(k)), jac.value
+
+
+def vegas_refine(hist, edges, alpha):
+    h = _f64(hist)
+    e = _f64(edges).copy()
+    lib().orc_vegas_refine(_p(h), _p(e), h.shape[0], alpha)
+    return e
+
+
+def vegas_integrate(process, p, events, n_points, seed, event_offset=0, return_grid=False):
+    ev = _f64(events)
+    ne = ev.shape[1]
+    D = n_dims(process)
+    op, oe = np.empty(ne), np.empty(ne)
+    grid = np.empty((ne, D, p.vegas_bins + 1))
+    rc = lib().orc_vegas_integrate(process, C.byref(p), _p(ev), ne, event_offset, n_points, seed,
+                                   _p(op), _p(oe), _p(grid))
+    if rc != 0:
+        raise ValueError("orc_vegas_integrate failed")
+    return (op, oe, grid) if return_grid else (op, oe)

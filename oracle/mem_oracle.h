@@ -1,0 +1,100 @@
+/* oracle/mem_oracle.h -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, single-threaded fp64 CPU oracle for the per-event Monte Carlo
+ * estimate of the matrix-element-method likelihood of arXiv 1407.7595
+ * (PAPER.md:45 Eq. 1, :49 Eq. 2, :56 Eq. 3, :76-81 Eq. 5-6, :103-118 Eq. 7-8).
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may use it.  It shares no code, header, table or
+ * constant with the CUDA path under paper_1407_7595_b200/csrc/ (its parameter
+ * struct below is its own, deliberately laid out differently from mem_params).
+ *
+ * All momenta are (E, px, py, pz), natural units, GeV, metric (+,-,-,-).
+ */
+#ifndef MEM_ORACLE_H
+#define MEM_ORACLE_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { ORC_W_ENU = 1, ORC_Z_BB = 2, ORC_TT_LJETS = 3, ORC_TT_DILEP = 4 };
+
+/* DESIGN.md "Readings" O8/A13: the paper gives no constants; BASELINE.json
+ * configs give sqrt_s, m_W, Gam_W, m_t, Gam_t, the toy PDF and the TF numbers. */
+typedef struct orc_params {
+  /* physics constants */
+  double sqrt_s, G_F, alpha_s, sin2_thw;
+  double m_W, Gam_W, m_Z, Gam_Z, m_t, Gam_t;
+  double V_ud, V_tb;
+  /* toy PDF f(x) = A x^pow_x (1-x)^pow_1mx (BASELINE.json:configs[0]) */
+  double pdf_A_q, pdf_A_g, pdf_pow_x, pdf_pow_1mx;
+  /* double-Gaussian jet TF, as fractions of the parton energy (configs[1]) */
+  double tf_w_tail, tf_mu1, tf_sig1, tf_mu2, tf_sig2;
+  /* integration windows */
+  double jetE_rlo, jetE_rhi, bw_nwidths, nu_pz_max, nu_eta_max, met_sigma, met_nsigma;
+  /* VEGAS (configs[4]) */
+  double vegas_alpha;
+  int64_t vegas_points;
+  int32_t vegas_iters, vegas_bins;
+  int32_t n_flav, reserved;
+} orc_params;
+
+int  orc_params_default(int process, orc_params* p);
+int  orc_n_fields(int process);   /* 5 / 6 / 17 / 14 */
+int  orc_n_dims(int process);     /* 1 / 2 / 6 / 8  */
+
+/* --- random numbers (O2) --- */
+void   orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+double orc_u52(uint32_t a, uint32_t b);
+void   orc_uniforms(uint64_t seed, uint64_t event, uint64_t point, uint32_t iteration,
+                    int n_dims, double* u);
+
+/* --- building blocks, exposed so that the tests can pin each one --- */
+double orc_pdf_shape(const orc_params* p, double x);
+double orc_tf_jet(const orc_params* p, double E_jet, double E_parton);
+/* Breit-Wigner map: t-window of [s_lo, s_hi]; at t: s - m^2, ds/dt, D(s). */
+void   orc_bw_window(double m, double Gam, double s_lo, double s_hi, double* t_lo, double* t_hi);
+void   orc_bw_point(double m, double Gam, double t, double* s_minus_m2, double* dsdt, double* D);
+/* spin/colour averaged (initial), summed (final) LO matrix elements */
+double orc_me_w(const orc_params* p, const double qa[4], const double qb[4],
+                const double lep[4], const double nu[4]);           /* u(qa) dbar(qb) -> e+ nu */
+double orc_me_z(const orc_params* p, int up_type, const double qa[4], const double qb[4],
+                const double p1[4], const double p2[4]);            /* q(qa) qbar(qb) -> b(p1) bbar(p2) */
+double orc_me_tt_qq(const orc_params* p, const double q1[4], const double q2[4],
+                    const double pt[4], const double ptb[4]);
+double orc_me_tt_gg(const orc_params* p, const double q1[4], const double q2[4],
+                    const double pt[4], const double ptb[4]);
+/* sum over ALL spins of |M(t -> b f fbar')|^2, colour factor n_c (1 leptonic, 3 hadronic) */
+double orc_me_top_decay(const orc_params* p, double n_c, const double pt[4], const double pb[4],
+                        const double pf_down[4], const double pf_up[4]);
+void   orc_boost_transverse(const double P[4], int n, double* mom /* n x 4, in place */);
+
+/* --- the integrand: one event record (n_fields doubles), one unit-cube point --- */
+/* dbg (may be NULL): [0]=n_sol, [1..]= per solution: x1, x2, then the boosted final momenta. */
+double orc_weight(int process, const orc_params* p, const double* rec, const double* u, double* dbg);
+
+/* events: SoA, field-major [n_fields][n_events].  grid (may be NULL) = VEGAS edges
+ * [n_events][D][bins+1]; then u is warped through it first. */
+int orc_eval_points(int process, const orc_params* p, const double* events, int64_t n_events,
+                    int64_t event, uint64_t event_offset, int64_t first_point, int64_t n,
+                    uint64_t seed, int32_t iteration, const double* grid, double* out_w);
+int orc_integrate(int process, const orc_params* p, const double* events, int64_t n_events,
+                  uint64_t event_offset, int64_t n_points, uint64_t seed,
+                  double* out_p, double* out_err);
+
+/* --- VEGAS (DESIGN.md config 5, reading A14) --- */
+void orc_vegas_map(const double* edges /* [D][bins+1] */, int bins, int n_dims, const double* u,
+                   double* z, int* k, double* jac);
+void orc_vegas_refine(const double* hist /* [bins] */, double* edges /* [bins+1], in place */,
+                      int bins, double alpha);
+/* runs p->vegas_iters adaptation passes of p->vegas_points, then a final pass of n_points;
+ * grid_out (may be NULL): final edges [n_events][D][bins+1]. */
+int orc_vegas_integrate(int process, const orc_params* p, const double* events, int64_t n_events,
+                        uint64_t event_offset, int64_t n_points, uint64_t seed,
+                        double* out_p, double* out_err, double* grid_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
