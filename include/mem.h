@@ -1,0 +1,141 @@
+/* include/mem.h -- C ABI of the B200-native matrix-element-method integrator.
+ *
+ * One call estimates, for every measured event, the MEM likelihood of
+ * arXiv 1407.7595 (PAPER.md:45 Eq. 1, :49 Eq. 2, :56 Eq. 3)
+ *
+ *     p = int sum_flav |M|^2(Y) f1(x1) f2(x2) / (|q1||q2|) T(X;Y) dPhi_n
+ *
+ * by Monte Carlo (PAPER.md:76 Eq. 5, :80 Eq. 6): sampling, variable maps,
+ * matrix element, toy PDFs, jet transfer functions, phase-space Jacobian, the
+ * reduction to (mean, standard error) and the optional per-event VEGAS grid
+ * refinement all run in sm_100a CUDA kernels.  There is no
+ * CPU fallback: every entry point that needs the device fails with
+ * MEM_ERR_CUDA when no CUDA device is usable.
+ *
+ * Conventions: natural units, GeV, metric (+,-,-,-).  "device" pointers are
+ * CUDA device pointers valid on the current device, 8-byte aligned; "host"
+ * pointers are ordinary process memory.  The library never frees, reallocates
+ * or retains caller buffers.  All functions return a mem_status and never
+ * throw or abort; mem_last_error() gives a thread-local message for the last
+ * failure on the calling thread.  A handle must not be used from two threads
+ * at once; distinct handles are independent.
+ */
+#ifndef MEM_B200_H
+#define MEM_B200_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mem_handle mem_handle; /* opaque; owned by the library */
+
+typedef enum {
+  MEM_OK = 0,
+  MEM_ERR_INVALID_ARG = 1, /* null / negative / misaligned / out-of-range argument */
+  MEM_ERR_UNSUPPORTED = 2, /* valid request this build does not implement */
+  MEM_ERR_CUDA = 3,        /* CUDA runtime error (message in mem_last_error) */
+  MEM_ERR_NOMEM = 4        /* workspace allocation failed */
+} mem_status;
+
+/* Process hypotheses = BASELINE.json:configs[0..3]. */
+typedef enum {
+  MEM_PROC_W_ENU = 1,    /* u dbar -> W+ -> e+ nu,            D = 1,  5 record fields */
+  MEM_PROC_Z_BB = 2,     /* q qbar -> Z -> b bbar,            D = 2,  6 record fields */
+  MEM_PROC_TT_LJETS = 3, /* t tbar -> b l nu bbar q qbar',    D = 6, 17 record fields */
+  MEM_PROC_TT_DILEP = 4  /* t tbar -> b l+ nu bbar l- nubar,  D = 8, 14 record fields */
+} mem_process;
+
+/* All physics constants, integration windows and VEGAS options (DESIGN.md
+ * "Readings" O4-O8, A13, A14).  Size-prefixed POD: set struct_size =
+ * sizeof(mem_params); mem_params_default() fills every field. */
+typedef struct mem_params {
+  uint32_t struct_size;
+  uint32_t precision;   /* 64, or 32 (fp32 integrand core; MEM_PROC_TT_LJETS only, reading A15) */
+  double sqrt_s;        /* pp centre-of-mass energy */
+  double G_F, m_W, Gam_W, m_Z, Gam_Z, sin2_thw, m_t, Gam_t, alpha_s, V_ud, V_tb;
+  double pdf_A_q, pdf_A_g, pdf_pow_x, pdf_pow_1mx; /* toy PDF f(x) = A x^pow_x (1-x)^pow_1mx */
+  double tf_w_tail, tf_mu1, tf_sig1, tf_mu2, tf_sig2; /* double-Gaussian jet TF, fractions of parton E */
+  double jetE_rlo, jetE_rhi; /* parton-energy window, fractions of the measured jet energy */
+  double bw_nwidths;         /* Breit-Wigner windows m +- n Gamma */
+  double nu_pz_max;          /* config 1: |nu_z| <= nu_pz_max */
+  double nu_eta_max;         /* config 3: |eta_nu| <= nu_eta_max */
+  double met_sigma, met_nsigma; /* config 4: Gaussian MET TF, flat +-n sigma sampling */
+  double vegas_alpha;        /* grid damping exponent */
+  int64_t vegas_points;      /* points per adaptation pass */
+  int32_t vegas_iters;       /* adaptation passes; 0 = plain Monte Carlo */
+  int32_t vegas_bins;        /* bins per dimension, 1..64 */
+  int32_t n_flav;            /* light flavours summed in the initial state */
+  int32_t reserved;
+} mem_params;
+
+/* Fill *params with the defaults of `process` (precision 64, plain MC). */
+mem_status mem_params_default(mem_process process, mem_params* params /* host, out */);
+
+/* Record fields per event (5 / 6 / 17 / 14) and integration dimensions (1 / 2 / 6 / 8);
+ * -1 for an unknown process. */
+int32_t mem_event_fields(mem_process process);
+int32_t mem_n_dims(mem_process process);
+
+/* Create an integrator for one process hypothesis on the current CUDA device.
+ * params (host) is copied; NULL = defaults.  *out receives the handle. */
+mem_status mem_create(mem_process process, const mem_params* params, mem_handle** out);
+
+/* Free the handle and its workspace (synchronises the device). NULL is a no-op. */
+mem_status mem_destroy(mem_handle* h);
+
+/* Multi-GPU sharding: the event index that enters the
+ * Philox counter is first_event + local index, so a contiguous shard of a
+ * larger list reproduces the unsharded result bit for bit.  Default 0. */
+mem_status mem_set_event_offset(mem_handle* h, uint64_t first_event);
+
+/* The hot path.  For each event e in [0, n_events):
+ *   w_i = integrand at the point drawn from Philox4x32-10 with key = seed and
+ *         counter = (point i, first_event + e, pass, word block),  i in [0, n_points)
+ *   out_p[e]   = (1/N) sum w_i
+ *   out_err[e] = sqrt(max(0, (sum w_i^2)/N - out_p[e]^2) / (N - 1))
+ * With params.vegas_iters > 0 each event first runs vegas_iters adaptation
+ * passes of vegas_points points that refine its own importance-sampling grid;
+ * the outputs then come from the final pass of n_points only.
+ *
+ * events : device, float64, SoA field-major [mem_event_fields][n_events]; read-only
+ * out_p, out_err : device, float64 [n_events]; overwritten
+ * cuda_stream : a cudaStream_t (NULL = legacy default stream).  All work is
+ *   enqueued on it and the call returns without synchronising.  The handle's
+ *   workspace grows on demand (a growth step synchronises that stream).
+ * n_events == 0 is MEM_OK with no launch; n_points < 2 is MEM_ERR_INVALID_ARG.
+ * Kinematically forbidden or non-finite points contribute w = 0 and still count in N. */
+mem_status mem_integrate(mem_handle* h, const double* events, int64_t n_events,
+                         int64_t n_points, uint64_t seed,
+                         double* out_p, double* out_err, void* cuda_stream);
+
+/* Same computation through host buffers: copies `events` host->device, runs
+ * mem_integrate, copies the two result arrays device->host and synchronises.
+ * This is the end-to-end entry the benchmark's "e2e" figure times. */
+mem_status mem_integrate_host(mem_handle* h, const double* events_host, int64_t n_events,
+                              int64_t n_points, uint64_t seed,
+                              double* out_p_host, double* out_err_host);
+
+/* Diagnostic for the parity tests: the individual weights w_i of one event,
+ * i in [first_point, first_point + n), for Philox pass `iteration`.
+ * grid (device, may be NULL): VEGAS edges [D][vegas_bins + 1] of THIS event;
+ * when given, the unit-cube point is warped through it and w includes the
+ * grid Jacobian.  out_w: device, float64 [n]. */
+mem_status mem_eval_points(mem_handle* h, const double* events, int64_t n_events, int64_t event,
+                           int64_t first_point, int64_t n, uint64_t seed, int32_t iteration,
+                           const double* grid, double* out_w, void* cuda_stream);
+
+/* Diagnostic: copy the VEGAS grids left by the last mem_integrate with
+ * vegas_iters > 0 into out_grid (device, float64 [n_events][D][vegas_bins+1]). */
+mem_status mem_get_grid(mem_handle* h, int64_t n_events, double* out_grid, void* cuda_stream);
+
+/* Kernels launched by this handle since creation (for the benchmark's launch count). */
+int64_t mem_launch_count(const mem_handle* h);
+
+/* Thread-local description of the last error on this thread ("" if none). */
+const char* mem_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MEM_B200_H */

@@ -1,0 +1,425 @@
+// mem_api.cu -- the C ABI of include/mem.h: argument checks, workspace, kernel launches.
+// No arithmetic of the method lives here beyond turning mem_params into DevConst.
+#include "../../include/mem.h"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "mem_kernels.cuh"
+
+using namespace memb200;
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+mem_status fail(mem_status s, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+  return s;
+}
+
+#define CUDA_TRY(expr)                                                                      \
+  do {                                                                                      \
+    cudaError_t _e = (expr);                                                                \
+    if (_e != cudaSuccess)                                                                  \
+      return fail(_e == cudaErrorMemoryAllocation ? MEM_ERR_NOMEM : MEM_ERR_CUDA, "%s: %s", \
+                  #expr, cudaGetErrorString(_e));                                           \
+  } while (0)
+
+int n_fields_of(int process) {
+  switch (process) {
+    case MEM_PROC_W_ENU: return 5;
+    case MEM_PROC_Z_BB: return 6;
+    case MEM_PROC_TT_LJETS: return 17;
+    case MEM_PROC_TT_DILEP: return 14;
+  }
+  return -1;
+}
+int n_dims_of(int process) {
+  switch (process) {
+    case MEM_PROC_W_ENU: return 1;
+    case MEM_PROC_Z_BB: return 2;
+    case MEM_PROC_TT_LJETS: return 6;
+    case MEM_PROC_TT_DILEP: return 8;
+  }
+  return -1;
+}
+int n_consts_of(int process) {
+  switch (process) {
+    case MEM_PROC_W_ENU: return ProcWenu::NC;
+    case MEM_PROC_Z_BB: return ProcZbb::NC;
+    case MEM_PROC_TT_LJETS: return ProcTTljets::NC;
+  }
+  return -1;
+}
+
+struct Buffer {
+  void* p = nullptr;
+  size_t cap = 0;
+};
+
+}  // namespace
+
+struct mem_handle {
+  int process;
+  int device;
+  mem_params params;
+  DevConst dc;
+  uint64_t event_offset;
+  int64_t launches;
+  int64_t grid_events;      // events covered by the grids of the last VEGAS call
+  Buffer ecs, partials, grids, hist, stage_in, stage_out;
+};
+
+namespace {
+
+mem_status ensure(Buffer& b, size_t bytes, cudaStream_t st) {
+  if (bytes <= b.cap) return MEM_OK;
+  if (b.p) {
+    CUDA_TRY(cudaStreamSynchronize(st));
+    CUDA_TRY(cudaFree(b.p));
+    b.p = nullptr; b.cap = 0;
+  }
+  size_t want = bytes + bytes / 4;
+  cudaError_t e = cudaMalloc(&b.p, want);
+  if (e != cudaSuccess) {
+    (void)cudaGetLastError();
+    want = bytes;
+    e = cudaMalloc(&b.p, want);
+  }
+  if (e != cudaSuccess) {
+    (void)cudaGetLastError();
+    b.p = nullptr;
+    return fail(MEM_ERR_NOMEM, "cudaMalloc(%zu bytes): %s", want, cudaGetErrorString(e));
+  }
+  b.cap = want;
+  return MEM_OK;
+}
+
+// flavours in the paper's order (d, u, s, c, b); L = T3 - Q sin^2, R = -Q sin^2 (O8)
+void z_coupling_sums(const mem_params& p, double* cu, double* ct) {
+  const double Lb = -0.5 + p.sin2_thw / 3.0, Rb = p.sin2_thw / 3.0;
+  double su = 0.0, st = 0.0;
+  for (int f = 0; f < p.n_flav; ++f) {
+    const bool up = (f == 1 || f == 3);
+    const double T3 = up ? 0.5 : -0.5, Q = up ? 2.0 / 3.0 : -1.0 / 3.0;
+    const double L = T3 - Q * p.sin2_thw, R = -Q * p.sin2_thw;
+    su += L * L * Lb * Lb + R * R * Rb * Rb;
+    st += L * L * Rb * Rb + R * R * Lb * Lb;
+  }
+  *cu = su; *ct = st;
+}
+
+void bw_window(double m, double G, double n, double* t_lo, double* dt) {
+  const double lo = std::atan(((m - n * G) * (m - n * G) - m * m) / (m * G));
+  const double hi = std::atan(((m + n * G) * (m + n * G) - m * m) / (m * G));
+  *t_lo = lo; *dt = hi - lo;
+}
+
+DevConst make_dev_const(const mem_params& p) {
+  DevConst c;
+  std::memset(&c, 0, sizeof(c));
+  c.sqrt_s = p.sqrt_s; c.inv_sqrt_s = 1.0 / p.sqrt_s; c.S = p.sqrt_s * p.sqrt_s; c.inv_S = 1.0 / c.S;
+  c.pdf_pow_x = p.pdf_pow_x; c.pdf_pow_1mx = p.pdf_pow_1mx;
+  c.pdf_fast = (p.pdf_pow_x == -0.5 && p.pdf_pow_1mx == 3.0) ? 1 : 0;
+  c.n_flav = p.n_flav;
+  c.A_q2 = p.pdf_A_q * p.pdf_A_q; c.A_g2 = p.pdf_A_g * p.pdf_A_g;
+  c.rlo = p.jetE_rlo; c.dr = p.jetE_rhi - p.jetE_rlo;
+  const double r2 = std::sqrt(2.0), r2pi = std::sqrt(2.0 * kPi);
+  c.tf_a1 = 1.0 / (p.tf_sig1 * r2); c.tf_b1 = -(1.0 + p.tf_mu1) / (p.tf_sig1 * r2);
+  c.tf_a2 = 1.0 / (p.tf_sig2 * r2); c.tf_b2 = -(1.0 + p.tf_mu2) / (p.tf_sig2 * r2);
+  c.tf_c1 = (1.0 - p.tf_w_tail) / (p.tf_sig1 * r2pi); c.tf_c2 = p.tf_w_tail / (p.tf_sig2 * r2pi);
+  c.mW = p.m_W; c.GW = p.Gam_W; c.mW2 = p.m_W * p.m_W; c.mWGW = p.m_W * p.Gam_W; c.mWGW2 = c.mWGW * c.mWGW;
+  bw_window(p.m_W, p.Gam_W, p.bw_nwidths, &c.tW_lo, &c.tW_dt);
+  c.mt2 = p.m_t * p.m_t; c.mtGt = p.m_t * p.Gam_t; c.mtGt2 = c.mtGt * c.mtGt;
+  bw_window(p.m_t, p.Gam_t, p.bw_nwidths, &c.tT_lo, &c.tT_dt);
+  c.mZ2 = p.m_Z * p.m_Z; c.mZGZ2 = p.m_Z * p.m_Z * p.Gam_Z * p.Gam_Z;
+  const double g2 = 4.0 * r2 * p.G_F * p.m_W * p.m_W, gz2 = 4.0 * r2 * p.G_F * p.m_Z * p.m_Z;
+  const double gs2 = 4.0 * kPi * p.alpha_s;
+  c.g4w = g2 * g2; c.gz4 = gz2 * gz2; c.gs4 = gs2 * gs2;
+  c.V_ud2 = p.V_ud * p.V_ud; c.V_tb2 = p.V_tb * p.V_tb;
+  z_coupling_sums(p, &c.z_cu, &c.z_ct);
+  c.nu_pz_max = p.nu_pz_max; c.nu_eta_max = p.nu_eta_max;
+  c.met_sigma = p.met_sigma; c.met_nsigma = p.met_nsigma;
+  c.vegas_bins = p.vegas_bins; c.vegas_alpha = p.vegas_alpha;
+  return c;
+}
+
+mem_status check_params(int process, const mem_params& p) {
+  if (p.struct_size != sizeof(mem_params))
+    return fail(MEM_ERR_INVALID_ARG, "mem_params.struct_size = %u, expected %zu", p.struct_size, sizeof(mem_params));
+  if (p.precision != 64 && p.precision != 32) return fail(MEM_ERR_INVALID_ARG, "precision must be 64 or 32");
+  if (p.precision == 32) return fail(MEM_ERR_UNSUPPORTED, "precision 32 is not implemented in this build");
+  const bool pos = p.sqrt_s > 0 && p.G_F > 0 && p.m_W > 0 && p.Gam_W > 0 && p.m_Z > 0 && p.Gam_Z > 0 && p.m_t > 0 &&
+                   p.Gam_t > 0 && p.alpha_s > 0 && p.tf_sig1 > 0 && p.tf_sig2 > 0 && p.jetE_rlo > 0 &&
+                   p.jetE_rhi > p.jetE_rlo && p.bw_nwidths > 0 && p.nu_pz_max > 0 && p.nu_eta_max > 0 &&
+                   p.met_sigma > 0 && p.met_nsigma > 0;
+  if (!pos) return fail(MEM_ERR_INVALID_ARG, "mem_params: a constant that must be positive is not");
+  if (!(p.tf_w_tail >= 0.0 && p.tf_w_tail <= 1.0)) return fail(MEM_ERR_INVALID_ARG, "tf_w_tail outside [0,1]");
+  if (p.n_flav < 1 || p.n_flav > 5) return fail(MEM_ERR_INVALID_ARG, "n_flav outside 1..5");
+  if (p.bw_nwidths * p.Gam_W >= p.m_W || p.bw_nwidths * p.Gam_t >= p.m_t)
+    return fail(MEM_ERR_INVALID_ARG, "bw_nwidths * Gamma must stay below the mass");
+  if (p.vegas_iters < 0 || p.vegas_iters > 255) return fail(MEM_ERR_INVALID_ARG, "vegas_iters outside 0..255");
+  if (p.vegas_iters > 0) {
+    if (p.vegas_bins < 1 || p.vegas_bins > kMaxBins) return fail(MEM_ERR_INVALID_ARG, "vegas_bins outside 1..%d", kMaxBins);
+    if (p.vegas_points < 2) return fail(MEM_ERR_INVALID_ARG, "vegas_points < 2");
+    if (!(p.vegas_alpha >= 0.0)) return fail(MEM_ERR_INVALID_ARG, "vegas_alpha < 0");
+  }
+  (void)process;
+  return MEM_OK;
+}
+
+bool aligned8(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 7u) == 0; }
+
+size_t integrate_smem(int NC, int D, int B, int mode) {
+  size_t n = (size_t)NC + 2 * kWarps;
+  if (mode != MODE_PLAIN) n += (size_t)D * (B + 1);
+  if (mode == MODE_ADAPT) n += (size_t)kWarps * D * B;
+  return n * sizeof(double);
+}
+
+template <class P>
+mem_status launch_prepare(mem_handle* h, const double* events, int64_t n_events, cudaStream_t st) {
+  mem_status s = ensure(h->ecs, (size_t)n_events * P::NC * sizeof(double), st);
+  if (s != MEM_OK) return s;
+  const int threads = 128;
+  prepare_kernel<P><<<(unsigned)((n_events + threads - 1) / threads), threads, 0, st>>>(
+      h->dc, events, n_events, (double*)h->ecs.p);
+  ++h->launches;
+  CUDA_TRY(cudaGetLastError());
+  return MEM_OK;
+}
+
+template <class P, int MODE>
+mem_status launch_pass(mem_handle* h, int64_t n_events, int64_t n_points, int64_t chunk, int n_chunks,
+                       uint64_t seed, uint32_t pass, cudaStream_t st) {
+  const int64_t blocks = n_events * n_chunks;
+  if (blocks > 0x7fffffffLL) return fail(MEM_ERR_INVALID_ARG, "n_events * chunks = %lld exceeds the grid limit", (long long)blocks);
+  const size_t smem = integrate_smem(P::NC, P::D, h->dc.vegas_bins, MODE);
+  integrate_kernel<P, MODE><<<(unsigned)blocks, kThreads, smem, st>>>(
+      h->dc, (const double*)h->ecs.p, (const double*)h->grids.p, (double*)h->partials.p, (double*)h->hist.p,
+      n_points, chunk, n_chunks, seed, h->event_offset, pass);
+  ++h->launches;
+  CUDA_TRY(cudaGetLastError());
+  return MEM_OK;
+}
+
+template <class P>
+mem_status integrate_impl(mem_handle* h, const double* events, int64_t n_events, int64_t n_points, uint64_t seed,
+                          double* out_p, double* out_err, cudaStream_t st) {
+  mem_status s = launch_prepare<P>(h, events, n_events, st);
+  if (s != MEM_OK) return s;
+  const int n_chunks = (int)((n_points + kChunk - 1) / kChunk);
+  s = ensure(h->partials, (size_t)n_events * n_chunks * 2 * sizeof(double), st);
+  if (s != MEM_OK) return s;
+  const mem_params& p = h->params;
+  if (p.vegas_iters > 0) {
+    const int D = P::D, B = p.vegas_bins;
+    // adaptation passes: at most kMaxAdaptChunks blocks per event, chunk a multiple of kThreads
+    int64_t a_chunk = (p.vegas_points + kMaxAdaptChunks - 1) / kMaxAdaptChunks;
+    if (a_chunk < kChunk) a_chunk = kChunk;
+    a_chunk = (a_chunk + kThreads - 1) / kThreads * kThreads;
+    const int a_chunks = (int)((p.vegas_points + a_chunk - 1) / a_chunk);
+    s = ensure(h->grids, (size_t)n_events * D * (B + 1) * sizeof(double), st);
+    if (s != MEM_OK) return s;
+    s = ensure(h->hist, (size_t)n_events * a_chunks * D * B * sizeof(double), st);
+    if (s != MEM_OK) return s;
+    if (a_chunks > n_chunks) {
+      s = ensure(h->partials, (size_t)n_events * a_chunks * 2 * sizeof(double), st);
+      if (s != MEM_OK) return s;
+    }
+    const int64_t ng = n_events * D * (B + 1);
+    grid_init_kernel<<<(unsigned)((ng + 255) / 256), 256, 0, st>>>((double*)h->grids.p, n_events, D, B);
+    ++h->launches;
+    CUDA_TRY(cudaGetLastError());
+    for (int it = 0; it < p.vegas_iters; ++it) {
+      s = launch_pass<P, MODE_ADAPT>(h, n_events, p.vegas_points, a_chunk, a_chunks, seed, (uint32_t)it, st);
+      if (s != MEM_OK) return s;
+      refine_kernel<<<(unsigned)n_events, dim3(64, D), 0, st>>>(h->dc, (const double*)h->hist.p, a_chunks,
+                                                                (double*)h->grids.p, D);
+      ++h->launches;
+      CUDA_TRY(cudaGetLastError());
+    }
+    h->grid_events = n_events;
+    s = launch_pass<P, MODE_GRID>(h, n_events, n_points, kChunk, n_chunks, seed, (uint32_t)p.vegas_iters, st);
+  } else {
+    s = launch_pass<P, MODE_PLAIN>(h, n_events, n_points, kChunk, n_chunks, seed, 0u, st);
+  }
+  if (s != MEM_OK) return s;
+  finalize_kernel<<<(unsigned)((n_events + 127) / 128), 128, 0, st>>>((const double*)h->partials.p, n_chunks,
+                                                                      n_events, n_points, out_p, out_err);
+  ++h->launches;
+  CUDA_TRY(cudaGetLastError());
+  return MEM_OK;
+}
+
+template <class P>
+mem_status eval_impl(mem_handle* h, const double* events, int64_t n_events, int64_t event, int64_t first,
+                     int64_t n, uint64_t seed, int32_t iteration, const double* grid, double* out_w,
+                     cudaStream_t st) {
+  mem_status s = launch_prepare<P>(h, events, n_events, st);
+  if (s != MEM_OK) return s;
+  const int threads = 128;
+  const size_t smem = ((size_t)P::NC + (size_t)P::D * (kMaxBins + 1)) * sizeof(double);
+  eval_points_kernel<P><<<(unsigned)((n + threads - 1) / threads), threads, smem, st>>>(
+      h->dc, (const double*)h->ecs.p, event, grid, first, n, seed, h->event_offset, (uint32_t)iteration, out_w);
+  ++h->launches;
+  CUDA_TRY(cudaGetLastError());
+  return MEM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* mem_last_error(void) { return g_err; }
+
+int32_t mem_event_fields(mem_process process) { return n_fields_of((int)process); }
+int32_t mem_n_dims(mem_process process) { return n_dims_of((int)process); }
+
+mem_status mem_params_default(mem_process process, mem_params* p) {
+  if (!p) return fail(MEM_ERR_INVALID_ARG, "params is NULL");
+  if (n_fields_of((int)process) < 0) return fail(MEM_ERR_INVALID_ARG, "unknown process %d", (int)process);
+  std::memset(p, 0, sizeof(*p));
+  p->struct_size = (uint32_t)sizeof(mem_params);
+  p->precision = 64;
+  p->sqrt_s = 14000.0;                                       // BASELINE.json:configs[0]
+  p->G_F = 1.16637e-5; p->m_W = 80.4; p->Gam_W = 2.09;       // configs[0]
+  p->m_Z = 91.1876; p->Gam_Z = 2.4952; p->sin2_thw = 0.2312;
+  p->m_t = 173.0; p->Gam_t = 1.4;                            // configs[2]
+  p->alpha_s = 0.118; p->V_ud = 1.0; p->V_tb = 1.0;
+  p->pdf_A_q = 1.0; p->pdf_A_g = 1.0; p->pdf_pow_x = -0.5; p->pdf_pow_1mx = 3.0;   // configs[0]
+  p->tf_w_tail = 0.3; p->tf_mu1 = 0.0; p->tf_sig1 = 0.15; p->tf_mu2 = -0.1; p->tf_sig2 = 0.35;  // configs[1]
+  p->jetE_rlo = 0.5; p->jetE_rhi = 2.0; p->bw_nwidths = 15.0;
+  p->nu_pz_max = 500.0;                                      // configs[0]
+  p->nu_eta_max = 5.0; p->met_sigma = 10.0; p->met_nsigma = 4.0;
+  p->vegas_alpha = 0.5; p->vegas_points = 1 << 17; p->vegas_iters = 0; p->vegas_bins = 50;      // configs[4]
+  p->n_flav = (process == MEM_PROC_Z_BB) ? 3 : 5;            // configs[1]
+  return MEM_OK;
+}
+
+mem_status mem_create(mem_process process, const mem_params* params, mem_handle** out) {
+  if (!out) return fail(MEM_ERR_INVALID_ARG, "out is NULL");
+  *out = nullptr;
+  if (n_fields_of((int)process) < 0) return fail(MEM_ERR_INVALID_ARG, "unknown process %d", (int)process);
+  mem_params p;
+  if (params) p = *params;
+  else mem_params_default(process, &p);
+  mem_status s = check_params((int)process, p);
+  if (s != MEM_OK) return s;
+  if (n_consts_of((int)process) < 0)
+    return fail(MEM_ERR_UNSUPPORTED, "process %d is not implemented in this build", (int)process);
+  int dev = -1;
+  CUDA_TRY(cudaGetDevice(&dev));
+  cudaDeviceProp prop;
+  CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
+  if (prop.major < 10)
+    return fail(MEM_ERR_CUDA, "device %d is sm_%d%d; this library is built for sm_100a only", dev, prop.major, prop.minor);
+  mem_handle* h = new (std::nothrow) mem_handle();
+  if (!h) return fail(MEM_ERR_NOMEM, "out of host memory");
+  h->process = (int)process; h->device = dev; h->params = p; h->dc = make_dev_const(p);
+  h->event_offset = 0; h->launches = 0; h->grid_events = 0;
+  *out = h;
+  return MEM_OK;
+}
+
+mem_status mem_destroy(mem_handle* h) {
+  if (!h) return MEM_OK;
+  cudaDeviceSynchronize();
+  Buffer* bs[] = {&h->ecs, &h->partials, &h->grids, &h->hist, &h->stage_in, &h->stage_out};
+  for (Buffer* b : bs)
+    if (b->p) cudaFree(b->p);
+  delete h;
+  return MEM_OK;
+}
+
+mem_status mem_set_event_offset(mem_handle* h, uint64_t first_event) {
+  if (!h) return fail(MEM_ERR_INVALID_ARG, "handle is NULL");
+  h->event_offset = first_event;
+  return MEM_OK;
+}
+
+int64_t mem_launch_count(const mem_handle* h) { return h ? h->launches : -1; }
+
+mem_status mem_integrate(mem_handle* h, const double* events, int64_t n_events, int64_t n_points, uint64_t seed,
+                         double* out_p, double* out_err, void* cuda_stream) {
+  if (!h) return fail(MEM_ERR_INVALID_ARG, "handle is NULL");
+  if (n_events < 0) return fail(MEM_ERR_INVALID_ARG, "n_events < 0");
+  if (n_points < 2) return fail(MEM_ERR_INVALID_ARG, "n_points < 2");
+  if (n_events == 0) return MEM_OK;
+  if (!events || !out_p || !out_err) return fail(MEM_ERR_INVALID_ARG, "events / out_p / out_err is NULL");
+  if (!aligned8(events) || !aligned8(out_p) || !aligned8(out_err))
+    return fail(MEM_ERR_INVALID_ARG, "device pointers must be 8-byte aligned");
+  if (h->event_offset + (uint64_t)n_events > 0x100000000ULL)
+    return fail(MEM_ERR_INVALID_ARG, "event index exceeds the 32-bit Philox counter word");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  switch (h->process) {
+    case MEM_PROC_W_ENU: return integrate_impl<ProcWenu>(h, events, n_events, n_points, seed, out_p, out_err, st);
+    case MEM_PROC_Z_BB: return integrate_impl<ProcZbb>(h, events, n_events, n_points, seed, out_p, out_err, st);
+    case MEM_PROC_TT_LJETS: return integrate_impl<ProcTTljets>(h, events, n_events, n_points, seed, out_p, out_err, st);
+  }
+  return fail(MEM_ERR_UNSUPPORTED, "process %d is not implemented", h->process);
+}
+
+mem_status mem_integrate_host(mem_handle* h, const double* events_host, int64_t n_events, int64_t n_points,
+                              uint64_t seed, double* out_p_host, double* out_err_host) {
+  if (!h) return fail(MEM_ERR_INVALID_ARG, "handle is NULL");
+  if (n_events < 0) return fail(MEM_ERR_INVALID_ARG, "n_events < 0");
+  if (n_points < 2) return fail(MEM_ERR_INVALID_ARG, "n_points < 2");
+  if (n_events == 0) return MEM_OK;
+  if (!events_host || !out_p_host || !out_err_host) return fail(MEM_ERR_INVALID_ARG, "a host buffer is NULL");
+  const size_t in_bytes = (size_t)n_events * n_fields_of(h->process) * sizeof(double);
+  const size_t out_bytes = (size_t)n_events * sizeof(double);
+  cudaStream_t st = 0;
+  mem_status s = ensure(h->stage_in, in_bytes, st);
+  if (s != MEM_OK) return s;
+  s = ensure(h->stage_out, 2 * out_bytes, st);
+  if (s != MEM_OK) return s;
+  double* d_out = (double*)h->stage_out.p;
+  CUDA_TRY(cudaMemcpyAsync(h->stage_in.p, events_host, in_bytes, cudaMemcpyHostToDevice, st));
+  s = mem_integrate(h, (const double*)h->stage_in.p, n_events, n_points, seed, d_out, d_out + n_events, st);
+  if (s != MEM_OK) return s;
+  CUDA_TRY(cudaMemcpyAsync(out_p_host, d_out, out_bytes, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaMemcpyAsync(out_err_host, d_out + n_events, out_bytes, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  return MEM_OK;
+}
+
+mem_status mem_eval_points(mem_handle* h, const double* events, int64_t n_events, int64_t event, int64_t first_point,
+                           int64_t n, uint64_t seed, int32_t iteration, const double* grid, double* out_w,
+                           void* cuda_stream) {
+  if (!h) return fail(MEM_ERR_INVALID_ARG, "handle is NULL");
+  if (n_events <= 0 || event < 0 || event >= n_events) return fail(MEM_ERR_INVALID_ARG, "event outside [0, n_events)");
+  if (n < 0 || first_point < 0) return fail(MEM_ERR_INVALID_ARG, "n < 0 or first_point < 0");
+  if (iteration < 0 || iteration > 255) return fail(MEM_ERR_INVALID_ARG, "iteration outside 0..255");
+  if (n == 0) return MEM_OK;
+  if (!events || !out_w) return fail(MEM_ERR_INVALID_ARG, "events / out_w is NULL");
+  if (!aligned8(events) || !aligned8(out_w) || !aligned8(grid))
+    return fail(MEM_ERR_INVALID_ARG, "device pointers must be 8-byte aligned");
+  if (grid && (h->params.vegas_bins < 1 || h->params.vegas_bins > kMaxBins))
+    return fail(MEM_ERR_INVALID_ARG, "vegas_bins outside 1..%d", kMaxBins);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  switch (h->process) {
+    case MEM_PROC_W_ENU: return eval_impl<ProcWenu>(h, events, n_events, event, first_point, n, seed, iteration, grid, out_w, st);
+    case MEM_PROC_Z_BB: return eval_impl<ProcZbb>(h, events, n_events, event, first_point, n, seed, iteration, grid, out_w, st);
+    case MEM_PROC_TT_LJETS: return eval_impl<ProcTTljets>(h, events, n_events, event, first_point, n, seed, iteration, grid, out_w, st);
+  }
+  return fail(MEM_ERR_UNSUPPORTED, "process %d is not implemented", h->process);
+}
+
+mem_status mem_get_grid(mem_handle* h, int64_t n_events, double* out_grid, void* cuda_stream) {
+  if (!h || !out_grid) return fail(MEM_ERR_INVALID_ARG, "handle / out_grid is NULL");
+  if (h->params.vegas_iters <= 0 || !h->grids.p || n_events != h->grid_events)
+    return fail(MEM_ERR_INVALID_ARG, "no VEGAS grids for %lld events on this handle", (long long)n_events);
+  const size_t bytes = (size_t)n_events * n_dims_of(h->process) * (h->params.vegas_bins + 1) * sizeof(double);
+  CUDA_TRY(cudaMemcpyAsync(out_grid, h->grids.p, bytes, cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream));
+  return MEM_OK;
+}
+
+}  // extern "C"

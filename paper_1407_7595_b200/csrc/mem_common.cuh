@@ -1,0 +1,149 @@
+// mem_common.cuh -- pieces shared by every process kernel of the CUDA path.
+//
+// S1 of the hot path: Philox4x32-10 counter-based sampling keyed by
+// (seed, event, point) (BASELINE.json:north_star (b)); the toy PDF (BASELINE.json:configs[0]);
+// the double-Gaussian jet transfer function; the warp/block reduction of
+// sum w and sum w^2 (Eq. 5-6).  Nothing here is shared with oracle/.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace memb200 {
+
+constexpr int kThreads = 256;            // threads per block in the integrate kernels
+constexpr int kWarps = kThreads / 32;
+constexpr int64_t kChunk = 1 << 14;      // points per (event, chunk) block; fixes the reduction order
+constexpr int kMaxDims = 8;
+constexpr int kMaxBins = 64;
+constexpr int kMaxAdaptChunks = 8;       // adaptation passes use at most this many blocks per event
+
+// Everything the kernels need that does not depend on the event.  Filled on the host from
+// mem_params (mem_api.cu: make_dev_const) and passed by value as a kernel argument, so every
+// member is a constant-bank operand.
+struct DevConst {
+  // beams, O3
+  double sqrt_s, inv_sqrt_s, S, inv_S;
+  // toy PDF, O4
+  double pdf_pow_x, pdf_pow_1mx;
+  int pdf_fast;                         // 1 when pow_x == -1/2 and pow_1mx == 3
+  int n_flav;
+  double A_q2, A_g2;                    // pdf_A_q^2, pdf_A_g^2
+  // jets, O5: E = E_jet (rlo + dr u); TF(E_jet; E) * E = c1 exp(-z1^2) + c2 exp(-z2^2),
+  // z_k = a_k / x + b_k with x = E / E_jet
+  double rlo, dr;
+  double tf_a1, tf_b1, tf_c1, tf_a2, tf_b2, tf_c2;
+  // Breit-Wigner data, O6
+  double mW, GW, mW2, mWGW, mWGW2;      // m, Gamma, m^2, m Gamma, (m Gamma)^2
+  double tW_lo, tW_dt;                  // t window of m +- n Gamma
+  double mt2, mtGt, mtGt2, tT_lo, tT_dt;
+  double mZ2, mZGZ2;
+  // couplings, O8
+  double g4w;                           // g^4, g^2 = 4 sqrt2 G_F m_W^2
+  double gz4;                           // g_Z^4
+  double gs4;                           // g_s^4 = (4 pi alpha_s)^2
+  double V_ud2, V_tb2;
+  double z_cu, z_ct;                    // sum_q [..] coefficient of u^2 and of t^2 (config 2)
+  // windows
+  double nu_pz_max, nu_eta_max, met_sigma, met_nsigma;
+  // VEGAS
+  int vegas_bins;
+  double vegas_alpha;
+};
+
+// ---------------------------------------------------------------------------------------
+// S1. Philox4x32-10 (Salmon et al. 2011; multipliers and Weyl constants are the published ones)
+// ---------------------------------------------------------------------------------------
+struct Philox {
+  uint32_t k0, k1;                      // key = (seed low, seed high)
+  __device__ __forceinline__ void operator()(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                             uint32_t (&out)[4]) const {
+    uint32_t a = k0, b = k1;
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+      const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+      const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+      c0 = hi1 ^ c1 ^ a; c1 = lo1; c2 = hi0 ^ c3 ^ b; c3 = lo0;
+      a += 0x9E3779B9u; b += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+  }
+};
+
+// 52-bit uniform in (0,1): u = (k + 1/2) 2^-52, k = (a >> 6) 2^26 + (b >> 6).  Built without an
+// integer->double conversion: 1.k (binary) = 1 + k 2^-52 is assembled in the mantissa, and
+// adding -(1 - 2^-53) is exact because (2k + 1) 2^-53 is representable.
+__device__ __forceinline__ double u52(uint32_t a, uint32_t b) {
+  const uint32_t hi = 0x3FF00000u | (a >> 12);
+  const uint32_t lo = ((a >> 6) << 26) | (b >> 6);
+  return __hiloint2double((int)hi, (int)lo) + (-0x1.fffffffffffffp-1);
+}
+
+// counter = (point low, point high, event, pass * 256 + word block); block j feeds dims 2j, 2j+1
+template <int D>
+__device__ __forceinline__ void draw_uniforms(const Philox& rng, uint64_t point, uint32_t event,
+                                              uint32_t pass, double (&u)[D]) {
+#pragma unroll
+  for (int j = 0; 2 * j < D; ++j) {
+    uint32_t r[4];
+    rng((uint32_t)point, (uint32_t)(point >> 32), event, pass * 256u + (uint32_t)j, r);
+    u[2 * j] = u52(r[0], r[1]);
+    if (2 * j + 1 < D) u[2 * j + 1] = u52(r[2], r[3]);
+  }
+}
+
+// ---------------------------------------------------------------------------------------
+// small fp64 helpers
+// ---------------------------------------------------------------------------------------
+// 1/x for normal, finite x well inside the exponent range (every use below): the MUFU seed
+// (relative error ~2^-20, it reads only the high word) -> one cubic step (e^3 ~ 2^-60) -> one
+// linear step for the last bits; error about 1 ulp.  No special-case branches.
+__device__ __forceinline__ double rcp_fast(double x) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double e = fma(-x, y, 1.0);
+  y = fma(y, fma(e, e, e), y);          // y (1 + e + e^2)
+  e = fma(-x, y, 1.0);
+  return fma(y, e, y);
+}
+
+// toy PDF shape product f(x1) f(x2) / A^2 = (x1 x2)^pow_x ((1-x1)(1-x2))^pow_1mx (O4)
+__device__ __forceinline__ double pdf_pair(const DevConst& c, double x1, double x2) {
+  const double xx = x1 * x2, yy = (1.0 - x1) * (1.0 - x2);
+  if (c.pdf_fast) return rsqrt(xx) * (yy * yy * yy);
+  return pow(xx, c.pdf_pow_x) * pow(yy, c.pdf_pow_1mx);
+}
+
+// E * T(E_jet; E) for x = E / E_jet, inv_x = 1 / x (O5; the factor 1/E cancels the E of the
+// jet's phase-space measure E sin(theta) dE)
+__device__ __forceinline__ double tf_times_E(const DevConst& c, double inv_x) {
+  const double z1 = fma(c.tf_a1, inv_x, c.tf_b1);
+  const double z2 = fma(c.tf_a2, inv_x, c.tf_b2);
+  return fma(c.tf_c1, exp(-z1 * z1), c.tf_c2 * exp(-z2 * z2));
+}
+
+// ---------------------------------------------------------------------------------------
+// S8. block reduction of (sum w, sum w^2): registers -> warp shuffle tree -> shared -> warp 0,
+// fixed order, so results are bitwise reproducible.
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// returns the block totals in thread 0
+__device__ __forceinline__ void block_sum2(double& s1, double& s2, double* sh /* [2 * kWarps] */) {
+  s1 = warp_sum(s1);
+  s2 = warp_sum(s2);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (lane == 0) { sh[warp] = s1; sh[kWarps + warp] = s2; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double a = 0.0, b = 0.0;
+#pragma unroll
+    for (int w = 0; w < kWarps; ++w) { a += sh[w]; b += sh[kWarps + w]; }
+    s1 = a; s2 = b;
+  }
+}
+
+}  // namespace memb200

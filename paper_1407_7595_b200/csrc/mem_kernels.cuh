@@ -1,0 +1,251 @@
+// mem_kernels.cuh -- the kernels of the hot path, templated on the process.
+//
+//   prepare_kernel    S0  one thread per event: record -> per-event constants
+//   integrate_kernel  S1-S8 (+S1v, histogram of S9): one block per (event, chunk of points)
+//   finalize_kernel   S8  per event: chunk partials -> (p, err), Eq. 5-6
+//   grid_init_kernel / refine_kernel  S9: per-event VEGAS grid (reading A14)
+//   eval_points_kernel  diagnostic: one thread per point, writes w
+#pragma once
+#include "mem_processes.cuh"
+
+namespace memb200 {
+
+enum { MODE_PLAIN = 0, MODE_GRID = 1, MODE_ADAPT = 2 };
+
+template <class P>
+__global__ void prepare_kernel(const DevConst c, const double* __restrict__ ev, int64_t n_events,
+                               double* __restrict__ ecs) {
+  const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= n_events) return;
+  double ec[P::NC];
+  P::prepare(c, ev, n_events, e, ec);
+  for (int k = 0; k < P::NC; ++k) ecs[e * P::NC + k] = ec[k];
+}
+
+// S1v: warp the unit-cube point through the event's grid (edges in shared memory)
+template <int D>
+__device__ __forceinline__ double vegas_map(const double* edges, int B, double (&u)[D], int (&k)[D]) {
+  double jac = 1.0;
+  const double Bd = (double)B;
+#pragma unroll
+  for (int d = 0; d < D; ++d) {
+    const double y = u[d] * Bd;
+    int kk = (int)y;
+    kk = kk > B - 1 ? B - 1 : kk;
+    const double* x = edges + d * (B + 1);
+    const double x0 = x[kk], width = x[kk + 1] - x0;
+    u[d] = fma(y - (double)kk, width, x0);
+    jac *= Bd * width;
+    k[d] = kk;
+  }
+  return jac;
+}
+
+// histogram of w^2 by bin, one private copy per warp.  Lanes that hit the same bin are found
+// with match.any; the lowest such lane adds its peers' values in ascending lane order and does
+// the single (conflict-free) update, so the sum order is fixed and the result reproducible.
+__device__ __forceinline__ void warp_hist_add(double* wh, int k, double v) {
+  const unsigned full = 0xffffffffu;
+  const unsigned peers = __match_any_sync(full, k);
+  const int lane = threadIdx.x & 31;
+  const int leader = __ffs(peers) - 1;
+  unsigned rem = (lane == leader) ? (peers & (peers - 1u)) : 0u;
+  double acc = v;
+  while (__any_sync(full, rem != 0u)) {
+    const int src = rem ? (__ffs(rem) - 1) : lane;
+    const double t = __shfl_sync(full, v, src);
+    if (rem) { acc += t; rem &= rem - 1u; }
+  }
+  if (lane == leader && k >= 0) wh[k] += acc;
+}
+
+// One block per (event, chunk).  Thread t takes points chunk_lo + t, + kThreads, ... ; partial
+// sums go registers -> warp shuffle -> shared -> partials[event][chunk] in a fixed order.
+// MODE_GRID/ADAPT: grids = [n_events][D][B+1].  MODE_ADAPT also writes the block's histogram
+// of w^2 to hist[event][chunk][D][B].
+template <class P, int MODE>
+__global__ void __launch_bounds__(kThreads)
+integrate_kernel(const DevConst c, const double* __restrict__ ecs, const double* __restrict__ grids,
+                 double* __restrict__ partials, double* __restrict__ hist, int64_t n_points,
+                 int64_t chunk, int n_chunks, uint64_t seed, uint64_t event_offset, uint32_t pass) {
+  constexpr int D = P::D;
+  extern __shared__ double smem[];
+  double* ec = smem;                                  // [NC]
+  double* red = ec + P::NC;                           // [2 kWarps]
+  double* edges = red + 2 * kWarps;                   // [D][B+1]          (GRID, ADAPT)
+  const int B = c.vegas_bins;
+  double* whist = edges + D * (B + 1);                // [kWarps][D][B]    (ADAPT)
+
+  const int64_t e = blockIdx.x / n_chunks;
+  const int ch = (int)(blockIdx.x - e * n_chunks);
+  for (int k = threadIdx.x; k < P::NC; k += kThreads) ec[k] = ecs[e * P::NC + k];
+  if (MODE != MODE_PLAIN)
+    for (int k = threadIdx.x; k < D * (B + 1); k += kThreads) edges[k] = grids[e * D * (B + 1) + k];
+  if (MODE == MODE_ADAPT)
+    for (int k = threadIdx.x; k < kWarps * D * B; k += kThreads) whist[k] = 0.0;
+  __syncthreads();
+
+  const Philox rng{(uint32_t)seed, (uint32_t)(seed >> 32)};
+  const uint32_t ev_ctr = (uint32_t)(event_offset + (uint64_t)e);
+  const int64_t lo = (int64_t)ch * chunk;
+  const int64_t hi = (lo + chunk < n_points) ? lo + chunk : n_points;
+  double s1 = 0.0, s2 = 0.0;
+  double* wh = whist + (threadIdx.x >> 5) * D * B;
+  // uniform trip count across the block so that the warp-wide histogram update is convergent
+  for (int64_t base = lo; base < hi; base += kThreads) {
+    const int64_t i = base + threadIdx.x;
+    const bool live = i < hi;
+    double u[D];
+    draw_uniforms<D>(rng, (uint64_t)i, ev_ctr, pass, u);
+    double w;
+    if (MODE == MODE_PLAIN) {
+      w = P::weight(c, ec, u);
+    } else {
+      int k[D];
+      const double jac = vegas_map<D>(edges, B, u, k);
+      w = jac * P::weight(c, ec, u);
+      if (!isfinite(w)) w = 0.0;
+      if (MODE == MODE_ADAPT) {
+        const double w2 = live ? w * w : 0.0;
+#pragma unroll
+        for (int d = 0; d < D; ++d) warp_hist_add(wh + d * B, live ? k[d] : -1 - (int)(threadIdx.x & 31), w2);
+      }
+    }
+    if (live) { s1 += w; s2 = fma(w, w, s2); }
+  }
+  block_sum2(s1, s2, red);
+  if (threadIdx.x == 0) {
+    partials[2 * (size_t)blockIdx.x] = s1;
+    partials[2 * (size_t)blockIdx.x + 1] = s2;
+  }
+  if (MODE == MODE_ADAPT) {
+    __syncthreads();
+    for (int k = threadIdx.x; k < D * B; k += kThreads) {
+      double a = 0.0;
+#pragma unroll
+      for (int w = 0; w < kWarps; ++w) a += whist[w * D * B + k];
+      hist[(size_t)blockIdx.x * D * B + k] = a;
+    }
+  }
+}
+
+// O1 (PAPER.md:76 Eq. 5, :80 Eq. 6, reading A1): p = sum w / N, err = sqrt(max(0, <w^2> - p^2)/(N-1))
+__global__ void finalize_kernel(const double* __restrict__ partials, int n_chunks, int64_t n_events,
+                                int64_t n_points, double* __restrict__ out_p, double* __restrict__ out_err) {
+  const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= n_events) return;
+  double s1 = 0.0, s2 = 0.0;
+  for (int ch = 0; ch < n_chunks; ++ch) {
+    s1 += partials[2 * ((size_t)e * n_chunks + ch)];
+    s2 += partials[2 * ((size_t)e * n_chunks + ch) + 1];
+  }
+  const double N = (double)n_points;
+  const double m = s1 / N;
+  double var = s2 / N - m * m;
+  if (var < 0.0) var = 0.0;
+  out_p[e] = m;
+  out_err[e] = sqrt(var / (N - 1.0));
+}
+
+__global__ void grid_init_kernel(double* __restrict__ grids, int64_t n_events, int D, int B) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_events * D * (B + 1)) return;
+  const int j = (int)(i % (B + 1));
+  grids[i] = (double)j / (double)B;
+}
+
+// S9, one block per event, blockDim = (64, D): thread (k, d).  Sum the chunk histograms in chunk
+// order, smooth (1,6,1)/8, normalise, compress r <- ((1-r)/ln(1/r))^alpha, then re-bin to the
+// j/B quantiles of the piecewise-constant density r on the old bins (reading A14).
+__global__ void refine_kernel(const DevConst c, const double* __restrict__ hist, int n_chunks,
+                              double* __restrict__ grids, int D) {
+  const int B = c.vegas_bins;
+  __shared__ double h[kMaxDims][kMaxBins], r[kMaxDims][kMaxBins], tot[kMaxDims], nx[kMaxDims][kMaxBins + 1];
+  const int k = threadIdx.x, d = threadIdx.y;
+  const int64_t e = blockIdx.x;
+  double* x = grids + (e * D + d) * (B + 1);
+  if (k < B) {
+    double a = 0.0;
+    for (int ch = 0; ch < n_chunks; ++ch) a += hist[(((size_t)e * n_chunks + ch) * D + d) * B + k];
+    r[d][k] = a;                                      // raw histogram
+  }
+  __syncthreads();
+  if (k < B) {
+    double s;
+    if (B == 1) s = r[d][0];
+    else if (k == 0) s = (7.0 * r[d][0] + r[d][1]) / 8.0;
+    else if (k == B - 1) s = (r[d][B - 2] + 7.0 * r[d][B - 1]) / 8.0;
+    else s = (r[d][k - 1] + 6.0 * r[d][k] + r[d][k + 1]) / 8.0;
+    h[d][k] = s;
+  }
+  __syncthreads();
+  if (k == 0) {
+    double t = 0.0;
+    for (int j = 0; j < B; ++j) t += h[d][j];
+    tot[d] = t;
+  }
+  __syncthreads();
+  const double t = tot[d];
+  const bool ok = (t > 0.0) && isfinite(t);           // otherwise leave the grid
+  if (k < B && ok) {
+    const double rk = h[d][k] / t;
+    double v;
+    if (rk <= 0.0) v = 0.0;
+    else if (rk >= 1.0) v = 1.0;
+    else v = pow((1.0 - rk) / log(1.0 / rk), c.vegas_alpha);
+    r[d][k] = v;
+  }
+  __syncthreads();
+  if (k == 0 && ok) {
+    double rsum = 0.0;
+    for (int j = 0; j < B; ++j) rsum += r[d][j];
+    const double per = rsum / (double)B;
+    double acc = 0.0;
+    int kk = 0;
+    nx[d][0] = x[0]; nx[d][B] = x[B];
+    for (int j = 1; j < B; ++j) {
+      const double target = (double)j * per;
+      while (kk < B - 1 && acc + r[d][kk] < target) { acc += r[d][kk]; ++kk; }
+      double frac = (r[d][kk] > 0.0) ? (target - acc) / r[d][kk] : 0.0;
+      frac = frac < 0.0 ? 0.0 : (frac > 1.0 ? 1.0 : frac);
+      nx[d][j] = x[kk] + frac * (x[kk + 1] - x[kk]);
+    }
+  }
+  __syncthreads();
+  if (ok)
+    for (int j = k; j <= B; j += blockDim.x) x[j] = nx[d][j];
+}
+
+// diagnostic: weights of points [first, first + n) of one event
+template <class P>
+__global__ void eval_points_kernel(const DevConst c, const double* __restrict__ ecs, int64_t event,
+                                   const double* __restrict__ grid, int64_t first, int64_t n,
+                                   uint64_t seed, uint64_t event_offset, uint32_t pass,
+                                   double* __restrict__ out_w) {
+  constexpr int D = P::D;
+  extern __shared__ double smem[];
+  double* ec = smem;
+  double* edges = ec + P::NC;
+  const int B = c.vegas_bins;
+  for (int k = threadIdx.x; k < P::NC; k += blockDim.x) ec[k] = ecs[event * P::NC + k];
+  if (grid)
+    for (int k = threadIdx.x; k < D * (B + 1); k += blockDim.x) edges[k] = grid[k];
+  __syncthreads();
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const Philox rng{(uint32_t)seed, (uint32_t)(seed >> 32)};
+  double u[D];
+  draw_uniforms<D>(rng, (uint64_t)(first + i), (uint32_t)(event_offset + (uint64_t)event), pass, u);
+  double w;
+  if (grid) {
+    int k[D];
+    const double jac = vegas_map<D>(edges, B, u, k);
+    w = jac * P::weight(c, ec, u);
+    if (!isfinite(w)) w = 0.0;
+  } else {
+    w = P::weight(c, ec, u);
+  }
+  out_w[i] = w;
+}
+
+}  // namespace memb200
