@@ -1,0 +1,327 @@
+#!/usr/bin/env python
+"""Benchmark of the hot path.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl reference]
+
+One step = one pass of the whole hot path (S0-S8, plus S1v/S9 for config 5) over one batch of
+seeded synthetic events: mem_integrate on BASELINE.json's configs[2] by default (4096 t tbar
+lepton+jets events x 2^20 points, 6-D, fp64 -- the configuration north_star's target is quoted
+on).  Rank 0 prints ONE JSON line.  With N > 1 (torchrun) every rank integrates its own shard of
+4096 events of a 4096*N list (weak scaling, no data-path collective); the time is the max over
+ranks.
+
+--impl reference times the CPU oracle as it stands on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+SEED = 20140729
+
+# Algorithmic FP64 work per integrand call of the dominant kernel: executed
+# thread-level DFMA / DMUL / DADD per point, from the ncu capture in profiles/ (r01_ncu_config3.md):
+# smsp__sass_thread_inst_executed_op_{dfma,dmul,dadd}_pred_on.sum / points.  flop = 2 DFMA + DMUL + DADD.
+FP64_PER_CALL = {
+    3: {"dfma": 268.0, "dmul": 86.0, "dadd": 77.0},
+}
+NOMINAL_FP64_FMA_PER_CLK_PER_SM = 64      # 4 SMSPs x 16 lanes; confirmed by the microbenchmark
+VEGAS_ITERS, VEGAS_POINTS = 5, 1 << 17    # BASELINE.json:configs[4]
+
+
+def flops_per_call(cfg):
+    c = FP64_PER_CALL[3 if cfg == 5 else cfg]
+    return 2.0 * c["dfma"] + c["dmul"] + c["dadd"]
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 5])
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--events", type=int, default=0, help="override the event count (default: the config's)")
+    ap.add_argument("--points", type=int, default=0, help="override points/event (default: the config's)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def workload(cfg, args):
+    from paper_1407_7595_b200 import workloads as wl
+    proc, ne, npts = wl.CONFIGS[3 if cfg == 5 else cfg]
+    if args.events:
+        ne = args.events
+    if args.points:
+        npts = args.points
+    name = {1: "config1 W->e nu 1-D", 2: "config2 Z->bb 2-D", 3: "config3 ttbar l+jets 6-D",
+            5: "config5 ttbar l+jets 6-D + VEGAS 5x2^17"}[cfg]
+    return proc, ne, npts, "%s, %d events x %d points/event, fp64" % (name, ne, npts)
+
+
+# --------------------------------------------------------------------------------------------
+# clocks during the timed region
+# --------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            out, _ = self.proc.communicate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 6:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# --------------------------------------------------------------------------------------------
+# CPU oracle legs
+# --------------------------------------------------------------------------------------------
+def _oracle_worker(job):
+    cfg, proc, ev, lo, n_points, seed = job
+    import oracle
+    p = oracle.params_default(proc)
+    t0 = time.perf_counter()
+    if cfg == 5:
+        p.vegas_iters, p.vegas_points = VEGAS_ITERS, VEGAS_POINTS
+        oracle.vegas_integrate(proc, p, ev, n_points, seed, event_offset=lo)
+        evals = ev.shape[1] * (n_points + VEGAS_ITERS * VEGAS_POINTS)
+    else:
+        oracle.integrate(proc, p, ev, n_points, seed, event_offset=lo)
+        evals = ev.shape[1] * n_points
+    return evals, time.perf_counter() - t0
+
+
+def oracle_sample(cfg, proc, ev, n_points, events_per_core, pool, cores):
+    """The oracle, single-threaded by design, run as `cores` independent processes over disjoint
+    event ranges.  Returns (evaluations, wall seconds, events)."""
+    jobs = []
+    for k in range(cores):
+        lo = k * events_per_core
+        jobs.append((cfg, proc, ev[:, lo:lo + events_per_core].copy(), lo, n_points, SEED))
+    t0 = time.perf_counter()
+    res = pool.map(_oracle_worker, jobs)
+    wall = time.perf_counter() - t0
+    return sum(r[0] for r in res), wall, cores * events_per_core
+
+
+def run_reference(args):
+    import multiprocessing as mp
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_1407_7595_b200 import workloads as wl
+    import oracle
+    oracle.build()
+    cfg = args.config
+    proc, ne, n_points, name = workload(cfg, args)
+    cores = min(os.cpu_count() or 1, 64)
+    per_core = 1 if n_points >= (1 << 20) else max(1, (1 << 20) // n_points)
+    per_core = min(per_core, max(1, ne // cores))
+    ev = wl.make_events(proc, ne)
+    with mp.get_context("spawn").Pool(cores) as pool:
+        for _ in range(args.warmup):
+            oracle_sample(cfg, proc, ev, n_points, per_core, pool, cores)
+        evals = wall = events = 0
+        for _ in range(args.steps):
+            a, b, c = oracle_sample(cfg, proc, ev, n_points, per_core, pool, cores)
+            evals += a; wall += b; events += c
+    value = evals / wall
+    sample = "%d events (%d per core) x %d points/event per step" % (cores * per_core, per_core, n_points)
+    line = {
+        "impl": "reference", "metric": "integrand_evals_per_s", "value": value, "unit": "evals/s",
+        "events_per_s": events / wall, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * wall / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": {"workload": name, "sample": sample},
+        "cpu_baseline": {"value": value, "unit": "evals/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "evals/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# --------------------------------------------------------------------------------------------
+# the CUDA path
+# --------------------------------------------------------------------------------------------
+def run_b200(args):
+    import torch
+
+    import paper_1407_7595_b200 as mem
+    from paper_1407_7595_b200 import sharding
+    from paper_1407_7595_b200 import workloads as wl
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
+    rank, local_rank, world = sharding.dist_env()
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        sharding.init_process_group("nccl")
+    import torch.distributed as dist
+
+    cfg = args.config
+    proc, ne, n_points, name = workload(cfg, args)
+    # weak scaling: every rank owns `ne` events of a list of ne * world (contiguous shard)
+    ev_all = wl.make_events(proc, ne * world)
+    lo = rank * ne
+    ev_host = torch.from_numpy(ev_all[:, lo:lo + ne].copy()).pin_memory()
+    ev_dev = ev_host.cuda()
+    over = dict(vegas_iters=VEGAS_ITERS, vegas_points=VEGAS_POINTS) if cfg == 5 else {}
+    it = mem.Integrator(proc, **over)
+    it.set_event_offset(lo)
+    out_p = torch.empty(ne, dtype=torch.float64, device="cuda")
+    out_err = torch.empty_like(out_p)
+    hp = torch.empty(ne, dtype=torch.float64).pin_memory()
+    he = torch.empty(ne, dtype=torch.float64).pin_memory()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")       # > 126 MB L2
+    evals_per_step = ne * (n_points + (VEGAS_ITERS * VEGAS_POINTS if cfg == 5 else 0))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, steps, collect_kernel=False):
+        """time exactly `steps` steps: per-step CUDA events on torch's current stream (the stream
+        the library launches on), L2 flushed between steps outside the event pairs"""
+        ms, kms = [], []
+        for _ in range(steps):
+            flush.fill_(0)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            fn()
+            b.record()
+            b.synchronize()
+            ms.append(a.elapsed_time(b))
+            if collect_kernel:
+                kms.append(it.last_pass_ms()[0])
+        return ms, kms
+
+    def step_dev():
+        it.integrate(ev_dev, n_points, SEED, out_p=out_p, out_err=out_err)
+
+    def step_host():
+        it.integrate_host(ev_host, n_points, SEED, out_p=hp, out_err=he)
+
+    for _ in range(max(args.warmup, 3)):
+        step_dev()
+    step_host()
+    barrier()
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    launches0 = it.launches
+    barrier()
+    ms, kms = timed(step_dev, args.steps, collect_kernel=True)
+    barrier()
+    launches = it.launches - launches0
+    clocks = sampler.stop() if sampler else None
+    t_dev = sharding.max_over_ranks(sum(ms) / 1e3, device="cuda")
+    barrier()
+    ms_h, _ = timed(step_host, args.steps)
+    barrier()
+    t_host = sharding.max_over_ranks(sum(ms_h) / 1e3, device="cuda")
+
+    if rank != 0:
+        it.close()
+        return
+
+    total_evals = evals_per_step * world * args.steps
+    value = total_evals / t_dev
+    # roofline of the dominant kernel (the integrate pass that produces the outputs)
+    k_ms = sum(kms) / len(kms)
+    k_evals = ne * n_points
+    peak_meas = mem.mem_measure_fp64_peak(5)
+    fl = flops_per_call(cfg)
+    achieved = k_evals * fl / (k_ms * 1e-3) / 1e12
+    c = FP64_PER_CALL[3 if cfg == 5 else cfg]
+    pipe_inst = c["dfma"] + c["dmul"] + c["dadd"]
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    sm_mhz = (clocks or {}).get("sm_mhz") or 0.0
+    roofline = {
+        "bound": "alu", "kernel": "integrate_kernel<%s>" % ("ProcTTljets,GRID" if cfg == 5 else "proc%d,PLAIN" % proc),
+        "achieved": achieved, "peak": peak_meas, "unit": "TFLOP/s", "frac": achieved / peak_meas,
+        "peak_source": "measured in this run: independent DFMA chains on all SMs (mem_measure_fp64_peak)",
+        "peak_nominal_at_observed_clock": 2e-6 * NOMINAL_FP64_FMA_PER_CLK_PER_SM * sms * sm_mhz,
+        "fp64_pipe_frac": (k_evals * pipe_inst / (k_ms * 1e-3)) / (peak_meas * 1e12 / 2.0),
+        "flop_per_call": fl, "fp64_inst_per_call": pipe_inst, "kernel_ms": k_ms,
+        "kernel_share_of_step": k_ms * len(kms) / sum(ms),
+        "traffic": None,
+        "hbm_gbs_event_result_path": (ne * mem.mem_event_fields(proc) * 8 + ne * 16) / (sum(ms) / len(ms) * 1e-3) / 1e9,
+    }
+    h2d = ne * mem.mem_event_fields(proc) * 8
+    d2h = 2 * ne * 8
+    line = {
+        "metric": "integrand_evals_per_s", "value": value, "unit": "evals/s",
+        "events_per_s": ne * world * args.steps / t_dev,
+        "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": 1e3 * t_dev / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": name, "events_per_gpu": ne, "points_per_event": n_points, "seed": SEED,
+                   "l2": "flushed between timed steps (256 MiB fill); inputs are 0.5 MB",
+                   "parallelism": "events sharded over %d GPU(s), no collective" % world},
+        "clocks": clocks,
+        "e2e": {"value": total_evals / t_host, "unit": "evals/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "ms_per_step": 1e3 * t_host / args.steps, "entry": "mem_integrate_host (pinned host buffers)"},
+        "gpu_launches": launches,
+        "roofline": roofline,
+    }
+    it.close()
+    if world == 1 and not args.no_cpu_baseline:
+        import multiprocessing as mp
+        import oracle
+        oracle.build()
+        cores = min(os.cpu_count() or 1, 64)
+        per_core = 8 if n_points >= (1 << 20) else max(1, (8 << 20) // n_points)
+        per_core = max(1, min(per_core, ne // cores))
+        with mp.get_context("spawn").Pool(cores) as pool:
+            evals, wall, events = oracle_sample(cfg, proc, ev_all, n_points, per_core, pool, cores)
+        line["cpu_baseline"] = {"value": evals / wall, "unit": "evals/s", "cores": cores, "kind": "oracle",
+                                "events_per_s": events / wall, "seconds": wall,
+                                "sample": "first %d events (%d per core) x %d points/event of the same workload"
+                                          % (events, per_core, n_points)}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_b200(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -132,6 +132,17 @@ mem_status mem_get_grid(mem_handle* h, int64_t n_events, double* out_grid, void*
 /* Kernels launched by this handle since creation (for the benchmark's launch count). */
 int64_t mem_launch_count(const mem_handle* h);
 
+/* Measurement support.  Every mem_integrate records CUDA events on
+ * its stream around the dominant kernel, i.e. the integrate pass that produces the outputs.
+ * mem_last_pass_ms waits for that pass and returns its duration in *ms (host, out) and the
+ * number of integrand evaluations it made in *evals (host, out; may be NULL). */
+mem_status mem_last_pass_ms(mem_handle* h, double* ms, int64_t* evals);
+
+/* FP64 FMA peak of the current device, measured with independent DFMA chains on all SMs:
+ * *tflops (host, out) = 2 * fused multiply-adds / second / 1e12, best of `repeats` launches.
+ * The denominator of the "alu" roofline (MEASURED_PEAKS.json has no FP64 figure). */
+mem_status mem_measure_fp64_peak(int32_t repeats, double* tflops, void* cuda_stream);
+
 /* Thread-local description of the last error on this thread ("" if none). */
 const char* mem_last_error(void);
 

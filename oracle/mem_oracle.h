@@ -73,12 +73,18 @@ void   orc_boost_transverse(const double P[4], int n, double* mom /* n x 4, in p
 /* --- the integrand: one event record (n_fields doubles), one unit-cube point --- */
 /* dbg (may be NULL): [0]=n_sol, [1..]= per solution: x1, x2, then the boosted final momenta. */
 double orc_weight(int process, const orc_params* p, const double* rec, const double* u, double* dbg);
+/* Extended-precision referee: the same templates instantiated in long double (x87, 64-bit
+ * mantissa), result rounded to double.  Used by the tests to adjudicate ill-conditioned points. */
+double orc_weight_x(int process, const orc_params* p, const double* rec, const double* u);
 
 /* events: SoA, field-major [n_fields][n_events].  grid (may be NULL) = VEGAS edges
  * [n_events][D][bins+1]; then u is warped through it first. */
 int orc_eval_points(int process, const orc_params* p, const double* events, int64_t n_events,
                     int64_t event, uint64_t event_offset, int64_t first_point, int64_t n,
                     uint64_t seed, int32_t iteration, const double* grid, double* out_w);
+int orc_eval_points_x(int process, const orc_params* p, const double* events, int64_t n_events,
+                      int64_t event, uint64_t event_offset, int64_t first_point, int64_t n,
+                      uint64_t seed, int32_t iteration, double* out_w);
 int orc_integrate(int process, const orc_params* p, const double* events, int64_t n_events,
                   uint64_t event_offset, int64_t n_points, uint64_t seed,
                   double* out_p, double* out_err);

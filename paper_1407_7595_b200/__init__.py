@@ -19,7 +19,7 @@ MEM_PROC_W_ENU, MEM_PROC_Z_BB, MEM_PROC_TT_LJETS, MEM_PROC_TT_DILEP = 1, 2, 3, 4
 
 EXPORTS = ("mem_params_default", "mem_event_fields", "mem_n_dims", "mem_create", "mem_destroy",
            "mem_set_event_offset", "mem_integrate", "mem_integrate_host", "mem_eval_points",
-           "mem_get_grid", "mem_launch_count", "mem_last_error")
+           "mem_get_grid", "mem_launch_count", "mem_last_error", "mem_last_pass_ms", "mem_measure_fp64_peak")
 
 
 class mem_params(C.Structure):
@@ -67,6 +67,8 @@ def lib():
         L.mem_get_grid.argtypes = [vp, i64, dp, vp]
         L.mem_launch_count.argtypes = [vp]
         L.mem_launch_count.restype = i64
+        L.mem_last_pass_ms.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
+        L.mem_measure_fp64_peak.argtypes = [C.c_int32, C.POINTER(C.c_double), vp]
         L.mem_last_error.argtypes = []
         L.mem_last_error.restype = C.c_char_p
         _lib = L
@@ -112,6 +114,20 @@ def mem_set_event_offset(handle, first_event: int) -> None:
 
 def mem_launch_count(handle) -> int:
     return int(lib().mem_launch_count(handle))
+
+
+def mem_last_pass_ms(handle):
+    """(milliseconds, integrand evaluations) of the dominant kernel of the last mem_integrate."""
+    ms, ev = C.c_double(), C.c_int64()
+    _check(lib().mem_last_pass_ms(handle, C.byref(ms), C.byref(ev)))
+    return ms.value, ev.value
+
+
+def mem_measure_fp64_peak(repeats: int = 5, stream=None) -> float:
+    """Measured FP64 FMA peak of the current device in TFLOP/s."""
+    t = C.c_double()
+    _check(lib().mem_measure_fp64_peak(int(repeats), C.byref(t), _stream_ptr(stream)))
+    return t.value
 
 
 def _stream_ptr(stream):
@@ -212,6 +228,9 @@ class Integrator:
 
     def set_event_offset(self, first_event):
         mem_set_event_offset(self.handle, first_event)
+
+    def last_pass_ms(self):
+        return mem_last_pass_ms(self.handle)
 
     @property
     def launches(self):

@@ -75,6 +75,8 @@ struct mem_handle {
   int64_t launches;
   int64_t grid_events;      // events covered by the grids of the last VEGAS call
   Buffer ecs, partials, grids, hist, stage_in, stage_out;
+  cudaEvent_t ev_begin, ev_end;  // around the dominant kernel of the last mem_integrate
+  int64_t last_evals;            // integrand evaluations of that kernel; 0 = none yet
 };
 
 namespace {
@@ -210,6 +212,18 @@ mem_status launch_pass(mem_handle* h, int64_t n_events, int64_t n_points, int64_
   return MEM_OK;
 }
 
+// the pass that produces the outputs, bracketed by the handle's events
+template <class P, int MODE>
+mem_status launch_timed_pass(mem_handle* h, int64_t n_events, int64_t n_points, int n_chunks, uint64_t seed,
+                             uint32_t pass, cudaStream_t st) {
+  CUDA_TRY(cudaEventRecord(h->ev_begin, st));
+  mem_status s = launch_pass<P, MODE>(h, n_events, n_points, kChunk, n_chunks, seed, pass, st);
+  if (s != MEM_OK) return s;
+  CUDA_TRY(cudaEventRecord(h->ev_end, st));
+  h->last_evals = n_events * n_points;
+  return MEM_OK;
+}
+
 template <class P>
 mem_status integrate_impl(mem_handle* h, const double* events, int64_t n_events, int64_t n_points, uint64_t seed,
                           double* out_p, double* out_err, cudaStream_t st) {
@@ -247,9 +261,9 @@ mem_status integrate_impl(mem_handle* h, const double* events, int64_t n_events,
       CUDA_TRY(cudaGetLastError());
     }
     h->grid_events = n_events;
-    s = launch_pass<P, MODE_GRID>(h, n_events, n_points, kChunk, n_chunks, seed, (uint32_t)p.vegas_iters, st);
+    s = launch_timed_pass<P, MODE_GRID>(h, n_events, n_points, n_chunks, seed, (uint32_t)p.vegas_iters, st);
   } else {
-    s = launch_pass<P, MODE_PLAIN>(h, n_events, n_points, kChunk, n_chunks, seed, 0u, st);
+    s = launch_timed_pass<P, MODE_PLAIN>(h, n_events, n_points, n_chunks, seed, 0u, st);
   }
   if (s != MEM_OK) return s;
   finalize_kernel<<<(unsigned)((n_events + 127) / 128), 128, 0, st>>>((const double*)h->partials.p, n_chunks,
@@ -324,7 +338,13 @@ mem_status mem_create(mem_process process, const mem_params* params, mem_handle*
   mem_handle* h = new (std::nothrow) mem_handle();
   if (!h) return fail(MEM_ERR_NOMEM, "out of host memory");
   h->process = (int)process; h->device = dev; h->params = p; h->dc = make_dev_const(p);
-  h->event_offset = 0; h->launches = 0; h->grid_events = 0;
+  h->event_offset = 0; h->launches = 0; h->grid_events = 0; h->last_evals = 0;
+  cudaError_t ce = cudaEventCreate(&h->ev_begin);
+  if (ce == cudaSuccess) ce = cudaEventCreate(&h->ev_end);
+  if (ce != cudaSuccess) {
+    delete h;
+    return fail(MEM_ERR_CUDA, "cudaEventCreate: %s", cudaGetErrorString(ce));
+  }
   *out = h;
   return MEM_OK;
 }
@@ -335,6 +355,8 @@ mem_status mem_destroy(mem_handle* h) {
   Buffer* bs[] = {&h->ecs, &h->partials, &h->grids, &h->hist, &h->stage_in, &h->stage_out};
   for (Buffer* b : bs)
     if (b->p) cudaFree(b->p);
+  cudaEventDestroy(h->ev_begin);
+  cudaEventDestroy(h->ev_end);
   delete h;
   return MEM_OK;
 }
@@ -346,6 +368,49 @@ mem_status mem_set_event_offset(mem_handle* h, uint64_t first_event) {
 }
 
 int64_t mem_launch_count(const mem_handle* h) { return h ? h->launches : -1; }
+
+mem_status mem_last_pass_ms(mem_handle* h, double* ms, int64_t* evals) {
+  if (!h || !ms) return fail(MEM_ERR_INVALID_ARG, "handle / ms is NULL");
+  if (h->last_evals == 0) return fail(MEM_ERR_INVALID_ARG, "no mem_integrate has run on this handle");
+  CUDA_TRY(cudaEventSynchronize(h->ev_end));
+  float f = 0.f;
+  CUDA_TRY(cudaEventElapsedTime(&f, h->ev_begin, h->ev_end));
+  *ms = (double)f;
+  if (evals) *evals = h->last_evals;
+  return MEM_OK;
+}
+
+mem_status mem_measure_fp64_peak(int32_t repeats, double* tflops, void* cuda_stream) {
+  if (!tflops || repeats < 1) return fail(MEM_ERR_INVALID_ARG, "tflops is NULL or repeats < 1");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int dev = 0, sms = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  double* sink = nullptr;
+  CUDA_TRY(cudaMalloc(&sink, sizeof(double)));
+  cudaEvent_t a, b;
+  CUDA_TRY(cudaEventCreate(&a));
+  CUDA_TRY(cudaEventCreate(&b));
+  const int blocks = sms * 8 * 4, threads = 256;           // 4 waves of 8 resident blocks per SM
+  double best = 0.0;
+  for (int r = 0; r < repeats + 1; ++r) {                  // first launch is the warm-up
+    cudaEventRecord(a, st);
+    fp64_peak_kernel<<<blocks, threads, 0, st>>>(sink, 0.999999, 1e-9);
+    cudaEventRecord(b, st);
+    cudaError_t e = cudaEventSynchronize(b);
+    float ms = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, a, b);
+    if (e != cudaSuccess) {
+      cudaFree(sink); cudaEventDestroy(a); cudaEventDestroy(b);
+      return fail(MEM_ERR_CUDA, "fp64 peak kernel: %s", cudaGetErrorString(e));
+    }
+    const double flops = 2.0 * 8.0 * kPeakIters * (double)threads * (double)blocks;
+    if (r > 0 && flops / (ms * 1e-3) / 1e12 > best) best = flops / (ms * 1e-3) / 1e12;
+  }
+  cudaFree(sink); cudaEventDestroy(a); cudaEventDestroy(b);
+  *tflops = best;
+  return MEM_OK;
+}
 
 mem_status mem_integrate(mem_handle* h, const double* events, int64_t n_events, int64_t n_points, uint64_t seed,
                          double* out_p, double* out_err, void* cuda_stream) {

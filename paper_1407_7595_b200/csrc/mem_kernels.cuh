@@ -248,4 +248,18 @@ __global__ void eval_points_kernel(const DevConst c, const double* __restrict__ 
   out_w[i] = w;
 }
 
+// FP64 peak microbenchmark: 8 independent DFMA chains per thread, kPeakIters x 8 FMAs each.
+constexpr int kPeakIters = 4096;
+__global__ void __launch_bounds__(256) fp64_peak_kernel(double* __restrict__ sink, double a, double b) {
+  double x0 = threadIdx.x, x1 = x0 + 1.0, x2 = x0 + 2.0, x3 = x0 + 3.0, x4 = x0 + 4.0, x5 = x0 + 5.0, x6 = x0 + 6.0,
+         x7 = x0 + 7.0;
+#pragma unroll 8
+  for (int i = 0; i < kPeakIters; ++i) {
+    x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+    x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+  }
+  const double s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+  if (s == 12345.678) sink[0] = s;     // never true for the arguments used; keeps the chains alive
+}
+
 }  // namespace memb200

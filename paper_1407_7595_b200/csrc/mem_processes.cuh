@@ -33,7 +33,7 @@ __device__ inline double one_minus_cos(double eta_a, double phi_a, double eta_b,
 // =========================================================================================
 struct ProcWenu {
   static constexpr int D = 1, NF = 5, NC = 16;
-  enum { LM, LP, LE, LZ, PT, NT2, A, TLO, DT, CTLO, DSM, PTNT, IPT2, C0, THI_C, _N };
+  enum { LM, LP, LE, LZ, PT, NT2, A, CLO, CHI, DT, SCLO, DSM, PTNT, IPT2, C0, _N };
 
   __device__ static void prepare(const DevConst& c, const double* ev, int64_t n, int64_t e, double* ec) {
     const double pT = ev[0 * n + e], eta = ev[1 * n + e], phi = ev[2 * n + e];
@@ -49,31 +49,32 @@ struct ProcWenu {
     const double s_m = 2.0 * (lE * sqrt(nT2 + Pz * Pz) - a + lz * Pz);
     const double s_min = (nz_star > Pz) ? s_p : (nz_star < -Pz) ? s_m : s_star;
     const double s_max = fmax(s_p, s_m);
-    const double t_lo = atan((s_min - c.mW2) / c.mWGW), t_hi = atan((s_max - c.mW2) / c.mWGW);
-    const double dt = t_hi - t_lo;
+    // Breit-Wigner angle through its complement c = pi/2 - t = atan2(m Gam, s - m^2) in (0, pi):
+    // events far above the W pole have t within 1e-3 of pi/2, where t itself loses 3-4 digits
+    const double c_lo = atan2(c.mWGW, s_min - c.mW2), c_hi = atan2(c.mWGW, s_max - c.mW2);
+    const double dt = c_lo - c_hi;
     ec[LM] = pT * exp(-eta);            // E_l - l_z
     ec[LP] = pT * exp(eta);             // E_l + l_z
     ec[LE] = lE; ec[LZ] = lz; ec[PT] = pT; ec[NT2] = nT2; ec[A] = a;
-    ec[TLO] = t_lo; ec[DT] = dt; ec[CTLO] = cos(t_lo);
+    ec[CLO] = c_lo; ec[CHI] = c_hi; ec[DT] = dt; ec[SCLO] = sin(c_lo);   // sin(c_lo) = cos(t_lo)
     ec[DSM] = s_min - s_star;
     ec[PTNT] = pT * nT;
     ec[IPT2] = 1.0 / (pT * pT);
     // dt * (ds/dt * D_W = 1/(m Gam)) * g^4 |V_ud|^2 / 12 * A_q^2 * (4 / (x1 x2 S)) * (4 h^2 = S)
     //    * 1 / (8 pi^2 S E_l E_nu) * (jac = E_nu / (2 rt))
     ec[C0] = dt / c.mWGW * c.g4w * c.V_ud2 / 12.0 * c.A_q2 * 4.0 / (8.0 * kPi * kPi * c.S * lE) * 0.5;
-    ec[THI_C] = 0.0;
   }
 
   __device__ static double weight(const DevConst& c, const double* ec, const double (&u)[D]) {
-    const double du = ec[DT] * u[0];
-    const double t = ec[TLO] + du;
-    double st, ct;
-    sincos(t, &st, &ct);
-    const double smm = c.mWGW * (st / ct);
+    // pi/2 - t = c_lo (1 - u) + c_hi u: positive terms only (1 - u is exact)
+    const double cc_t = fma(ec[CLO], 1.0 - u[0], ec[CHI] * u[0]);
+    double sc, cs;
+    sincos(cc_t, &sc, &cs);
+    const double smm = c.mWGW * (cs / sc);            // m Gam tan t = m Gam cot(pi/2 - t)
     const double sW = c.mW2 + smm;
     // s_W - s_min = m Gam (tan t - tan t_lo) = m Gam sin(dt u) / (cos t cos t_lo): no cancellation
     // at the transverse-mass edge
-    const double ds = c.mWGW * sin(du) / (ct * ec[CTLO]);
+    const double ds = c.mWGW * sin(ec[DT] * u[0]) / (sc * ec[SCLO]);
     const double half = 0.5 * (ds + ec[DSM]);
     const double cc = 0.5 * sW + ec[A];
     const double disc = half * (cc + ec[PTNT]);
@@ -125,34 +126,42 @@ __device__ __forceinline__ Jet jet_point(const DevConst& c, const double* o, dou
 // =========================================================================================
 struct ProcZbb {
   static constexpr int D = 2, NF = 6, NC = 12;
-  enum { J0 = 0, J1 = 5, C0 = 10 };
+  enum { J0 = 0, J1 = 5, C0 = 10, KT = 11 };
 
   __device__ static void prepare(const DevConst& c, const double* ev, int64_t n, int64_t e, double* ec) {
-    double vol = 1.0, sth = 1.0;
+    double vol = 1.0, sth = 1.0, eta[2], phi[2];
     for (int j = 0; j < 2; ++j) {
-      const double Ej = ev[(3 * j) * n + e], eta = ev[(3 * j + 1) * n + e], phi = ev[(3 * j + 2) * n + e];
-      jet_prepare(c, Ej, eta, phi, ec + 5 * j);
+      const double Ej = ev[(3 * j) * n + e];
+      eta[j] = ev[(3 * j + 1) * n + e]; phi[j] = ev[(3 * j + 2) * n + e];
+      jet_prepare(c, Ej, eta[j], phi[j], ec + 5 * j);
       vol *= Ej * c.dr;
-      sth *= (1.0 / cosh(eta)) / (2.0 * kTwoPi3);
+      sth *= (1.0 / cosh(eta[j])) / (2.0 * kTwoPi3);
     }
+    // 1 - n1T.n2T = (cosh eta1 cosh eta2 - cos dphi)/(cosh eta1 cosh eta2), as a sum of squares
+    const double sp = sinh(0.5 * (eta[0] + eta[1])), sm = sinh(0.5 * (eta[0] - eta[1])), sn = sin(0.5 * (phi[0] - phi[1]));
+    ec[KT] = (sp * sp + sm * sm + 2.0 * sn * sn) / (cosh(eta[0]) * cosh(eta[1]));
+    // the slot n_y of jet 0 is not needed: it holds K12 = 1 - n1.n2
+    ec[J0 + 3] = one_minus_cos(eta[0], phi[0], eta[1], phi[1]);
     // vol * prod sin(theta)/(2 (2pi)^3) * (2pi)^4 * (2/S) * g_Z^4 * A_q^2 * 4 (flux) * S (u^2, t^2 carry 4 h^2)
     ec[C0] = vol * sth * kTwoPi4 * (2.0 * c.inv_S) * c.gz4 * c.A_q2 * 4.0 * c.S;
-    ec[11] = 0.0;
   }
 
   __device__ static double weight(const DevConst& c, const double* ec, const double (&u)[D]) {
     double tf = 1.0;
     const Jet p1 = jet_point(c, ec + J0, u[0], tf), p2 = jet_point(c, ec + J1, u[1], tf);
-    const double PE = p1.E + p2.E, Px = p1.x + p2.x, Py = p1.y + p2.y, Pz = p1.z + p2.z;
-    // O7: beta = P_T / P_E, gamma = 1/sqrt(1 - beta^2); only the boosted energies are needed
-    const double iPE = rcp_fast(PE);
-    const double bx = Px * iPE, by = Py * iPE;
-    const double gam = rsqrt(1.0 - (bx * bx + by * by));
-    const double E1 = gam * (p1.E - bx * p1.x - by * p1.y), E2 = gam * (p2.E - bx * p2.x - by * p2.y);
-    const double PEb = E1 + E2;
-    const double x1 = (PEb + Pz) * c.inv_sqrt_s, x2 = (PEb - Pz) * c.inv_sqrt_s;
+    // O7 without the cancellation in 1 - beta^2 (nearly collinear jets): with P = p1 + p2,
+    //   P_E'^2 = P_E^2 - P_T^2 = p1z^2 + p2z^2 + 2 E1 E2 (1 - n1T.n2T)
+    //   E_i'   = gamma (E_i - beta.p_iT) = (p_iz^2 + E1 E2 (1 - n1T.n2T)) / P_E'
+    //   s-hat  = 2 E1 E2 (1 - n1.n2) = (P_E' + P_z)(P_E' - P_z)
+    const double e12 = p1.E * p2.E, ekt = e12 * ec[KT];
+    const double Pz = p1.z + p2.z;
+    const double PEb = sqrt(fma(p1.z, p1.z, fma(p2.z, p2.z, 2.0 * ekt)));
+    const double iPEb = rcp_fast(PEb);
+    const double E1 = fma(p1.z, p1.z, ekt) * iPEb, E2 = fma(p2.z, p2.z, ekt) * iPEb;
+    const double shat = 2.0 * e12 * ec[J0 + 3];
+    const double Xb = PEb + fabs(Pz), Xs = shat / Xb;
+    const double x1 = (Pz >= 0.0 ? Xb : Xs) * c.inv_sqrt_s, x2 = (Pz >= 0.0 ? Xs : Xb) * c.inv_sqrt_s;
     if (!(x1 > 0.0 && x1 < 1.0 && x2 > 0.0 && x2 < 1.0)) return 0.0;
-    const double xx = x1 * x2, shat = xx * c.S;
     // u = -2 qa.p2', t = -2 qa.p1' for qa = q1 and qa = q2 (both beam orderings), in units of -2h
     const double u1 = x1 * (E2 - p2.z), t1 = x1 * (E1 - p1.z);
     const double u2 = x2 * (E2 + p2.z), t2 = x2 * (E1 + p1.z);
