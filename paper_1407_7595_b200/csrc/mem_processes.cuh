@@ -57,7 +57,13 @@ struct ProcWenu {
     ec[LP] = pT * exp(eta);             // E_l + l_z
     ec[LE] = lE; ec[LZ] = lz; ec[PT] = pT; ec[NT2] = nT2; ec[A] = a;
     ec[CLO] = c_lo; ec[CHI] = c_hi; ec[DT] = dt; ec[SCLO] = sin(c_lo);   // sin(c_lo) = cos(t_lo)
-    ec[DSM] = s_min - s_star;
+    // s_min - s* without cancellation: E_l E_nu - l_z nu_z = pT nT cosh(eta - y_nu), so at the
+    // boundary nu_z = +-P (y_P = +-asinh(P / nT)):  s(+-P) - s* = 4 pT nT sinh^2((eta - y_P) / 2)
+    {
+      const double yP = asinh(Pz / nT);
+      const double shp = sinh(0.5 * (eta - yP)), shm = sinh(0.5 * (eta + yP));
+      ec[DSM] = (nz_star > Pz) ? 4.0 * pT * nT * shp * shp : (nz_star < -Pz) ? 4.0 * pT * nT * shm * shm : 0.0;
+    }
     ec[PTNT] = pT * nT;
     ec[IPT2] = 1.0 / (pT * pT);
     // dt * (ds/dt * D_W = 1/(m Gam)) * g^4 |V_ud|^2 / 12 * A_q^2 * (4 / (x1 x2 S)) * (4 h^2 = S)
