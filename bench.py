@@ -29,17 +29,21 @@ if ROOT not in sys.path:
 SEED = 20140729
 
 # Algorithmic FP64 work per integrand call of the dominant kernel: executed
-# thread-level DFMA / DMUL / DADD per point, from the ncu capture in profiles/ (r01_ncu_config3.md):
-# smsp__sass_thread_inst_executed_op_{dfma,dmul,dadd}_pred_on.sum / points.  flop = 2 DFMA + DMUL + DADD.
+# thread-level DFMA / DMUL / DADD per point from the ncu captures in profiles/ (r01_ncu_config3.md,
+# r01_fp64_counts.md): smsp__sass_thread_inst_executed_op_{dfma,dmul,dadd}_pred_on.sum / points.
+# flop = 2 DFMA + DMUL + DADD.  Key = config; config 5's dominant kernel is the grid-mapped final pass.
 FP64_PER_CALL = {
-    3: {"dfma": 268.0, "dmul": 86.0, "dadd": 77.0},
+    1: {"dfma": 87.3, "dmul": 47.0, "dadd": 17.9},
+    2: {"dfma": 116.0, "dmul": 37.0, "dadd": 14.2},
+    3: {"dfma": 261.2, "dmul": 77.7, "dadd": 40.8},
+    5: {"dfma": 268.4, "dmul": 96.7, "dadd": 53.1},
 }
 NOMINAL_FP64_FMA_PER_CLK_PER_SM = 64      # 4 SMSPs x 16 lanes; confirmed by the microbenchmark
 VEGAS_ITERS, VEGAS_POINTS = 5, 1 << 17    # BASELINE.json:configs[4]
 
 
 def flops_per_call(cfg):
-    c = FP64_PER_CALL[3 if cfg == 5 else cfg]
+    c = FP64_PER_CALL[cfg]
     return 2.0 * c["dfma"] + c["dmul"] + c["dadd"]
 
 
@@ -267,7 +271,7 @@ def run_b200(args):
     peak_meas = mem.mem_measure_fp64_peak(5)
     fl = flops_per_call(cfg)
     achieved = k_evals * fl / (k_ms * 1e-3) / 1e12
-    c = FP64_PER_CALL[3 if cfg == 5 else cfg]
+    c = FP64_PER_CALL[cfg]
     pipe_inst = c["dfma"] + c["dmul"] + c["dadd"]
     sms = torch.cuda.get_device_properties(0).multi_processor_count
     sm_mhz = (clocks or {}).get("sm_mhz") or 0.0
