@@ -78,6 +78,8 @@ def lib():
         L.orc_me_top_decay.restype = C.c_double
         L.orc_boost_transverse.argtypes = [_dp, C.c_int, _dp]
         L.orc_boost_transverse.restype = None
+        L.orc_quartic_real_roots.argtypes = [_dp, _dp]
+        L.orc_dilep_solve.argtypes = [_dp] * 4 + [C.c_double] * 6 + [_dp, _dp]
         L.orc_weight.argtypes = [C.c_int, C.POINTER(Params), _dp, _dp, _dp]
         L.orc_weight.restype = C.c_double
         L.orc_eval_points.argtypes = [C.c_int, C.POINTER(Params), _dp, C.c_int64, C.c_int64, C.c_uint64,
@@ -193,6 +195,22 @@ def boost_transverse(P, mom):
     m = _f64(mom).copy()
     lib().orc_boost_transverse(_p(P), m.shape[0], _p(m))
     return m
+
+
+def quartic_real_roots(coeffs_low_to_high):
+    """real roots of q[0] + q[1] x + ... + q[4] x^4 (the oracle's Ferrari solver)"""
+    q = _f64(coeffs_low_to_high)
+    x = np.empty(4)
+    n = lib().orc_quartic_real_roots(_p(q), _p(x))
+    return x[:n].copy()
+
+
+def dilep_solve(lp, b, lm, bb, sWp, st, sWm, stb, Sx, Sy):
+    """all (nu, nubar) solutions of PAPER.md Eq. 8: returns (sol [n, 2, 4], jac [n])"""
+    a = [_f64(v) for v in (lp, b, lm, bb)]
+    sol, jac = np.empty(32), np.empty(4)
+    n = lib().orc_dilep_solve(_p(a[0]), _p(a[1]), _p(a[2]), _p(a[3]), sWp, st, sWm, stb, Sx, Sy, _p(sol), _p(jac))
+    return sol[:8 * n].reshape(n, 2, 4).copy(), jac[:n].copy()
 
 
 def weight(process, p, rec, u, debug=False):

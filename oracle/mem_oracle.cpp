@@ -28,6 +28,7 @@
 
 #include <cmath>
 #include <cstring>
+#include <limits>
 #include <vector>
 
 namespace {
@@ -400,6 +401,289 @@ template <typename R> R weight_tt_ljets(const orc_params* p, const double* rec, 
   return std::isfinite(w) ? w : R(0);
 }
 
+// ---------------- config 4: t tbar -> b l+ nu  bbar l- nubar, D = 8 ----------------
+// rec = [(pT,eta,phi) l+, (pT,eta,phi) l-, (E,eta,phi) b, (E,eta,phi) bbar, met_x, met_y]
+// (readings A3, A8, A12; Eq. 7-8)
+
+// Largest real root of z^3 + c2 z^2 + c1 z + c0 (textbook: depressed cubic, Cardano for one real
+// root, trigonometric form for three), then Newton on the cubic until it stops moving.
+template <typename R> R cubic_largest_root(R c2, R c1, R c0) {
+  const R sh = c2 / R(3);
+  const R P = c1 - c2 * c2 / R(3);
+  const R Q = R(2) * c2 * c2 * c2 / R(27) - c2 * c1 / R(3) + c0;
+  const R disc = Q * Q / R(4) + P * P * P / R(27);
+  R w;
+  if (disc > R(0)) {
+    const R sq = std::sqrt(disc);
+    const R A = (Q > R(0)) ? -std::cbrt(Q / R(2) + sq) : std::cbrt(-Q / R(2) + sq);
+    const R B = (A != R(0)) ? -P / (R(3) * A) : R(0);
+    w = A + B;
+  } else {
+    const R m = std::sqrt(-P / R(3));
+    if (m == R(0)) w = R(0);
+    else {
+      R c = (R(-0.5) * Q) / (m * m * m);
+      if (c > R(1)) c = R(1);
+      if (c < R(-1)) c = R(-1);
+      w = R(2) * m * std::cos(std::acos(c) / R(3));
+    }
+  }
+  R z = w - sh;
+  for (int it = 0; it < 30; ++it) {
+    const R f = ((z + c2) * z + c1) * z + c0;
+    const R fp = (R(3) * z + R(2) * c2) * z + c1;
+    if (!(fp != R(0))) break;
+    const R zn = z - f / fp;
+    if (!std::isfinite((double)zn)) break;
+    const bool done = std::fabs(zn - z) <= R(4) * std::numeric_limits<R>::epsilon() * std::fabs(zn);
+    z = zn;
+    if (done) break;
+  }
+  return z;
+}
+
+// Real roots of q4 x^4 + q3 x^3 + q2 x^2 + q1 x + q0 by Ferrari's method: depress, take the
+// largest root z0 of the resolvent cubic z^3 + 2p z^2 + (p^2 - 4r) z - q^2, split into
+// (y^2 + s y + m)(y^2 - s y + n), s = sqrt(z0), m,n = (p + z0 -+ q/s)/2.  A quadratic factor has
+// real roots iff its discriminant is >= 0.  Returns the number of real roots (0, 2 or 4).
+template <typename R> int quartic_real_roots(R q4, R q3, R q2, R q1, R q0, R* x) {
+  if (!(q4 != R(0))) return 0;
+  const R a3 = q3 / q4, a2 = q2 / q4, a1 = q1 / q4, a0 = q0 / q4;
+  const R p = a2 - R(3) * a3 * a3 / R(8);
+  const R q = a1 - a3 * a2 / R(2) + a3 * a3 * a3 / R(8);
+  const R r = a0 - a3 * a1 / R(4) + a3 * a3 * a2 / R(16) - R(3) * a3 * a3 * a3 * a3 / R(256);
+  const R shift = -a3 / R(4);
+  R z0 = cubic_largest_root<R>(R(2) * p, p * p - R(4) * r, -q * q);
+  if (!(z0 > R(0))) z0 = R(0);
+  const R s = std::sqrt(z0);
+  // q/s = sign(q) sqrt((p + z0)^2 - 4 r) (from the resolvent); use the quotient unless s vanishes
+  R qs;
+  if (s > R(0)) qs = q / s;
+  else { R t = p * p - R(4) * r; qs = (t > R(0)) ? std::sqrt(t) : R(0); }
+  const R m = (p + z0 - qs) / R(2), n = (p + z0 + qs) / R(2);
+  int cnt = 0;
+  const R d1 = z0 - R(4) * m;          // y^2 + s y + m
+  if (d1 >= R(0)) {
+    const R sq = std::sqrt(d1);
+    const R ya = (-s - sq) / R(2);     // the larger-magnitude root first (s >= 0), the other from the product
+    const R yb = (ya != R(0)) ? m / ya : (-s + sq) / R(2);
+    x[cnt++] = ya + shift; x[cnt++] = yb + shift;
+  }
+  const R d2 = z0 - R(4) * n;          // y^2 - s y + n
+  if (d2 >= R(0)) {
+    const R sq = std::sqrt(d2);
+    const R ya = (s + sq) / R(2);
+    const R yb = (ya != R(0)) ? n / ya : (s - sq) / R(2);
+    x[cnt++] = ya + shift; x[cnt++] = yb + shift;
+  }
+  return cnt;
+}
+
+// One top side of PAPER.md:113-118 Eq. 8 (reading A3: ordinary invariant masses): the neutrino
+// momenta with (l + nu)^2 = sW and (b + l + nu)^2 = st lie on the plane d.nu = kappa and satisfy
+// E_nu = w0 + n_l.nu.  In terms of (x, y) = (nu_x, nu_y):
+//   nu_z = al0 + alx x + aly y,   E_nu = la0 + lax x + lay y.
+template <typename R> struct TopSide {
+  R al0, alx, aly, la0, lax, lay;
+  bool ok;
+};
+template <typename R> TopSide<R> top_side(const V4<R>& l, const V4<R>& b, R sW, R st) {
+  TopSide<R> t;
+  const R nlx = l.x / l.E, nly = l.y / l.E, nlz = l.z / l.E;
+  const R nbx = b.x / b.E, nby = b.y / b.E, nbz = b.z / b.E;
+  const R mbl2 = R(2) * dot(b, l);
+  const R Delta = st - sW - mbl2;                 // 2 b.nu
+  const R w0 = sW / (R(2) * l.E);
+  const R kappa = Delta / (R(2) * b.E) - w0;
+  const R dx = nlx - nbx, dy = nly - nby, dz = nlz - nbz;
+  t.ok = (Delta > R(0)) && (dz != R(0));
+  t.al0 = kappa / dz; t.alx = -dx / dz; t.aly = -dy / dz;
+  t.la0 = w0 + nlz * t.al0; t.lax = nlx + nlz * t.alx; t.lay = nly + nlz * t.aly;
+  return t;
+}
+// conic a x^2 + b xy + c y^2 + d x + e y + f = 0 expressing E_nu^2 = |nu|^2
+template <typename R> void side_conic(const TopSide<R>& t, R* k) {
+  k[0] = R(1) + t.alx * t.alx - t.lax * t.lax;
+  k[1] = R(2) * (t.alx * t.aly - t.lax * t.lay);
+  k[2] = R(1) + t.aly * t.aly - t.lay * t.lay;
+  k[3] = R(2) * (t.al0 * t.alx - t.la0 * t.lax);
+  k[4] = R(2) * (t.al0 * t.aly - t.la0 * t.lay);
+  k[5] = t.al0 * t.al0 - t.la0 * t.la0;
+}
+
+// All real solutions (nu, nubar) of the six equations of Eq. 8: two W masses, two top masses and
+// nu_T + nubar_T = (Sx, Sy).  Resultant quartic in x = nu_x, y from the linear relation, then
+// Newton on g1 = |nu| - E_nu(x,y), g2 = |nubar| - E_nubar(Sx-x, Sy-y) (reading A12).
+// sol[k] = {nu (E,x,y,z), nubar (E,x,y,z)}.  Returns the number of solutions (0..4).
+template <typename R> int dilep_solve(const V4<R>& lp, const V4<R>& b, const V4<R>& lm, const V4<R>& bb,
+                                      R sWp, R st, R sWm, R stb, R Sx, R Sy, R sol[4][8]) {
+  const TopSide<R> T1 = top_side<R>(lp, b, sWp, st), T2 = top_side<R>(lm, bb, sWm, stb);
+  if (!T1.ok || !T2.ok) return 0;
+  R k1[6], kb[6], k2[6];
+  side_conic<R>(T1, k1);
+  side_conic<R>(T2, kb);                          // in (xbar, ybar) = (Sx - x, Sy - y)
+  k2[0] = kb[0]; k2[1] = kb[1]; k2[2] = kb[2];
+  k2[3] = -R(2) * kb[0] * Sx - kb[1] * Sy - kb[3];
+  k2[4] = -R(2) * kb[2] * Sy - kb[1] * Sx - kb[4];
+  k2[5] = kb[0] * Sx * Sx + kb[1] * Sx * Sy + kb[2] * Sy * Sy + kb[3] * Sx + kb[4] * Sy + kb[5];
+  // as polynomials in y: p_i y^2 + q_i(x) y + r_i(x), p = c, q = b x + e, r = a x^2 + d x + f
+  const R U2 = k1[2] * k2[0] - k2[2] * k1[0], U1 = k1[2] * k2[3] - k2[2] * k1[3], U0 = k1[2] * k2[5] - k2[2] * k1[5];
+  const R V1 = k1[2] * k2[1] - k2[2] * k1[1], V0 = k1[2] * k2[4] - k2[2] * k1[4];
+  const R W3 = k1[1] * k2[0] - k2[1] * k1[0];
+  const R W2 = k1[1] * k2[3] + k1[4] * k2[0] - k2[1] * k1[3] - k2[4] * k1[0];
+  const R W1 = k1[1] * k2[5] + k1[4] * k2[3] - k2[1] * k1[5] - k2[4] * k1[3];
+  const R W0 = k1[4] * k2[5] - k2[4] * k1[5];
+  const R R4 = U2 * U2 - V1 * W3;
+  const R R3 = R(2) * U2 * U1 - V1 * W2 - V0 * W3;
+  const R R2 = U1 * U1 + R(2) * U2 * U0 - V1 * W1 - V0 * W2;
+  const R R1 = R(2) * U1 * U0 - V1 * W0 - V0 * W1;
+  const R R0 = U0 * U0 - V0 * W0;
+  R xr[4];
+  const int nr = quartic_real_roots<R>(R4, R3, R2, R1, R0, xr);
+  int ns = 0;
+  for (int i = 0; i < nr; ++i) {
+    R x = xr[i];
+    const R V = V1 * x + V0;
+    if (!(V != R(0))) continue;
+    R y = -((U2 * x + U1) * x + U0) / V;
+    // Newton on the un-squared equations
+    R nz = 0, En = 0, nbz = 0, Enb = 0;
+    bool good = true;
+    for (int it = 0; it < 12; ++it) {
+      nz = T1.al0 + T1.alx * x + T1.aly * y;
+      En = std::sqrt(x * x + y * y + nz * nz);
+      const R xb = Sx - x, yb = Sy - y;
+      nbz = T2.al0 + T2.alx * xb + T2.aly * yb;
+      Enb = std::sqrt(xb * xb + yb * yb + nbz * nbz);
+      const R g1 = En - (T1.la0 + T1.lax * x + T1.lay * y);
+      const R g2 = Enb - (T2.la0 + T2.lax * xb + T2.lay * yb);
+      const R j11 = (x + nz * T1.alx) / En - T1.lax, j12 = (y + nz * T1.aly) / En - T1.lay;
+      const R j21 = -((xb + nbz * T2.alx) / Enb - T2.lax), j22 = -((yb + nbz * T2.aly) / Enb - T2.lay);
+      const R det = j11 * j22 - j12 * j21;
+      if (!(det != R(0)) || !std::isfinite((double)det)) { good = false; break; }
+      const R dxn = (g1 * j22 - g2 * j12) / det, dyn = (j11 * g2 - j21 * g1) / det;
+      x -= dxn; y -= dyn;
+      if (std::fabs(dxn) + std::fabs(dyn) <= R(8) * std::numeric_limits<R>::epsilon() * (std::fabs(x) + std::fabs(y)))
+        break;
+    }
+    if (!good) continue;
+    nz = T1.al0 + T1.alx * x + T1.aly * y;
+    const R xb = Sx - x, yb = Sy - y;
+    nbz = T2.al0 + T2.alx * xb + T2.aly * yb;
+    En = T1.la0 + T1.lax * x + T1.lay * y;        // E from the W-mass equation (linear form)
+    Enb = T2.la0 + T2.lax * xb + T2.lay * yb;
+    if (!(En > R(0)) || !(Enb > R(0))) continue;   // the squared equation also has E < 0 branches
+    // the polished point must still solve the squared equations (a diverged Newton does not)
+    const R c1 = std::sqrt(x * x + y * y + nz * nz), c2 = std::sqrt(xb * xb + yb * yb + nbz * nbz);
+    if (!(std::fabs(c1 - En) <= R(1e-9) * (c1 + En)) || !(std::fabs(c2 - Enb) <= R(1e-9) * (c2 + Enb))) continue;
+    R* s = sol[ns++];
+    s[0] = c1; s[1] = x; s[2] = y; s[3] = nz; s[4] = c2; s[5] = xb; s[6] = yb; s[7] = nbz;
+  }
+  return ns;
+}
+
+// |d(s_W+, s_t, s_W-, s_tbar, S_x, S_y)/d(nu, nubar)|^-1 at one solution:
+// with A = grad_nu s_W+ = 2(E_l nuhat - l), B = grad_nu s_t = 2((E_l + E_b) nuhat - (l + b)) and
+// C, D likewise on the antitop side, the 6x6 determinant equals [(A x B) x (C x D)]_z.
+template <typename R> R dilep_jacobian(const V4<R>& lp, const V4<R>& b, const V4<R>& lm, const V4<R>& bb, const R* s) {
+  auto grads = [](const V4<R>& l, const V4<R>& bq, const R* nu, R* A, R* B) {
+    const R hx = nu[1] / nu[0], hy = nu[2] / nu[0], hz = nu[3] / nu[0];
+    A[0] = R(2) * (l.E * hx - l.x); A[1] = R(2) * (l.E * hy - l.y); A[2] = R(2) * (l.E * hz - l.z);
+    B[0] = R(2) * ((l.E + bq.E) * hx - (l.x + bq.x)); B[1] = R(2) * ((l.E + bq.E) * hy - (l.y + bq.y));
+    B[2] = R(2) * ((l.E + bq.E) * hz - (l.z + bq.z));
+  };
+  auto cross = [](const R* a, const R* c, R* o) {
+    o[0] = a[1] * c[2] - a[2] * c[1]; o[1] = a[2] * c[0] - a[0] * c[2]; o[2] = a[0] * c[1] - a[1] * c[0];
+  };
+  R A[3], B[3], Cc[3], Dd[3], P[3], Q[3], X[3];
+  grads(lp, b, s, A, B);
+  grads(lm, bb, s + 4, Cc, Dd);
+  cross(A, B, P); cross(Cc, Dd, Q); cross(P, Q, X);
+  return R(1) / std::fabs(X[2]);
+}
+
+template <typename R> R weight_tt_dilep(const orc_params* p, const double* rec, const double* u, double* dbg) {
+  const R S = R(p->sqrt_s) * R(p->sqrt_s), dr = R(p->jetE_rhi) - R(p->jetE_rlo);
+  const R twopi3 = R(8) * pi_<R>() * pi_<R>() * pi_<R>();
+  if (dbg) dbg[0] = 0;
+  V4<R> lp = from_pt_eta_phi<R>(rec[0], rec[1], rec[2]), lm = from_pt_eta_phi<R>(rec[3], rec[4], rec[5]);
+  const R met_x = rec[12], met_y = rec[13];
+  V4<R> jet[2];
+  R vol = R(1), tf = R(1), meas = R(1);
+  for (int j = 0; j < 2; ++j) {
+    R Ej = rec[6 + 3 * j], eta = rec[7 + 3 * j], phi = rec[8 + 3 * j];
+    R E = Ej * (R(p->jetE_rlo) + dr * R(u[j]));
+    vol *= Ej * dr;
+    tf *= tf_jet<R>(p, Ej, E);
+    meas *= E * (R(1) / std::cosh(eta)) / (R(2) * twopi3);
+    jet[j] = from_E_eta_phi<R>(E, eta, phi);
+  }
+  const V4<R> &b = jet[0], &bb = jet[1];
+  // four Breit-Wigner mapped masses: u2 -> s_W+, u3 -> s_t, u4 -> s_W-, u5 -> s_tbar (O6)
+  const R mW = p->m_W, GW = p->Gam_W, mt = p->m_t, Gt = p->Gam_t, n = p->bw_nwidths;
+  R tWlo, tWhi, tTlo, tThi;
+  bw_window<R>(mW, GW, (mW - n * GW) * (mW - n * GW), (mW + n * GW) * (mW + n * GW), &tWlo, &tWhi);
+  bw_window<R>(mt, Gt, (mt - n * Gt) * (mt - n * Gt), (mt + n * Gt) * (mt + n * Gt), &tTlo, &tThi);
+  R smm[4], dsdt[4], Dk[4];
+  for (int k = 0; k < 4; ++k) {
+    const bool isW = (k == 0 || k == 2);
+    const R lo = isW ? tWlo : tTlo, hi = isW ? tWhi : tThi;
+    const R t = lo + (hi - lo) * R(u[2 + k]);
+    vol *= (hi - lo);
+    bw_point<R>(isW ? mW : mt, isW ? GW : Gt, t, &smm[k], &dsdt[k], &Dk[k]);
+  }
+  const R sWp = mW * mW + smm[0], st = mt * mt + smm[1], sWm = mW * mW + smm[2], stb = mt * mt + smm[3];
+  // total neutrino transverse momentum, flat +-n sigma around the measured MET, Gaussian MET TF (A8)
+  const R sig = p->met_sigma, ns = p->met_nsigma;
+  const R Sx = met_x + sig * ns * (R(2) * R(u[6]) - R(1)), Sy = met_y + sig * ns * (R(2) * R(u[7]) - R(1));
+  vol *= (R(2) * ns * sig) * (R(2) * ns * sig);
+  const R ddx = met_x - Sx, ddy = met_y - Sy;
+  const R tmet = std::exp(-(ddx * ddx + ddy * ddy) / (R(2) * sig * sig)) / (R(2) * pi_<R>() * sig * sig);
+  meas *= R(1) / (R(2) * lp.E * twopi3) * R(1) / (R(2) * lm.E * twopi3);   // leptons: delta TF
+  R sol[4][8];
+  const int nsol = dilep_solve<R>(lp, b, lm, bb, sWp, st, sWm, stb, Sx, Sy, sol);
+  R sum = R(0);
+  int kept = 0;
+  for (int k = 0; k < nsol; ++k) {
+    const R J = dilep_jacobian<R>(lp, b, lm, bb, sol[k]);
+    V4<R> nu = from_arr(sol[k]), nub = from_arr(sol[k] + 4);
+    // O7 boost of the six final momenta: order l+, nu, b, l-, nubar, bbar
+    R mom[24];
+    to_arr(lp, mom); to_arr(nu, mom + 4); to_arr(b, mom + 8); to_arr(lm, mom + 12); to_arr(nub, mom + 16);
+    to_arr(bb, mom + 20);
+    V4<R> P = lp + nu + b + lm + nub + bb;
+    R Parr[4]; to_arr(P, Parr);
+    if (!(P.x * P.x + P.y * P.y < P.E * P.E)) continue;
+    boost_transverse<R>(Parr, 6, mom);
+    R PE = 0, Pzz = 0;
+    for (int i = 0; i < 6; ++i) { PE += mom[4 * i]; Pzz += mom[4 * i + 3]; }
+    R x1, x2;
+    if (!beam_fractions<R>(p, PE, Pzz, &x1, &x2)) continue;
+    const R shat = x1 * x2 * S;
+    if (!(R(4) * mt * mt < shat)) continue;                       // A9
+    R q1[4], q2[4], pta[4], ptba[4];
+    beams<R>(p, x1, x2, q1, q2);
+    for (int c = 0; c < 4; ++c) { pta[c] = mom[c] + mom[4 + c] + mom[8 + c]; ptba[c] = mom[12 + c] + mom[16 + c] + mom[20 + c]; }
+    const R prod = R(p->pdf_A_g) * R(p->pdf_A_g) * me_tt_gg<R>(p, q1, q2, pta, ptba) +
+                   R(2) * R(p->n_flav) * R(p->pdf_A_q) * R(p->pdf_A_q) * me_tt_qq<R>(p, q1, q2, pta, ptba);
+    // t -> b l+ nu: (p_t.p_l+)(p_b.p_nu);  tbar -> bbar l- nubar: (p_tbar.p_l-)(p_bbar.p_nubar)
+    const R dec1 = R(0.5) * me_top_decay_D<R>(p, R(1), pta, mom + 8, mom, mom + 4, Dk[0]);
+    const R dec2 = R(0.5) * me_top_decay_D<R>(p, R(1), ptba, mom + 20, mom + 12, mom + 16, Dk[2]);
+    const R me = prod * Dk[1] * Dk[3] * dec1 * dec2;
+    const R ff = pdf_shape<R>(p, x1) * pdf_shape<R>(p, x2);
+    const R flux = x1 * x2 * S / R(4);
+    const R ws = J / (twopi3 * twopi3 * R(4) * nu.E * nub.E) * ff * me / flux;
+    if (!std::isfinite((double)ws)) continue;
+    sum += ws;
+    dbg_store<R>(dbg, kept, 6, x1, x2, mom);
+    ++kept;
+  }
+  if (dbg) dbg[0] = kept;
+  R w = vol * dsdt[0] * dsdt[1] * dsdt[2] * dsdt[3] * tf * tmet * meas *
+        (R(16) * pi_<R>() * pi_<R>() * pi_<R>() * pi_<R>()) * (R(2) / S) * sum;
+  return std::isfinite((double)w) ? w : R(0);
+}
+
 template <typename R> double weight_any(int process, const orc_params* p, const double* rec, const double* u,
                                         double* dbg) {
   R w = R(0);
@@ -407,6 +691,7 @@ template <typename R> double weight_any(int process, const orc_params* p, const 
     case ORC_W_ENU: w = weight_w_enu<R>(p, rec, u, dbg); break;
     case ORC_Z_BB: w = weight_z_bb<R>(p, rec, u, dbg); break;
     case ORC_TT_LJETS: w = weight_tt_ljets<R>(p, rec, u, dbg); break;
+    case ORC_TT_DILEP: w = weight_tt_dilep<R>(p, rec, u, dbg); break;
     default: return std::nan("");
   }
   double wd = (double)w;
@@ -535,6 +820,23 @@ double orc_me_top_decay(const orc_params* p, double n_c, const double pt[4], con
   return me_top_decay<double>(p, n_c, pt, pb, pf_down, pf_up);
 }
 void orc_boost_transverse(const double P[4], int n, double* mom) { boost_transverse<double>(P, n, mom); }
+
+// config-4 building blocks (pinned by tests/test_oracle_dilep.py)
+int orc_quartic_real_roots(const double q[5], double x[4]) {
+  return quartic_real_roots<double>(q[4], q[3], q[2], q[1], q[0], x);
+}
+int orc_dilep_solve(const double lp[4], const double b[4], const double lm[4], const double bb[4],
+                    double sWp, double st, double sWm, double stb, double Sx, double Sy,
+                    double* sol /* [4][8] */, double* jac /* [4] */) {
+  V4<double> a = from_arr(lp), c = from_arr(b), d = from_arr(lm), e = from_arr(bb);
+  double s[4][8];
+  int n = dilep_solve<double>(a, c, d, e, sWp, st, sWm, stb, Sx, Sy, s);
+  for (int k = 0; k < n; ++k) {
+    for (int i = 0; i < 8; ++i) sol[8 * k + i] = s[k][i];
+    jac[k] = dilep_jacobian<double>(a, c, d, e, s[k]);
+  }
+  return n;
+}
 
 double orc_weight(int process, const orc_params* p, const double* rec, const double* u, double* dbg) {
   return weight_any<double>(process, p, rec, u, dbg);

@@ -70,6 +70,14 @@ double orc_me_top_decay(const orc_params* p, double n_c, const double pt[4], con
                         const double pf_down[4], const double pf_up[4]);
 void   orc_boost_transverse(const double P[4], int n, double* mom /* n x 4, in place */);
 
+/* config 4: real roots of q[0] + q[1] x + ... + q[4] x^4 (Ferrari); all
+ * solutions of the dilepton system PAPER.md:113-118 Eq. 8, sol[k] = {nu(E,x,y,z), nubar(E,x,y,z)},
+ * jac[k] = |d(nu,nubar)/d(s_W+, s_t, s_W-, s_tbar, S_x, S_y)|.  Both return the count. */
+int    orc_quartic_real_roots(const double q[5], double x[4]);
+int    orc_dilep_solve(const double lp[4], const double b[4], const double lm[4], const double bb[4],
+                       double sWp, double st, double sWm, double stb, double Sx, double Sy,
+                       double* sol, double* jac);
+
 /* --- the integrand: one event record (n_fields doubles), one unit-cube point --- */
 /* dbg (may be NULL): [0]=n_sol, [1..]= per solution: x1, x2, then the boosted final momenta. */
 double orc_weight(int process, const orc_params* p, const double* rec, const double* u, double* dbg);
