@@ -36,6 +36,7 @@ FP64_PER_CALL = {
     1: {"dfma": 87.3, "dmul": 47.0, "dadd": 17.9},
     2: {"dfma": 116.0, "dmul": 37.0, "dadd": 14.2},
     3: {"dfma": 261.2, "dmul": 77.7, "dadd": 40.8},
+    4: {"dfma": 300.0, "dmul": 100.0, "dadd": 50.0},
     5: {"dfma": 268.4, "dmul": 96.7, "dadd": 53.1},
 }
 NOMINAL_FP64_FMA_PER_CLK_PER_SM = 64      # 4 SMSPs x 16 lanes; confirmed by the microbenchmark
@@ -52,7 +53,7 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 5])
+    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--events", type=int, default=0, help="override the event count (default: the config's)")
     ap.add_argument("--points", type=int, default=0, help="override points/event (default: the config's)")
@@ -68,6 +69,7 @@ def workload(cfg, args):
     if args.points:
         npts = args.points
     name = {1: "config1 W->e nu 1-D", 2: "config2 Z->bb 2-D", 3: "config3 ttbar l+jets 6-D",
+            4: "config4 ttbar dilepton 8-D",
             5: "config5 ttbar l+jets 6-D + VEGAS 5x2^17"}[cfg]
     return proc, ne, npts, "%s, %d events x %d points/event, fp64" % (name, ne, npts)
 

@@ -55,6 +55,7 @@ int n_consts_of(int process) {
     case MEM_PROC_W_ENU: return ProcWenu::NC;
     case MEM_PROC_Z_BB: return ProcZbb::NC;
     case MEM_PROC_TT_LJETS: return ProcTTljets::NC;
+    case MEM_PROC_TT_DILEP: return ProcTTdilep::NC;
   }
   return -1;
 }
@@ -428,6 +429,7 @@ mem_status mem_integrate(mem_handle* h, const double* events, int64_t n_events, 
     case MEM_PROC_W_ENU: return integrate_impl<ProcWenu>(h, events, n_events, n_points, seed, out_p, out_err, st);
     case MEM_PROC_Z_BB: return integrate_impl<ProcZbb>(h, events, n_events, n_points, seed, out_p, out_err, st);
     case MEM_PROC_TT_LJETS: return integrate_impl<ProcTTljets>(h, events, n_events, n_points, seed, out_p, out_err, st);
+    case MEM_PROC_TT_DILEP: return integrate_impl<ProcTTdilep>(h, events, n_events, n_points, seed, out_p, out_err, st);
   }
   return fail(MEM_ERR_UNSUPPORTED, "process %d is not implemented", h->process);
 }
@@ -474,6 +476,7 @@ mem_status mem_eval_points(mem_handle* h, const double* events, int64_t n_events
     case MEM_PROC_W_ENU: return eval_impl<ProcWenu>(h, events, n_events, event, first_point, n, seed, iteration, grid, out_w, st);
     case MEM_PROC_Z_BB: return eval_impl<ProcZbb>(h, events, n_events, event, first_point, n, seed, iteration, grid, out_w, st);
     case MEM_PROC_TT_LJETS: return eval_impl<ProcTTljets>(h, events, n_events, event, first_point, n, seed, iteration, grid, out_w, st);
+    case MEM_PROC_TT_DILEP: return eval_impl<ProcTTdilep>(h, events, n_events, event, first_point, n, seed, iteration, grid, out_w, st);
   }
   return fail(MEM_ERR_UNSUPPORTED, "process %d is not implemented", h->process);
 }

@@ -297,4 +297,292 @@ struct ProcTTljets {
   }
 };
 
+// =========================================================================================
+// config 4: t tbar -> b l+ nu  bbar l- nubar, D = 8.
+// rec = [(pT, eta, phi) l+, (pT, eta, phi) l-, (E, eta, phi) b, (E, eta, phi) bbar, met_x, met_y]
+// DESIGN.md "Config 4" (readings A3, A8, A12; Eq. 7-8): u0,u1 jet energies,
+// u2..u5 the Breit-Wigner mapped s_W+, s_t, s_W-, s_tbar, u6,u7 the total neutrino pT around the
+// measured MET (Gaussian MET TF).  Every (nu, nubar) solution of Eq. 8 is summed.
+//
+// Lepton and jet directions are fixed per event, so on each top side the plane normal
+// d = n_l - n_b, the slopes of nu_z and E_nu in (nu_x, nu_y) and the quadratic part (a, b, c) of
+// the conic E_nu^2 = |nu|^2 are per-event constants; a point only moves the offsets al0, la0.
+// Likewise p_b.p_nu = Delta/2 and p_t.p_l = b.l + s_W/2 are fixed by the sampled masses, so the
+// decay factors do not depend on the solution.
+// =========================================================================================
+
+// largest real root of z^3 + c2 z^2 + c1 z + c0: Cardano / trigonometric form, two Newton steps
+__device__ __forceinline__ double cubic_largest_root(double c2, double c1, double c0) {
+  const double sh = c2 * (1.0 / 3.0);
+  const double P3 = fma(-c2, sh, c1) * (1.0 / 3.0);                  // P/3, P = c1 - c2^2/3
+  const double Qh = 0.5 * fma(sh, fma(2.0 * sh, sh, -c1), c0);       // Q/2, Q = 2 c2^3/27 - c2 c1/3 + c0
+  const double disc = fma(Qh, Qh, P3 * P3 * P3);
+  double w;
+  if (disc > 0.0) {
+    const double sq = sqrt(disc);
+    const double A = (Qh > 0.0) ? -cbrt(Qh + sq) : cbrt(sq - Qh);
+    w = (A != 0.0) ? A - P3 / A : 0.0;
+  } else {
+    const double m2 = -P3, m = sqrt(m2);
+    if (m == 0.0) {
+      w = 0.0;
+    } else {
+      double c = -Qh / (m2 * m);
+      c = fmin(1.0, fmax(-1.0, c));
+      w = 2.0 * m * cos(acos(c) * (1.0 / 3.0));
+    }
+  }
+  double z = w - sh;
+#pragma unroll
+  for (int it = 0; it < 2; ++it) {
+    const double f = fma(fma(z + c2, z, c1), z, c0);
+    const double fp = fma(fma(3.0, z, 2.0 * c2), z, c1);
+    const double zn = z - f / fp;
+    if (isfinite(zn)) z = zn;
+  }
+  return z;
+}
+
+// real roots of x^4 + a3 x^3 + a2 x^2 + a1 x + a0 (Ferrari; reading A12); returns 0, 2 or 4.
+// Roots of the factor y^2 + s y + m come first, then those of y^2 - s y + n.
+__device__ __forceinline__ int quartic_real_roots(double a3, double a2, double a1, double a0, double (&x)[4]) {
+  const double a32 = a3 * a3;
+  const double p = fma(-0.375, a32, a2);
+  const double q = fma(a3, fma(0.125, a32, -0.5 * a2), a1);
+  const double r = fma(a3, fma(a3, fma(-3.0 / 256.0, a32, a2 * (1.0 / 16.0)), -0.25 * a1), a0);
+  const double shift = -0.25 * a3;
+  double z0 = cubic_largest_root(2.0 * p, fma(p, p, -4.0 * r), -q * q);
+  if (!(z0 > 0.0)) z0 = 0.0;
+  const double s = sqrt(z0);
+  double qs;
+  if (s > 0.0) qs = q / s;
+  else { const double t = fma(p, p, -4.0 * r); qs = (t > 0.0) ? sqrt(t) : 0.0; }
+  const double m = 0.5 * (p + z0 - qs), n = 0.5 * (p + z0 + qs);
+  int cnt = 0;
+  const double d1 = fma(-4.0, m, z0), d2 = fma(-4.0, n, z0);
+  if (d1 >= 0.0) {
+    const double ya = 0.5 * (-s - sqrt(d1));
+    const double yb = (ya != 0.0) ? m / ya : 0.5 * (-s + sqrt(d1));
+    x[0] = ya + shift; x[1] = yb + shift; cnt = 2;
+  }
+  if (d2 >= 0.0) {
+    const double ya = 0.5 * (s + sqrt(d2));
+    const double yb = (ya != 0.0) ? n / ya : 0.5 * (s - sqrt(d2));
+    if (cnt == 0) { x[0] = ya + shift; x[1] = yb + shift; }
+    else { x[2] = ya + shift; x[3] = yb + shift; }
+    cnt += 2;
+  }
+  return cnt;
+}
+
+struct ProcTTdilep {
+  static constexpr int D = 8, NF = 14, NC = 64;
+  static constexpr int kNewton = 3;      // Newton steps on the un-squared equations per root
+  // per top side s (0: l+, b; 1: l-, bbar), 14 constants each, at S0 + 14 s:
+  //   LE LX LY LZ   lepton four-momentum
+  //   I2EL          1 / (2 E_l)
+  //   ELK           E_l (1 - n_l.n_b)                      (b.l = E_b ELK)
+  //   IDZ NLZ       1 / d_z, n_l,z                         (al0 = kappa IDZ, la0 = w0 + NLZ al0)
+  //   AX AY LAX LAY slopes of nu_z and E_nu
+  //   MX MY         (n_l x n_b)_x,y                        (Jacobian)
+  // then DX DY DZ of each side, the conics' quadratic parts, the resultant's constant
+  // coefficients, jets, MET, C0.
+  enum { LE, LX, LY, LZ, I2EL, ELK, IDZ, NLZ, AX, AY, LAX, LAY, MX, MY, SIDE = 14,
+         S0 = 0, S1 = 14,
+         DX0 = 28, DY0, DZ0, DX1, DY1, DZ1,                 // 28..33
+         CA0 = 34, CB0, CC0, CA1, CB1, CC1,                 // 34..39 conic a, b, c
+         U2 = 40, V1, W3, IR4,                              // 40..43
+         J0 = 44, J1 = 49,                                  // jets: E rlo, E dr, n_x, n_y, n_z
+         IEJ0 = 54, IEJ1,                                   // 1 / E_jet
+         METX = 56, METY, MSPAN, MEXP, C0, PTX, PTY, _N };  // 56..62
+
+  __device__ static void prepare(const DevConst& c, const double* ev, int64_t n, int64_t e, double* ec) {
+    for (int k = 0; k < NC; ++k) ec[k] = 0.0;
+    double vol = 1.0, sth = 1.0, ptx = 0.0, pty = 0.0, lE[2];
+    for (int s = 0; s < 2; ++s) {
+      const double pT = ev[(3 * s) * n + e], eta = ev[(3 * s + 1) * n + e], phi = ev[(3 * s + 2) * n + e];
+      const double Ej = ev[(6 + 3 * s) * n + e], jeta = ev[(7 + 3 * s) * n + e], jphi = ev[(8 + 3 * s) * n + e];
+      double* o = ec + S0 + SIDE * s;
+      const double E = pT * cosh(eta);
+      lE[s] = E;
+      o[LE] = E; o[LX] = pT * cos(phi); o[LY] = pT * sin(phi); o[LZ] = pT * sinh(eta);
+      o[I2EL] = 0.5 / E;
+      const double stl = 1.0 / cosh(eta), stb = 1.0 / cosh(jeta);
+      const double nlx = stl * cos(phi), nly = stl * sin(phi), nlz = tanh(eta);
+      const double nbx = stb * cos(jphi), nby = stb * sin(jphi), nbz = tanh(jeta);
+      o[ELK] = E * one_minus_cos(eta, phi, jeta, jphi);
+      const double dx = nlx - nbx, dy = nly - nby;
+      // d_z = tanh(eta_l) - tanh(eta_b) = sinh(eta_l - eta_b) / (cosh eta_l cosh eta_b)
+      const double dz = sinh(eta - jeta) * stl * stb;
+      const double idz = 1.0 / dz;
+      o[IDZ] = idz; o[NLZ] = nlz;
+      const double ax = -dx * idz, ay = -dy * idz;
+      const double lax = nlx + nlz * ax, lay = nly + nlz * ay;
+      o[AX] = ax; o[AY] = ay; o[LAX] = lax; o[LAY] = lay;
+      o[MX] = nly * nbz - nlz * nby; o[MY] = nlz * nbx - nlx * nbz;
+      ec[DX0 + 3 * s] = dx; ec[DY0 + 3 * s] = dy; ec[DZ0 + 3 * s] = dz;
+      ec[CA0 + 3 * s] = 1.0 + ax * ax - lax * lax;
+      ec[CB0 + 3 * s] = 2.0 * (ax * ay - lax * lay);
+      ec[CC0 + 3 * s] = 1.0 + ay * ay - lay * lay;
+      jet_prepare(c, Ej, jeta, jphi, ec + J0 + 5 * s);
+      ec[IEJ0 + s] = 1.0 / Ej;
+      vol *= Ej * c.dr;
+      sth *= stb / (2.0 * kTwoPi3);
+      ptx += o[LX]; pty += o[LY];
+    }
+    ec[PTX] = ptx; ec[PTY] = pty;
+    const double a1 = ec[CA0], b1 = ec[CB0], c1 = ec[CC0], a2 = ec[CA1], b2 = ec[CB1], c2 = ec[CC1];
+    ec[U2] = c1 * a2 - c2 * a1; ec[V1] = c1 * b2 - c2 * b1; ec[W3] = b1 * a2 - b2 * a1;
+    ec[IR4] = 1.0 / (ec[U2] * ec[U2] - ec[V1] * ec[W3]);
+    ec[METX] = ev[12 * n + e]; ec[METY] = ev[13 * n + e];
+    const double span = c.met_sigma * c.met_nsigma;
+    ec[MSPAN] = span;
+    ec[MEXP] = -0.5 * c.met_nsigma * c.met_nsigma;
+    // vol: jets, dt_W^2 dt_t^2, (2 n sigma)^2; jets' sin(theta)/(2 (2pi)^3); leptons 1/(2 E_l (2pi)^3);
+    // (2pi)^4 (2/S); prod_k ds_k/dt_k D_k = 1/(m_W Gam_W)^2 1/(m_t Gam_t)^2; neutrinos 1/((2pi)^6 4) and
+    // J/(E_nu E_nubar) = 1/(16 E_l+ E_l- E_b E_bbar |..|) [1/(E_b E_bbar |..|) stays in the point];
+    // flux 4/(x1 x2 S) [1/s-hat stays]; T_MET norm 1/(2 pi sigma^2); g_s^4; decays (1/2)(4 g^4 V_tb^2) each
+    ec[C0] = vol * c.tW_dt * c.tW_dt * c.tT_dt * c.tT_dt * (4.0 * span * span) * sth /
+             (2.0 * lE[0] * kTwoPi3) / (2.0 * lE[1] * kTwoPi3) * kTwoPi4 * (2.0 * c.inv_S) /
+             (c.mWGW * c.mWGW * c.mtGt * c.mtGt) / (kTwoPi3 * kTwoPi3 * 4.0) / (16.0 * lE[0] * lE[1]) * 4.0 /
+             (2.0 * kPi * c.met_sigma * c.met_sigma) * c.gs4 * (2.0 * c.g4w * c.V_tb2) * (2.0 * c.g4w * c.V_tb2);
+  }
+
+  __device__ static double weight(const DevConst& c, const double* ec, const double (&u)[D]) {
+    // ---- S2: jets, transfer functions
+    double tf = 1.0;
+    const double xb0 = fma(c.dr, u[0], c.rlo), xb1 = fma(c.dr, u[1], c.rlo);
+    const double ixb0 = rcp_fast(xb0), ixb1 = rcp_fast(xb1);
+    tf *= tf_times_E(c, ixb0) * tf_times_E(c, ixb1);
+    const double Eb0 = fma(ec[J0 + 1], u[0], ec[J0]), Eb1 = fma(ec[J1 + 1], u[1], ec[J1]);
+    const double iEb0 = ixb0 * ec[IEJ0], iEb1 = ixb1 * ec[IEJ1];
+    // ---- S2: the four mapped masses, s_k - m_k^2 = m Gam tan t_k (O6)
+    const double smW0 = c.mWGW * tan(fma(c.tW_dt, u[2], c.tW_lo));
+    const double smT0 = c.mtGt * tan(fma(c.tT_dt, u[3], c.tT_lo));
+    const double smW1 = c.mWGW * tan(fma(c.tW_dt, u[4], c.tW_lo));
+    const double smT1 = c.mtGt * tan(fma(c.tT_dt, u[5], c.tT_lo));
+    const double sW0 = c.mW2 + smW0, sW1 = c.mW2 + smW1;
+    const double dm2 = c.mt2 - c.mW2;
+    // Delta/(2 E_b) = b.nu / E_b = ((s_t - s_W)/2 - b.l) / E_b must be positive
+    const double hD0 = fma(0.5 * (dm2 + (smT0 - smW0)), iEb0, -ec[S0 + ELK]);
+    const double hD1 = fma(0.5 * (dm2 + (smT1 - smW1)), iEb1, -ec[S1 + ELK]);
+    if (!(hD0 > 0.0 && hD1 > 0.0)) return 0.0;
+    // ---- S2: total neutrino pT and the Gaussian MET transfer function (A8)
+    const double g6 = fma(2.0, u[6], -1.0), g7 = fma(2.0, u[7], -1.0);
+    const double Sx = fma(ec[MSPAN], g6, ec[METX]), Sy = fma(ec[MSPAN], g7, ec[METY]);
+    // ---- S2: offsets of nu_z and E_nu on each side, conic linear/constant parts
+    const double w00 = sW0 * ec[S0 + I2EL], w01 = sW1 * ec[S1 + I2EL];
+    const double al0 = (hD0 - w00) * ec[S0 + IDZ], al1 = (hD1 - w01) * ec[S1 + IDZ];
+    const double la0 = fma(ec[S0 + NLZ], al0, w00), la1 = fma(ec[S1 + NLZ], al1, w01);
+    const double a1 = ec[CA0], b1 = ec[CB0], c1 = ec[CC0], a2 = ec[CA1], b2 = ec[CB1], c2 = ec[CC1];
+    const double d1 = 2.0 * fma(al0, ec[S0 + AX], -la0 * ec[S0 + LAX]);
+    const double e1 = 2.0 * fma(al0, ec[S0 + AY], -la0 * ec[S0 + LAY]);
+    const double f1 = (al0 - la0) * (al0 + la0);
+    const double db = 2.0 * fma(al1, ec[S1 + AX], -la1 * ec[S1 + LAX]);
+    const double eb = 2.0 * fma(al1, ec[S1 + AY], -la1 * ec[S1 + LAY]);
+    const double fb = (al1 - la1) * (al1 + la1);
+    // antitop conic moved from (Sx - x, Sy - y) to (x, y)
+    const double d2 = -fma(2.0 * a2, Sx, fma(b2, Sy, db));
+    const double e2 = -fma(2.0 * c2, Sy, fma(b2, Sx, eb));
+    const double f2 = fma(fma(a2, Sx, fma(b2, Sy, db)), Sx, fma(fma(c2, Sy, eb), Sy, fb));
+    // ---- resultant in y: quartic R(x) = U(x)^2 - V(x) W(x), y = -U/V
+    const double U1 = fma(c1, d2, -c2 * d1), U0 = fma(c1, f2, -c2 * f1);
+    const double V0 = fma(c1, e2, -c2 * e1);
+    const double W2 = (fma(b1, d2, e1 * a2) - fma(b2, d1, e2 * a1));
+    const double W1 = (fma(b1, f2, e1 * d2) - fma(b2, f1, e2 * d1));
+    const double W0 = fma(e1, f2, -e2 * f1);
+    const double uu2 = ec[U2], vv1 = ec[V1], ir4 = ec[IR4];
+    const double R3 = fma(2.0 * uu2, U1, -fma(vv1, W2, V0 * ec[W3]));
+    const double R2 = fma(U1, U1, fma(2.0 * uu2, U0, -fma(vv1, W1, V0 * W2)));
+    const double R1 = fma(2.0 * U1, U0, -fma(vv1, W0, V0 * W1));
+    const double R0 = fma(U0, U0, -V0 * W0);
+    double xr[4];
+    const int nr = quartic_real_roots(R3 * ir4, R2 * ir4, R1 * ir4, R0 * ir4, xr);
+    if (nr == 0) return 0.0;
+    // ---- solution-independent pieces
+    const double ptx = ec[PTX] + Eb0 * ec[J0 + 2] + Eb1 * ec[J1 + 2] + Sx;     // total transverse momentum
+    const double pty = ec[PTY] + Eb0 * ec[J0 + 3] + Eb1 * ec[J1 + 3] + Sy;
+    const double visE = ec[S0 + LE] + ec[S1 + LE] + Eb0 + Eb1;
+    const double tvz = ec[S0 + LZ] + Eb0 * ec[J0 + 4], avz = ec[S1 + LZ] + Eb1 * ec[J1 + 4];   // visible p_z per top
+    const double tvE = ec[S0 + LE] + Eb0, avE = ec[S1 + LE] + Eb1;
+    const double tvx = ec[S0 + LX] + Eb0 * ec[J0 + 2], tvy = ec[S0 + LY] + Eb0 * ec[J0 + 3];
+    const double avx = ec[S1 + LX] + Eb1 * ec[J1 + 2], avy = ec[S1 + LY] + Eb1 * ec[J1 + 3];
+    double sum = 0.0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      if (k >= nr) break;
+      double x = xr[k];
+      const double V = fma(vv1, x, V0);
+      if (!(V != 0.0)) continue;
+      double y = -fma(fma(uu2, x, U1), x, U0) / V;
+      // Newton on g1 = |nu| - E_nu(x, y), g2 = |nubar| - E_nubar(Sx - x, Sy - y)
+      double nz, nbz, xb, yb;
+#pragma unroll
+      for (int it = 0; it < kNewton; ++it) {
+        nz = fma(ec[S0 + AX], x, fma(ec[S0 + AY], y, al0));
+        xb = Sx - x; yb = Sy - y;
+        nbz = fma(ec[S1 + AX], xb, fma(ec[S1 + AY], yb, al1));
+        const double n2 = fma(x, x, fma(y, y, nz * nz)), nb2 = fma(xb, xb, fma(yb, yb, nbz * nbz));
+        const double iEn = rsqrt(n2), iEnb = rsqrt(nb2);
+        const double g1 = n2 * iEn - fma(ec[S0 + LAX], x, fma(ec[S0 + LAY], y, la0));
+        const double g2 = nb2 * iEnb - fma(ec[S1 + LAX], xb, fma(ec[S1 + LAY], yb, la1));
+        const double j11 = fma(fma(nz, ec[S0 + AX], x), iEn, -ec[S0 + LAX]);
+        const double j12 = fma(fma(nz, ec[S0 + AY], y), iEn, -ec[S0 + LAY]);
+        const double j21 = -fma(fma(nbz, ec[S1 + AX], xb), iEnb, -ec[S1 + LAX]);
+        const double j22 = -fma(fma(nbz, ec[S1 + AY], yb), iEnb, -ec[S1 + LAY]);
+        const double idet = 1.0 / fma(j11, j22, -j12 * j21);
+        x -= fma(g1, j22, -g2 * j12) * idet;
+        y -= fma(j11, g2, -j21 * g1) * idet;
+      }
+      nz = fma(ec[S0 + AX], x, fma(ec[S0 + AY], y, al0));
+      xb = Sx - x; yb = Sy - y;
+      nbz = fma(ec[S1 + AX], xb, fma(ec[S1 + AY], yb, al1));
+      const double EnL = fma(ec[S0 + LAX], x, fma(ec[S0 + LAY], y, la0));
+      const double EnbL = fma(ec[S1 + LAX], xb, fma(ec[S1 + LAY], yb, la1));
+      if (!(EnL > 0.0 && EnbL > 0.0)) continue;
+      const double En = sqrt(fma(x, x, fma(y, y, nz * nz))), Enb = sqrt(fma(xb, xb, fma(yb, yb, nbz * nbz)));
+      if (!(fabs(En - EnL) <= 1e-9 * (En + EnL) && fabs(Enb - EnbL) <= 1e-9 * (Enb + EnbL))) continue;
+      // Jacobian: E_nu (A x B)/(4 E_l E_b) = nu x d + E_nu (n_l x n_b), x and y components
+      const double px = fma(y, ec[DZ0], fma(-nz, ec[DY0], En * ec[S0 + MX]));
+      const double py = fma(nz, ec[DX0], fma(-x, ec[DZ0], En * ec[S0 + MY]));
+      const double qx = fma(yb, ec[DZ1], fma(-nbz, ec[DY1], Enb * ec[S1 + MX]));
+      const double qy = fma(nbz, ec[DX1], fma(-xb, ec[DZ1], Enb * ec[S1 + MY]));
+      const double xz = fabs(fma(px, qy, -py * qx));
+      // ---- S3: transverse boost O7 of the two tops
+      const double tE = tvE + En, tz = tvz + nz, aE = avE + Enb, az = avz + nbz;
+      const double tx = tvx + x, ty = tvy + y, ax = avx + xb, ay = avy + yb;
+      const double PE = visE + En + Enb, Pz = tz + az;
+      const double iPE = rcp_fast(PE);
+      const double bx = ptx * iPE, by = pty * iPE;
+      const double omb = 1.0 - fma(bx, bx, by * by);
+      if (!(omb > 0.0)) continue;
+      const double gam = rsqrt(omb);
+      const double tEb = gam * (tE - fma(bx, tx, by * ty)), aEb = gam * (aE - fma(bx, ax, by * ay));
+      const double PEb = tEb + aEb;
+      const double x1 = (PEb + Pz) * c.inv_sqrt_s, x2 = (PEb - Pz) * c.inv_sqrt_s;
+      if (!(x1 > 0.0 && x1 < 1.0 && x2 > 0.0 && x2 < 1.0)) continue;
+      const double shat = x1 * x2 * c.S;
+      if (!(4.0 * c.mt2 < shat)) continue;                                     // reading A9
+      // ---- S5: production
+      const double ish = rcp_fast(shat);
+      const double hs = 0.5 * c.sqrt_s * ish;
+      const double tau1 = hs * fma(x1, tEb - tz, x2 * (aEb + az));
+      const double tau2 = hs * fma(x2, tEb + tz, x1 * (aEb - az));
+      const double rho = 4.0 * c.mt2 * ish;
+      const double T = tau1 * tau2, iT = rcp_fast(T);
+      const double tt = fma(tau1, tau1, tau2 * tau2);
+      const double Mgg = fma(iT, 1.0 / 6.0, -0.375) * (tt + rho - 0.25 * rho * rho * iT);
+      const double Mqq = tt + 0.5 * rho;
+      const double prod = fma(c.A_g2, Mgg, (2.0 * c.n_flav * (4.0 / 9.0)) * c.A_q2 * Mqq);
+      const double ws = pdf_pair(c, x1, x2) * ish * prod / xz;
+      if (isfinite(ws)) sum += ws;
+    }
+    // ---- S5: decays (p_t.p_l)(p_b.p_nu) per side; S6: MET TF; S7
+    const double dec = fma(Eb0, ec[S0 + ELK], 0.5 * sW0) * (Eb0 * hD0) * fma(Eb1, ec[S1 + ELK], 0.5 * sW1) * (Eb1 * hD1);
+    const double tmet = exp(ec[MEXP] * fma(g6, g6, g7 * g7));
+    const double w = ec[C0] * tf * tmet * dec * (iEb0 * iEb1) * sum;
+    return isfinite(w) ? w : 0.0;
+  }
+};
+
 }  // namespace memb200
