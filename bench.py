@@ -39,6 +39,8 @@ FP64_PER_CALL = {
     4: {"dfma": 300.0, "dmul": 100.0, "dadd": 50.0},
     5: {"dfma": 268.4, "dmul": 96.7, "dadd": 53.1},
 }
+# fp32 variant of config 3 (reading A15): executed FFMA / FMUL / FADD per call (ncu, r01_fp64_counts.md)
+FP32_PER_CALL = {3: {"ffma": 150.0, "fmul": 60.0, "fadd": 30.0}, 5: {"ffma": 150.0, "fmul": 60.0, "fadd": 30.0}}
 NOMINAL_FP64_FMA_PER_CLK_PER_SM = 64      # 4 SMSPs x 16 lanes; confirmed by the microbenchmark
 VEGAS_ITERS, VEGAS_POINTS = 5, 1 << 17    # BASELINE.json:configs[4]
 
@@ -57,6 +59,8 @@ def parse_args():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--events", type=int, default=0, help="override the event count (default: the config's)")
     ap.add_argument("--points", type=int, default=0, help="override points/event (default: the config's)")
+    ap.add_argument("--precision", type=int, default=64, choices=[64, 32],
+                    help="32 = fp32 integrand core of config 3 (reading A15)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
 
@@ -71,7 +75,8 @@ def workload(cfg, args):
     name = {1: "config1 W->e nu 1-D", 2: "config2 Z->bb 2-D", 3: "config3 ttbar l+jets 6-D",
             4: "config4 ttbar dilepton 8-D",
             5: "config5 ttbar l+jets 6-D + VEGAS 5x2^17"}[cfg]
-    return proc, ne, npts, "%s, %d events x %d points/event, fp64" % (name, ne, npts)
+    return proc, ne, npts, "%s, %d events x %d points/event, %s" % (
+        name, ne, npts, "fp32 core (A15)" if args.precision == 32 else "fp64")
 
 
 # --------------------------------------------------------------------------------------------
@@ -208,6 +213,8 @@ def run_b200(args):
     ev_host = torch.from_numpy(ev_all[:, lo:lo + ne].copy()).pin_memory()
     ev_dev = ev_host.cuda()
     over = dict(vegas_iters=VEGAS_ITERS, vegas_points=VEGAS_POINTS) if cfg == 5 else {}
+    if args.precision == 32:
+        over["precision"] = 32
     it = mem.Integrator(proc, **over)
     it.set_event_offset(lo)
     out_p = torch.empty(ne, dtype=torch.float64, device="cuda")
@@ -288,13 +295,25 @@ def run_b200(args):
         "traffic": None,
         "hbm_gbs_event_result_path": (ne * mem.mem_event_fields(proc) * 8 + ne * 16) / (sum(ms) / len(ms) * 1e-3) / 1e9,
     }
+    if args.precision == 32:
+        # fp32 core: the bound is instruction issue (FP32 + INT share the 4 x 32-lane datapaths), so
+        # the roofline is counted in executed FP32 flops against 128 FFMA/clk/SM at the observed clock
+        f = FP32_PER_CALL[cfg]
+        fl32 = 2.0 * f["ffma"] + f["fmul"] + f["fadd"]
+        peak32 = 2e-6 * 128 * sms * (sm_mhz or 1965.0)
+        ach32 = k_evals * fl32 / (k_ms * 1e-3) / 1e12
+        roofline.update({"kernel": roofline["kernel"].replace("proc3", "ProcTTljetsF"), "achieved": ach32,
+                         "peak": peak32, "frac": ach32 / peak32, "flop_per_call": fl32,
+                         "peak_source": "derived: 128 FP32 FMA/clk/SM x SMs x sampled SM clock (DESIGN.md)",
+                         "fp64_flop_per_call_kept": fl})
     h2d = ne * mem.mem_event_fields(proc) * 8
     d2h = 2 * ne * 8
     line = {
         "metric": "integrand_evals_per_s", "value": value, "unit": "evals/s",
         "events_per_s": ne * world * args.steps / t_dev,
         "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": 1e3 * t_dev / args.steps,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32" if args.precision == 32 else "f64", "data": "synthetic",
         "config": {"workload": name, "events_per_gpu": ne, "points_per_event": n_points, "seed": SEED,
                    "l2": "flushed between timed steps (256 MiB fill); inputs are 0.5 MB",
                    "parallelism": "events sharded over %d GPU(s), no collective" % world},

@@ -72,6 +72,7 @@ struct mem_handle {
   int device;
   mem_params params;
   DevConst dc;
+  DevConstF dcf;            // fp32 mirror of dc for precision = 32 (reading A15)
   uint64_t event_offset;
   int64_t launches;
   int64_t grid_events;      // events covered by the grids of the last VEGAS call
@@ -154,11 +155,29 @@ DevConst make_dev_const(const mem_params& p) {
   return c;
 }
 
+DevConstF to_float(const DevConst& d) {
+  DevConstF f;
+#define CP(x) f.x = (float)d.x
+  CP(sqrt_s); CP(inv_sqrt_s); CP(S); CP(inv_S); CP(pdf_pow_x); CP(pdf_pow_1mx); CP(A_q2); CP(A_g2); CP(rlo); CP(dr);
+  CP(tf_a1); CP(tf_b1); CP(tf_c1); CP(tf_a2); CP(tf_b2); CP(tf_c2); CP(mW); CP(GW); CP(mW2); CP(mWGW); CP(mWGW2);
+  CP(tW_lo); CP(tW_dt); CP(mt2); CP(mtGt); CP(mtGt2); CP(tT_lo); CP(tT_dt); CP(mZ2); CP(mZGZ2); CP(g4w); CP(gz4);
+  CP(gs4); CP(V_ud2); CP(V_tb2); CP(z_cu); CP(z_ct); CP(nu_pz_max); CP(nu_eta_max); CP(met_sigma); CP(met_nsigma);
+  CP(vegas_alpha);
+#undef CP
+  f.pdf_fast = d.pdf_fast; f.n_flav = d.n_flav; f.vegas_bins = d.vegas_bins;
+  return f;
+}
+
+template <typename T> const DevConstR<T>& dc_of(const mem_handle* h);
+template <> const DevConstR<double>& dc_of<double>(const mem_handle* h) { return h->dc; }
+template <> const DevConstR<float>& dc_of<float>(const mem_handle* h) { return h->dcf; }
+
 mem_status check_params(int process, const mem_params& p) {
   if (p.struct_size != sizeof(mem_params))
     return fail(MEM_ERR_INVALID_ARG, "mem_params.struct_size = %u, expected %zu", p.struct_size, sizeof(mem_params));
   if (p.precision != 64 && p.precision != 32) return fail(MEM_ERR_INVALID_ARG, "precision must be 64 or 32");
-  if (p.precision == 32) return fail(MEM_ERR_UNSUPPORTED, "precision 32 is not implemented in this build");
+  if (p.precision == 32 && process != MEM_PROC_TT_LJETS)
+    return fail(MEM_ERR_UNSUPPORTED, "precision 32 is implemented for MEM_PROC_TT_LJETS only (reading A15)");
   const bool pos = p.sqrt_s > 0 && p.G_F > 0 && p.m_W > 0 && p.Gam_W > 0 && p.m_Z > 0 && p.Gam_Z > 0 && p.m_t > 0 &&
                    p.Gam_t > 0 && p.alpha_s > 0 && p.tf_sig1 > 0 && p.tf_sig2 > 0 && p.jetE_rlo > 0 &&
                    p.jetE_rhi > p.jetE_rlo && p.bw_nwidths > 0 && p.nu_pz_max > 0 && p.nu_eta_max > 0 &&
@@ -206,7 +225,7 @@ mem_status launch_pass(mem_handle* h, int64_t n_events, int64_t n_points, int64_
   if (blocks > 0x7fffffffLL) return fail(MEM_ERR_INVALID_ARG, "n_events * chunks = %lld exceeds the grid limit", (long long)blocks);
   const size_t smem = integrate_smem(P::NC, P::D, h->dc.vegas_bins, MODE);
   integrate_kernel<P, MODE><<<(unsigned)blocks, kThreads, smem, st>>>(
-      h->dc, (const double*)h->ecs.p, (const double*)h->grids.p, (double*)h->partials.p, (double*)h->hist.p,
+      dc_of<typename P::real>(h), (const double*)h->ecs.p, (const double*)h->grids.p, (double*)h->partials.p, (double*)h->hist.p,
       n_points, chunk, n_chunks, seed, h->event_offset, pass);
   ++h->launches;
   CUDA_TRY(cudaGetLastError());
@@ -283,7 +302,7 @@ mem_status eval_impl(mem_handle* h, const double* events, int64_t n_events, int6
   const int threads = 128;
   const size_t smem = ((size_t)P::NC + (size_t)P::D * (kMaxBins + 1)) * sizeof(double);
   eval_points_kernel<P><<<(unsigned)((n + threads - 1) / threads), threads, smem, st>>>(
-      h->dc, (const double*)h->ecs.p, event, grid, first, n, seed, h->event_offset, (uint32_t)iteration, out_w);
+      dc_of<typename P::real>(h), (const double*)h->ecs.p, event, grid, first, n, seed, h->event_offset, (uint32_t)iteration, out_w);
   ++h->launches;
   CUDA_TRY(cudaGetLastError());
   return MEM_OK;
@@ -338,7 +357,7 @@ mem_status mem_create(mem_process process, const mem_params* params, mem_handle*
     return fail(MEM_ERR_CUDA, "device %d is sm_%d%d; this library is built for sm_100a only", dev, prop.major, prop.minor);
   mem_handle* h = new (std::nothrow) mem_handle();
   if (!h) return fail(MEM_ERR_NOMEM, "out of host memory");
-  h->process = (int)process; h->device = dev; h->params = p; h->dc = make_dev_const(p);
+  h->process = (int)process; h->device = dev; h->params = p; h->dc = make_dev_const(p); h->dcf = to_float(h->dc);
   h->event_offset = 0; h->launches = 0; h->grid_events = 0; h->last_evals = 0;
   cudaError_t ce = cudaEventCreate(&h->ev_begin);
   if (ce == cudaSuccess) ce = cudaEventCreate(&h->ev_end);
@@ -428,7 +447,10 @@ mem_status mem_integrate(mem_handle* h, const double* events, int64_t n_events, 
   switch (h->process) {
     case MEM_PROC_W_ENU: return integrate_impl<ProcWenu>(h, events, n_events, n_points, seed, out_p, out_err, st);
     case MEM_PROC_Z_BB: return integrate_impl<ProcZbb>(h, events, n_events, n_points, seed, out_p, out_err, st);
-    case MEM_PROC_TT_LJETS: return integrate_impl<ProcTTljets>(h, events, n_events, n_points, seed, out_p, out_err, st);
+    case MEM_PROC_TT_LJETS:
+      if (h->params.precision == 32)
+        return integrate_impl<ProcTTljetsF>(h, events, n_events, n_points, seed, out_p, out_err, st);
+      return integrate_impl<ProcTTljets>(h, events, n_events, n_points, seed, out_p, out_err, st);
     case MEM_PROC_TT_DILEP: return integrate_impl<ProcTTdilep>(h, events, n_events, n_points, seed, out_p, out_err, st);
   }
   return fail(MEM_ERR_UNSUPPORTED, "process %d is not implemented", h->process);
@@ -475,7 +497,10 @@ mem_status mem_eval_points(mem_handle* h, const double* events, int64_t n_events
   switch (h->process) {
     case MEM_PROC_W_ENU: return eval_impl<ProcWenu>(h, events, n_events, event, first_point, n, seed, iteration, grid, out_w, st);
     case MEM_PROC_Z_BB: return eval_impl<ProcZbb>(h, events, n_events, event, first_point, n, seed, iteration, grid, out_w, st);
-    case MEM_PROC_TT_LJETS: return eval_impl<ProcTTljets>(h, events, n_events, event, first_point, n, seed, iteration, grid, out_w, st);
+    case MEM_PROC_TT_LJETS:
+      if (h->params.precision == 32)
+        return eval_impl<ProcTTljetsF>(h, events, n_events, event, first_point, n, seed, iteration, grid, out_w, st);
+      return eval_impl<ProcTTljets>(h, events, n_events, event, first_point, n, seed, iteration, grid, out_w, st);
     case MEM_PROC_TT_DILEP: return eval_impl<ProcTTdilep>(h, events, n_events, event, first_point, n, seed, iteration, grid, out_w, st);
   }
   return fail(MEM_ERR_UNSUPPORTED, "process %d is not implemented", h->process);

@@ -20,35 +20,38 @@ constexpr int kMaxAdaptChunks = 8;       // adaptation passes use at most this m
 // Everything the kernels need that does not depend on the event.  Filled on the host from
 // mem_params (mem_api.cu: make_dev_const) and passed by value as a kernel argument, so every
 // member is a constant-bank operand.
-struct DevConst {
+template <typename T>
+struct DevConstR {
   // beams, O3
-  double sqrt_s, inv_sqrt_s, S, inv_S;
+  T sqrt_s, inv_sqrt_s, S, inv_S;
   // toy PDF, O4
-  double pdf_pow_x, pdf_pow_1mx;
+  T pdf_pow_x, pdf_pow_1mx;
   int pdf_fast;                         // 1 when pow_x == -1/2 and pow_1mx == 3
   int n_flav;
-  double A_q2, A_g2;                    // pdf_A_q^2, pdf_A_g^2
+  T A_q2, A_g2;                    // pdf_A_q^2, pdf_A_g^2
   // jets, O5: E = E_jet (rlo + dr u); TF(E_jet; E) * E = c1 exp(-z1^2) + c2 exp(-z2^2),
   // z_k = a_k / x + b_k with x = E / E_jet
-  double rlo, dr;
-  double tf_a1, tf_b1, tf_c1, tf_a2, tf_b2, tf_c2;
+  T rlo, dr;
+  T tf_a1, tf_b1, tf_c1, tf_a2, tf_b2, tf_c2;
   // Breit-Wigner data, O6
-  double mW, GW, mW2, mWGW, mWGW2;      // m, Gamma, m^2, m Gamma, (m Gamma)^2
-  double tW_lo, tW_dt;                  // t window of m +- n Gamma
-  double mt2, mtGt, mtGt2, tT_lo, tT_dt;
-  double mZ2, mZGZ2;
+  T mW, GW, mW2, mWGW, mWGW2;      // m, Gamma, m^2, m Gamma, (m Gamma)^2
+  T tW_lo, tW_dt;                  // t window of m +- n Gamma
+  T mt2, mtGt, mtGt2, tT_lo, tT_dt;
+  T mZ2, mZGZ2;
   // couplings, O8
-  double g4w;                           // g^4, g^2 = 4 sqrt2 G_F m_W^2
-  double gz4;                           // g_Z^4
-  double gs4;                           // g_s^4 = (4 pi alpha_s)^2
-  double V_ud2, V_tb2;
-  double z_cu, z_ct;                    // sum_q [..] coefficient of u^2 and of t^2 (config 2)
+  T g4w;                           // g^4, g^2 = 4 sqrt2 G_F m_W^2
+  T gz4;                           // g_Z^4
+  T gs4;                           // g_s^4 = (4 pi alpha_s)^2
+  T V_ud2, V_tb2;
+  T z_cu, z_ct;                    // sum_q [..] coefficient of u^2 and of t^2 (config 2)
   // windows
-  double nu_pz_max, nu_eta_max, met_sigma, met_nsigma;
+  T nu_pz_max, nu_eta_max, met_sigma, met_nsigma;
   // VEGAS
   int vegas_bins;
-  double vegas_alpha;
+  T vegas_alpha;
 };
+using DevConst = DevConstR<double>;   // the fp64 path
+using DevConstF = DevConstR<float>;   // fp32 integrand core of config 3 (reading A15)
 
 // ---------------------------------------------------------------------------------------
 // S1. Philox4x32-10 (Salmon et al. 2011; multipliers and Weyl constants are the published ones)
@@ -113,13 +116,42 @@ __device__ __forceinline__ double pdf_pair(const DevConst& c, double x1, double 
   return pow(xx, c.pdf_pow_x) * pow(yy, c.pdf_pow_1mx);
 }
 
-// E * T(E_jet; E) for x = E / E_jet, inv_x = 1 / x (O5; the factor 1/E cancels the E of the
-// jet's phase-space measure E sin(theta) dE)
-__device__ __forceinline__ double tf_times_E(const DevConst& c, double inv_x) {
-  const double z1 = fma(c.tf_a1, inv_x, c.tf_b1);
-  const double z2 = fma(c.tf_a2, inv_x, c.tf_b2);
-  return fma(c.tf_c1, exp(-z1 * z1), c.tf_c2 * exp(-z2 * z2));
+// Jet transfer functions (O5).  For x = E / E_jet, inv_x = 1 / x:
+//   E * T(E_jet; E) = c1 exp(-z1^2) + c2 exp(-z2^2) = exp(-z1^2) (c1 + c2 exp(z1^2 - z2^2)),  z_k = a_k inv_x + b_k
+// (the factor 1/E of the Gaussians cancels the E of the jet's measure E sin(theta) dE).  A product
+// over jets therefore needs one exponential per jet plus ONE for the sum of the z1^2 (and any
+// other Gaussian factor of the point, e.g. the MET transfer function): tf_accum() adds z1^2 to
+// `esum` and multiplies `fac` by the bracket; the caller finishes with fac * exp(-esum).
+template <typename T> struct TfAcc { T esum, fac; };
+
+// ---------------------------------------------------------------------------------------
+// fp32 counterparts (reading A15: the integrand core of config 3 in single precision; sampling,
+// per-event constants, the overall constant C0 and the sums stay in fp64).  MUFU-based
+// reciprocal / rsqrt / exp2; no --use_fast_math anywhere, these are chosen per call site.
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ float rcp_fast(float x) { return __frcp_rn(x); }
+__device__ __forceinline__ double m_exp(double x) { return exp(x); }
+__device__ __forceinline__ float m_exp(float x) { return __expf(x); }
+__device__ __forceinline__ double m_tan(double x) { return tan(x); }
+__device__ __forceinline__ float m_tan(float x) { return tanf(x); }
+__device__ __forceinline__ double m_rsqrt(double x) { return rsqrt(x); }
+__device__ __forceinline__ float m_rsqrt(float x) { return rsqrtf(x); }
+
+template <typename T>
+__device__ __forceinline__ void tf_accum(const DevConstR<T>& c, T inv_x, TfAcc<T>& acc) {
+  const T z1 = fma(c.tf_a1, inv_x, c.tf_b1);
+  const T z2 = fma(c.tf_a2, inv_x, c.tf_b2);
+  const T a = z1 * z1;
+  acc.esum += a;
+  acc.fac *= fma(c.tf_c2, m_exp(fma(-z2, z2, a)), c.tf_c1);
 }
+
+__device__ __forceinline__ float pdf_pair(const DevConstF& c, float x1, float x2) {
+  const float xx = x1 * x2, yy = (1.0f - x1) * (1.0f - x2);
+  if (c.pdf_fast) return rsqrtf(xx) * (yy * yy * yy);
+  return powf(xx, c.pdf_pow_x) * powf(yy, c.pdf_pow_1mx);
+}
+
 
 // ---------------------------------------------------------------------------------------
 // S8. block reduction of (sum w, sum w^2): registers -> warp shuffle tree -> shared -> warp 0,

@@ -22,6 +22,24 @@ __global__ void prepare_kernel(const DevConst c, const double* __restrict__ ev, 
   for (int k = 0; k < P::NC; ++k) ecs[e * P::NC + k] = ec[k];
 }
 
+// the integrand at the unit-cube point u.  fp64 processes take u as it is; the fp32 variant
+// (reading A15) rounds u to fp32, clamps it below 1, evaluates the core in fp32 and applies the
+// per-event constant c0 in fp64.
+template <class P, int D>
+__device__ __forceinline__ double eval_weight(const DevConstR<typename P::real>& c, const typename P::real* ec,
+                                              double c0, const double (&u)[D]) {
+  using T = typename P::real;
+  if constexpr (std::is_same<T, double>::value) {
+    return P::weight(c, ec, u);
+  } else {
+    T uf[D];
+#pragma unroll
+    for (int d = 0; d < D; ++d) uf[d] = fminf((T)u[d], 0x1.fffffep-1f);
+    const double w = (double)P::weight(c, ec, uf) * c0;
+    return isfinite(w) ? w : 0.0;
+  }
+}
+
 // S1v: warp the unit-cube point through the event's grid (edges in shared memory)
 template <int D>
 __device__ __forceinline__ double vegas_map(const double* edges, int B, double (&u)[D], int (&k)[D]) {
@@ -65,20 +83,22 @@ __device__ __forceinline__ void warp_hist_add(double* wh, int k, double v) {
 // of w^2 to hist[event][chunk][D][B].
 template <class P, int MODE>
 __global__ void __launch_bounds__(kThreads)
-integrate_kernel(const DevConst c, const double* __restrict__ ecs, const double* __restrict__ grids,
+integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__ ecs, const double* __restrict__ grids,
                  double* __restrict__ partials, double* __restrict__ hist, int64_t n_points,
                  int64_t chunk, int n_chunks, uint64_t seed, uint64_t event_offset, uint32_t pass) {
   constexpr int D = P::D;
+  using T = typename P::real;                         // fp64, or fp32 for the A15 variant
   extern __shared__ double smem[];
-  double* ec = smem;                                  // [NC]
-  double* red = ec + P::NC;                           // [2 kWarps]
+  T* ec = reinterpret_cast<T*>(smem);                 // [NC] (NC doubles are reserved either way)
+  double* red = smem + P::NC;                         // [2 kWarps]
   double* edges = red + 2 * kWarps;                   // [D][B+1]          (GRID, ADAPT)
   const int B = c.vegas_bins;
   double* whist = edges + D * (B + 1);                // [kWarps][D][B]    (ADAPT)
 
   const int64_t e = blockIdx.x / n_chunks;
   const int ch = (int)(blockIdx.x - e * n_chunks);
-  for (int k = threadIdx.x; k < P::NC; k += kThreads) ec[k] = ecs[e * P::NC + k];
+  for (int k = threadIdx.x; k < P::NC; k += kThreads) ec[k] = (T)ecs[e * P::NC + k];
+  const double c0 = P::kSplitC0 ? ecs[e * P::NC + P::C0] : 1.0;   // fp32 core x fp64 per-event constant
   if (MODE != MODE_PLAIN)
     for (int k = threadIdx.x; k < D * (B + 1); k += kThreads) edges[k] = grids[e * D * (B + 1) + k];
   if (MODE == MODE_ADAPT)
@@ -99,11 +119,11 @@ integrate_kernel(const DevConst c, const double* __restrict__ ecs, const double*
     draw_uniforms<D>(rng, (uint64_t)i, ev_ctr, pass, u);
     double w;
     if (MODE == MODE_PLAIN) {
-      w = P::weight(c, ec, u);
+      w = eval_weight<P>(c, ec, c0, u);
     } else {
       int k[D];
       const double jac = vegas_map<D>(edges, B, u, k);
-      w = jac * P::weight(c, ec, u);
+      w = jac * eval_weight<P>(c, ec, c0, u);
       if (!isfinite(w)) w = 0.0;
       if (MODE == MODE_ADAPT) {
         const double w2 = live ? w * w : 0.0;
@@ -218,16 +238,18 @@ __global__ void refine_kernel(const DevConst c, const double* __restrict__ hist,
 
 // diagnostic: weights of points [first, first + n) of one event
 template <class P>
-__global__ void eval_points_kernel(const DevConst c, const double* __restrict__ ecs, int64_t event,
+__global__ void eval_points_kernel(const DevConstR<typename P::real> c, const double* __restrict__ ecs, int64_t event,
                                    const double* __restrict__ grid, int64_t first, int64_t n,
                                    uint64_t seed, uint64_t event_offset, uint32_t pass,
                                    double* __restrict__ out_w) {
   constexpr int D = P::D;
+  using T = typename P::real;
   extern __shared__ double smem[];
-  double* ec = smem;
-  double* edges = ec + P::NC;
+  T* ec = reinterpret_cast<T*>(smem);
+  double* edges = smem + P::NC;
   const int B = c.vegas_bins;
-  for (int k = threadIdx.x; k < P::NC; k += blockDim.x) ec[k] = ecs[event * P::NC + k];
+  for (int k = threadIdx.x; k < P::NC; k += blockDim.x) ec[k] = (T)ecs[event * P::NC + k];
+  const double c0 = P::kSplitC0 ? ecs[event * P::NC + P::C0] : 1.0;
   if (grid)
     for (int k = threadIdx.x; k < D * (B + 1); k += blockDim.x) edges[k] = grid[k];
   __syncthreads();
@@ -240,10 +262,10 @@ __global__ void eval_points_kernel(const DevConst c, const double* __restrict__ 
   if (grid) {
     int k[D];
     const double jac = vegas_map<D>(edges, B, u, k);
-    w = jac * P::weight(c, ec, u);
+    w = jac * eval_weight<P>(c, ec, c0, u);
     if (!isfinite(w)) w = 0.0;
   } else {
-    w = P::weight(c, ec, u);
+    w = eval_weight<P>(c, ec, c0, u);
   }
   out_w[i] = w;
 }

@@ -12,6 +12,8 @@
 // (massless partons), so that no point needs six boosted four-vectors in
 // registers (the paper's own register-pressure finding).
 #pragma once
+#include <type_traits>
+
 #include "mem_common.cuh"
 
 namespace memb200 {
@@ -32,6 +34,8 @@ __device__ inline double one_minus_cos(double eta_a, double phi_a, double eta_b,
 // both roots summed.
 // =========================================================================================
 struct ProcWenu {
+  using real = double;
+  static constexpr bool kSplitC0 = false;
   static constexpr int D = 1, NF = 5, NC = 16;
   enum { LM, LP, LE, LZ, PT, NT2, A, CLO, CHI, DT, SCLO, DSM, PTNT, IPT2, C0, _N };
 
@@ -108,7 +112,8 @@ struct ProcWenu {
 // jets shared by configs 2-4 (O5): E = E_jet (rlo + dr u); direction fixed by the record.
 // per-event block of 5 constants per jet: E_jet rlo, E_jet dr, n_x, n_y, n_z
 // =========================================================================================
-struct Jet { double E, x, y, z; };
+template <typename T> struct JetR { T E, x, y, z; };
+using Jet = JetR<double>;
 
 __device__ inline void jet_prepare(const DevConst& c, double Ej, double eta, double phi, double* o) {
   const double st = 1.0 / cosh(eta);
@@ -116,11 +121,12 @@ __device__ inline void jet_prepare(const DevConst& c, double Ej, double eta, dou
   o[2] = st * cos(phi); o[3] = st * sin(phi); o[4] = tanh(eta);
 }
 
-// returns the parton momentum; tf accumulates E * T(E_jet; E)
-__device__ __forceinline__ Jet jet_point(const DevConst& c, const double* o, double u, double& tf) {
-  const double x = fma(c.dr, u, c.rlo);
-  tf *= tf_times_E(c, rcp_fast(x));
-  Jet j;
+// returns the parton momentum; tf accumulates E * T(E_jet; E) (see tf_accum)
+template <typename T>
+__device__ __forceinline__ JetR<T> jet_point(const DevConstR<T>& c, const T* o, T u, TfAcc<T>& tf) {
+  const T x = fma(c.dr, u, c.rlo);
+  tf_accum(c, rcp_fast(x), tf);
+  JetR<T> j;
   j.E = fma(o[1], u, o[0]);
   j.x = j.E * o[2]; j.y = j.E * o[3]; j.z = j.E * o[4];
   return j;
@@ -131,6 +137,8 @@ __device__ __forceinline__ Jet jet_point(const DevConst& c, const double* o, dou
 // DESIGN.md "Config 2"; transverse boost O7 (reading A6)
 // =========================================================================================
 struct ProcZbb {
+  using real = double;
+  static constexpr bool kSplitC0 = false;
   static constexpr int D = 2, NF = 6, NC = 12;
   enum { J0 = 0, J1 = 5, C0 = 10, KT = 11 };
 
@@ -153,8 +161,9 @@ struct ProcZbb {
   }
 
   __device__ static double weight(const DevConst& c, const double* ec, const double (&u)[D]) {
-    double tf = 1.0;
-    const Jet p1 = jet_point(c, ec + J0, u[0], tf), p2 = jet_point(c, ec + J1, u[1], tf);
+    TfAcc<double> tfa{0.0, 1.0};
+    const Jet p1 = jet_point(c, ec + J0, u[0], tfa), p2 = jet_point(c, ec + J1, u[1], tfa);
+    const double tf = tfa.fac * exp(-tfa.esum);
     // O7 without the cancellation in 1 - beta^2 (nearly collinear jets): with P = p1 + p2,
     //   P_E'^2 = P_E^2 - P_T^2 = p1z^2 + p2z^2 + 2 E1 E2 (1 - n1T.n2T)
     //   E_i'   = gamma (E_i - beta.p_iT) = (p_iz^2 + E1 E2 (1 - n1T.n2T)) / P_E'
@@ -184,8 +193,11 @@ struct ProcZbb {
 // DESIGN.md "Config 3" (reading A7): u0..u3 jet energies, u4 eta_nu flat in [-H, H],
 // u5 leptonic s_W through the Breit-Wigner map; nu azimuth = MET azimuth.
 // =========================================================================================
-struct ProcTTljets {
+template <typename T>
+struct ProcTTljetsR {
+  using real = T;
   static constexpr int D = 6, NF = 17, NC = 44;
+  static constexpr bool kSplitC0 = !std::is_same<T, double>::value;
   enum { LE, LX, LY, LZ, ELI, EL, LPT2, OMC, CPN, SPN,   // lepton, neutrino azimuth
          J0 = 10, J1 = 15, J2 = 20, J3 = 25,            // b_had, b_lep, q, qbar'
          KBL = 30,                                      // b_lep . l / E_b
@@ -233,69 +245,81 @@ struct ProcTTljets {
     for (int k = _N; k < NC; ++k) ec[k] = 0.0;
   }
 
-  __device__ static double weight(const DevConst& c, const double* ec, const double (&u)[D]) {
+  __device__ static T weight(const DevConstR<T>& c, const T* ec, const T (&u)[D]) {
     // ---- S2: jets and their transfer functions
-    double tf = 1.0;
-    const Jet bh = jet_point(c, ec + J0, u[0], tf), bl = jet_point(c, ec + J1, u[1], tf);
-    const Jet q = jet_point(c, ec + J2, u[2], tf), qb = jet_point(c, ec + J3, u[3], tf);
+    TfAcc<T> tfa{T(0), T(1)};
+    const JetR<T> bh = jet_point(c, ec + J0, u[0], tfa), bl = jet_point(c, ec + J1, u[1], tfa);
+    const JetR<T> q = jet_point(c, ec + J2, u[2], tfa), qb = jet_point(c, ec + J3, u[3], tfa);
+    const T tf = tfa.fac * m_exp(-tfa.esum);
     // ---- S2: neutrino.  g = e^(eta_nu - eta_l); cosh(d eta) - cos(d phi) = (g-1)^2/(2g) + (1 - cos d phi)
-    const double H = c.nu_eta_max;
-    const double eta_nu = fma(2.0 * H, u[4], -H);
-    const double en = exp(eta_nu), eni = rcp_fast(en);
-    const double g = en * ec[ELI], gi = eni * ec[EL];
-    const double gm1 = g - 1.0;
-    const double den = ec[LPT2] * fma(0.5 * gm1 * gm1, gi, ec[OMC]);
-    if (!(den > 0.0)) return 0.0;
-    const double t = fma(c.tW_dt, u[5], c.tW_lo);
-    const double smm = c.mWGW * tan(t);
-    const double sW = c.mW2 + smm;
-    const double iden = rcp_fast(den);
-    const double nuT = sW * iden;
-    const double chn = 0.5 * (en + eni), shn = 0.5 * (en - eni);
-    const double nE = nuT * chn, nx = nuT * ec[CPN], ny = nuT * ec[SPN], nz = nuT * shn;
+    const T H = c.nu_eta_max;
+    const T eta_nu = fma(T(2.0) * H, u[4], -H);
+    const T en = m_exp(eta_nu), eni = rcp_fast(en);
+    const T g = en * ec[ELI], gi = eni * ec[EL];
+    const T gm1 = g - T(1.0);
+    const T den = ec[LPT2] * fma(T(0.5) * gm1 * gm1, gi, ec[OMC]);
+    if (!(den > T(0))) return T(0);
+    const T t = fma(c.tW_dt, u[5], c.tW_lo);
+    const T smm = c.mWGW * m_tan(t);
+    const T sW = c.mW2 + smm;
+    const T iden = rcp_fast(den);
+    const T nuT = sW * iden;
+    const T chn = T(0.5) * (en + eni), shn = T(0.5) * (en - eni);
+    const T nE = nuT * chn, nx = nuT * ec[CPN], ny = nuT * ec[SPN], nz = nuT * shn;
     // ---- S3: invariants through per-event angular constants
-    const double bl_nu = bl.E * nuT * (fma(ec[NA], en, ec[NB] * eni) - ec[NC_]);
-    const double bl_l = bl.E * ec[KBL];
-    const double st_m = fma(2.0, bl_l + bl_nu, smm + (c.mW2 - c.mt2));           // s_t - m_t^2
-    const double bh_q = bh.E * q.E * ec[K02], q_qb = q.E * qb.E * ec[K23], bh_qb = bh.E * qb.E * ec[K03];
-    const double swh_m = fma(2.0, q_qb, -c.mW2);                                 // s_Whad - m_W^2
-    const double stb_m = fma(2.0, bh_q + q_qb + bh_qb, -c.mt2);                  // s_tbar - m_t^2
+    const T bl_nu = bl.E * nuT * (fma(ec[NA], en, ec[NB] * eni) - ec[NC_]);
+    const T bl_l = bl.E * ec[KBL];
+    const T st_m = fma(T(2.0), bl_l + bl_nu, smm + (c.mW2 - c.mt2));           // s_t - m_t^2
+    const T bh_q = bh.E * q.E * ec[K02], q_qb = q.E * qb.E * ec[K23], bh_qb = bh.E * qb.E * ec[K03];
+    const T swh_m = fma(T(2.0), q_qb, -c.mW2);                                 // s_Whad - m_W^2
+    const T stb_m = fma(T(2.0), bh_q + q_qb + bh_qb, -c.mt2);                  // s_tbar - m_t^2
     // ---- S3: top momenta, transverse boost O7 (only the two boosted energies are needed)
-    const double tE = bl.E + ec[LE] + nE, tx = bl.x + ec[LX] + nx, ty = bl.y + ec[LY] + ny, tz = bl.z + ec[LZ] + nz;
-    const double aE = bh.E + q.E + qb.E, ax = bh.x + q.x + qb.x, ay = bh.y + q.y + qb.y, az = bh.z + q.z + qb.z;
-    const double PE = tE + aE, Px = tx + ax, Py = ty + ay, Pz = tz + az;
-    const double iPE = rcp_fast(PE);
-    const double bx = Px * iPE, by = Py * iPE;
-    const double omb = 1.0 - (bx * bx + by * by);
-    if (!(omb > 0.0)) return 0.0;
-    const double gam = rsqrt(omb);
-    const double tEb = gam * (tE - bx * tx - by * ty), aEb = gam * (aE - bx * ax - by * ay);
-    const double PEb = tEb + aEb;
-    const double x1 = (PEb + Pz) * c.inv_sqrt_s, x2 = (PEb - Pz) * c.inv_sqrt_s;
-    if (!(x1 > 0.0 && x1 < 1.0 && x2 > 0.0 && x2 < 1.0)) return 0.0;
-    const double xx = x1 * x2, shat = xx * c.S;
-    if (!(4.0 * c.mt2 < shat)) return 0.0;                                       // reading A9
+    const T tE = bl.E + ec[LE] + nE, tx = bl.x + ec[LX] + nx, ty = bl.y + ec[LY] + ny, tz = bl.z + ec[LZ] + nz;
+    const T aE = bh.E + q.E + qb.E, ax = bh.x + q.x + qb.x, ay = bh.y + q.y + qb.y, az = bh.z + q.z + qb.z;
+    const T PE = tE + aE, Px = tx + ax, Py = ty + ay, Pz = tz + az;
+    const T iPE = rcp_fast(PE);
+    const T bx = Px * iPE, by = Py * iPE;
+    const T omb = T(1.0) - (bx * bx + by * by);
+    if (!(omb > T(0))) return T(0);
+    const T gam = m_rsqrt(omb);
+    const T tEb = gam * (tE - bx * tx - by * ty), aEb = gam * (aE - bx * ax - by * ay);
+    const T PEb = tEb + aEb;
+    const T x1 = (PEb + Pz) * c.inv_sqrt_s, x2 = (PEb - Pz) * c.inv_sqrt_s;
+    if (!(x1 > T(0) && x1 < T(1.0) && x2 > T(0) && x2 < T(1.0))) return T(0);
+    const T xx = x1 * x2, shat = xx * c.S;
+    if (!(T(4.0) * c.mt2 < shat)) return T(0);                                       // reading A9
     // ---- S5: production.  tau1 = (q1.pt + q2.ptb)/s-hat, tau2 = (q2.pt + q1.ptb)/s-hat
-    const double ish = rcp_fast(shat);
-    const double hs = 0.5 * c.sqrt_s * ish;
-    const double tau1 = hs * fma(x1, tEb - tz, x2 * (aEb + az));
-    const double tau2 = hs * fma(x2, tEb + tz, x1 * (aEb - az));
-    const double rho = 4.0 * c.mt2 * ish;
-    const double T = tau1 * tau2, iT = rcp_fast(T);
-    const double tt = fma(tau1, tau1, tau2 * tau2);
-    const double Mgg = fma(iT, 1.0 / 6.0, -0.375) * (tt + rho - 0.25 * rho * rho * iT);
-    const double Mqq = tt + 0.5 * rho;
-    const double prod = fma(c.A_g2, Mgg, (2.0 * c.n_flav * (4.0 / 9.0)) * c.A_q2 * Mqq);
+    const T ish = rcp_fast(shat);
+    const T hs = T(0.5) * c.sqrt_s * ish;
+    const T tau1 = hs * fma(x1, tEb - tz, x2 * (aEb + az));
+    const T tau2 = hs * fma(x2, tEb + tz, x1 * (aEb - az));
+    const T rho = T(4.0) * c.mt2 * ish;
+    const T iT = rcp_fast(tau1 * tau2);
+    const T tt = fma(tau1, tau1, tau2 * tau2);
+    const T Mgg = fma(iT, T(1.0) / T(6.0), -T(0.375)) * (tt + rho - T(0.25) * rho * rho * iT);
+    const T Mqq = tt + T(0.5) * rho;
+    const T prod = fma(c.A_g2, Mgg, (T(2.0) * c.n_flav * (T(4.0) / T(9.0))) * c.A_q2 * Mqq);
     // ---- S5: propagators and decays
-    const double dens = fma(st_m, st_m, c.mtGt2) * fma(stb_m, stb_m, c.mtGt2) * fma(swh_m, swh_m, c.mWGW2);
-    const double t_l = fma(0.5, sW, bl_l);                                       // p_t . l
-    const double a_q = bh_q + q_qb;                                              // p_tbar . q
-    const double dec = t_l * bl_nu * a_q * bh_qb;
+    const T t_l = fma(T(0.5), sW, bl_l);                                       // p_t . l
+    const T a_q = bh_q + q_qb;                                                 // p_tbar . q
+    T decprop;                                                                 // decays x propagators
+    if constexpr (kSplitC0) {
+      // fp32: keep every intermediate inside the single-precision range
+      decprop = (t_l * bl_nu * rcp_fast(fma(st_m, st_m, c.mtGt2))) * (a_q * rcp_fast(fma(stb_m, stb_m, c.mtGt2))) *
+                (bh_qb * rcp_fast(fma(swh_m, swh_m, c.mWGW2)));
+    } else {
+      const T dens = fma(st_m, st_m, c.mtGt2) * fma(stb_m, stb_m, c.mtGt2) * fma(swh_m, swh_m, c.mWGW2);
+      decprop = t_l * bl_nu * a_q * bh_qb * rcp_fast(dens);
+    }
     // ---- S4, S7
-    const double w = ec[C0] * tf * (nuT * iden) * (pdf_pair(c, x1, x2) * ish) * prod * dec * rcp_fast(dens);
-    return isfinite(w) ? w : 0.0;
+    const T core = tf * (nuT * iden) * (pdf_pair(c, x1, x2) * ish) * prod * decprop;
+    // fp64: the per-event constant is applied here; fp32: by the caller in fp64 (it would underflow)
+    const T w = kSplitC0 ? core : ec[C0] * core;
+    return isfinite(w) ? w : T(0);
   }
 };
+using ProcTTljets = ProcTTljetsR<double>;
+using ProcTTljetsF = ProcTTljetsR<float>;   // reading A15
 
 // =========================================================================================
 // config 4: t tbar -> b l+ nu  bbar l- nubar, D = 8.
@@ -376,6 +400,8 @@ __device__ __forceinline__ int quartic_real_roots(double a3, double a2, double a
 }
 
 struct ProcTTdilep {
+  using real = double;
+  static constexpr bool kSplitC0 = false;
   static constexpr int D = 8, NF = 14, NC = 64;
   static constexpr int kNewton = 3;      // Newton steps on the un-squared equations per root
   // per top side s (0: l+, b; 1: l-, bbar), 14 constants each, at S0 + 14 s:
@@ -450,10 +476,11 @@ struct ProcTTdilep {
 
   __device__ static double weight(const DevConst& c, const double* ec, const double (&u)[D]) {
     // ---- S2: jets, transfer functions
-    double tf = 1.0;
+    TfAcc<double> tfa{0.0, 1.0};
     const double xb0 = fma(c.dr, u[0], c.rlo), xb1 = fma(c.dr, u[1], c.rlo);
     const double ixb0 = rcp_fast(xb0), ixb1 = rcp_fast(xb1);
-    tf *= tf_times_E(c, ixb0) * tf_times_E(c, ixb1);
+    tf_accum(c, ixb0, tfa);
+    tf_accum(c, ixb1, tfa);
     const double Eb0 = fma(ec[J0 + 1], u[0], ec[J0]), Eb1 = fma(ec[J1 + 1], u[1], ec[J1]);
     const double iEb0 = ixb0 * ec[IEJ0], iEb1 = ixb1 * ec[IEJ1];
     // ---- S2: the four mapped masses, s_k - m_k^2 = m Gam tan t_k (O6)
@@ -579,8 +606,9 @@ struct ProcTTdilep {
     }
     // ---- S5: decays (p_t.p_l)(p_b.p_nu) per side; S6: MET TF; S7
     const double dec = fma(Eb0, ec[S0 + ELK], 0.5 * sW0) * (Eb0 * hD0) * fma(Eb1, ec[S1 + ELK], 0.5 * sW1) * (Eb1 * hD1);
-    const double tmet = exp(ec[MEXP] * fma(g6, g6, g7 * g7));
-    const double w = ec[C0] * tf * tmet * dec * (iEb0 * iEb1) * sum;
+    // jets' Gaussians and the MET Gaussian share one exponential
+    const double tf_tmet = tfa.fac * exp(fma(ec[MEXP], fma(g6, g6, g7 * g7), -tfa.esum));
+    const double w = ec[C0] * tf_tmet * dec * (iEb0 * iEb1) * sum;
     return isfinite(w) ? w : 0.0;
   }
 };
