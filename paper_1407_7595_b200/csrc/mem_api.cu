@@ -184,6 +184,7 @@ mem_status check_params(int process, const mem_params& p) {
                    p.met_sigma > 0 && p.met_nsigma > 0;
   if (!pos) return fail(MEM_ERR_INVALID_ARG, "mem_params: a constant that must be positive is not");
   if (!(p.tf_w_tail >= 0.0 && p.tf_w_tail <= 1.0)) return fail(MEM_ERR_INVALID_ARG, "tf_w_tail outside [0,1]");
+  if (p.nu_eta_max > 50.0) return fail(MEM_ERR_INVALID_ARG, "nu_eta_max above 50");
   if (p.n_flav < 1 || p.n_flav > 5) return fail(MEM_ERR_INVALID_ARG, "n_flav outside 1..5");
   if (p.bw_nwidths * p.Gam_W >= p.m_W || p.bw_nwidths * p.Gam_t >= p.m_t)
     return fail(MEM_ERR_INVALID_ARG, "bw_nwidths * Gamma must stay below the mass");

@@ -81,8 +81,15 @@ __device__ __forceinline__ void warp_hist_add(double* wh, int k, double v) {
 // sums go registers -> warp shuffle -> shared -> partials[event][chunk] in a fixed order.
 // MODE_GRID/ADAPT: grids = [n_events][D][B+1].  MODE_ADAPT also writes the block's histogram
 // of w^2 to hist[event][chunk][D][B].
+// Resident blocks per SM the register allocation aims at (measured on B200, profiles/r01_variants.md):
+// the plain config-1/2/3 kernels (no register cap: 64/63/126 registers, no spills) are bound by FP64 issue and
+// gain nothing from more warps; the divergent config-4 kernel and the VEGAS passes (shuffle/match
+// latency) gain 43 % / 7 % from 3 blocks at 80 registers.
 template <class P, int MODE>
-__global__ void __launch_bounds__(kThreads)
+constexpr int min_blocks() { return (P::kHeavy || MODE != MODE_PLAIN) ? 3 : 0; }   // 0 = no cap
+
+template <class P, int MODE>
+__global__ void __launch_bounds__(kThreads, min_blocks<P, MODE>())
 integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__ ecs, const double* __restrict__ grids,
                  double* __restrict__ partials, double* __restrict__ hist, int64_t n_points,
                  int64_t chunk, int n_chunks, uint64_t seed, uint64_t event_offset, uint32_t pass) {

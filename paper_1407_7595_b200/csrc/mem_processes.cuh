@@ -35,6 +35,7 @@ __device__ inline double one_minus_cos(double eta_a, double phi_a, double eta_b,
 // =========================================================================================
 struct ProcWenu {
   using real = double;
+  static constexpr bool kHeavy = false;   // see min_blocks() in mem_kernels.cuh
   static constexpr bool kSplitC0 = false;
   static constexpr int D = 1, NF = 5, NC = 16;
   enum { LM, LP, LE, LZ, PT, NT2, A, CLO, CHI, DT, SCLO, DSM, PTNT, IPT2, C0, _N };
@@ -132,12 +133,22 @@ __device__ __forceinline__ JetR<T> jet_point(const DevConstR<T>& c, const T* o, 
   return j;
 }
 
+// parton momentum alone (the transfer functions are accumulated separately)
+template <typename T>
+__device__ __forceinline__ JetR<T> jet_mom(const T* o, T u) {
+  JetR<T> j;
+  j.E = fma(o[1], u, o[0]);
+  j.x = j.E * o[2]; j.y = j.E * o[3]; j.z = j.E * o[4];
+  return j;
+}
+
 // =========================================================================================
 // config 2: q qbar -> Z -> b bbar, D = 2.  rec = [E1, eta1, phi1, E2, eta2, phi2]
 // DESIGN.md "Config 2"; transverse boost O7 (reading A6)
 // =========================================================================================
 struct ProcZbb {
   using real = double;
+  static constexpr bool kHeavy = false;   // see min_blocks() in mem_kernels.cuh
   static constexpr bool kSplitC0 = false;
   static constexpr int D = 2, NF = 6, NC = 12;
   enum { J0 = 0, J1 = 5, C0 = 10, KT = 11 };
@@ -196,6 +207,7 @@ struct ProcZbb {
 template <typename T>
 struct ProcTTljetsR {
   using real = T;
+  static constexpr bool kHeavy = false;
   static constexpr int D = 6, NF = 17, NC = 44;
   static constexpr bool kSplitC0 = !std::is_same<T, double>::value;
   enum { LE, LX, LY, LZ, ELI, EL, LPT2, OMC, CPN, SPN,   // lepton, neutrino azimuth
@@ -246,23 +258,34 @@ struct ProcTTljetsR {
   }
 
   __device__ static T weight(const DevConstR<T>& c, const T* ec, const T (&u)[D]) {
-    // ---- S2: jets and their transfer functions
-    TfAcc<T> tfa{T(0), T(1)};
-    const JetR<T> bh = jet_point(c, ec + J0, u[0], tfa), bl = jet_point(c, ec + J1, u[1], tfa);
-    const JetR<T> q = jet_point(c, ec + J2, u[2], tfa), qb = jet_point(c, ec + J3, u[3], tfa);
-    const T tf = tfa.fac * m_exp(-tfa.esum);
-    // ---- S2: neutrino.  g = e^(eta_nu - eta_l); cosh(d eta) - cos(d phi) = (g-1)^2/(2g) + (1 - cos d phi)
+    // ---- S2: jet energy fractions x_j = E_j / E_jet, neutrino rapidity.
+    // g = e^(eta_nu - eta_l); cosh(d eta) - cos(d phi) = ((g-1)^2/2 + (1 - cos d phi) g) / g =: denp / (LPT2 g)
+    const T x0 = fma(c.dr, u[0], c.rlo), x1j = fma(c.dr, u[1], c.rlo), x2j = fma(c.dr, u[2], c.rlo), x3 = fma(c.dr, u[3], c.rlo);
     const T H = c.nu_eta_max;
     const T eta_nu = fma(T(2.0) * H, u[4], -H);
-    const T en = m_exp(eta_nu), eni = rcp_fast(en);
-    const T g = en * ec[ELI], gi = eni * ec[EL];
+    const T en = m_exp(eta_nu);
+    const T g = en * ec[ELI];
     const T gm1 = g - T(1.0);
-    const T den = ec[LPT2] * fma(T(0.5) * gm1 * gm1, gi, ec[OMC]);
-    if (!(den > T(0))) return T(0);
+    const T denp = ec[LPT2] * fma(T(0.5) * gm1, gm1, ec[OMC] * g);
+    if (!(denp > T(0))) return T(0);
+    // one reciprocal for the six divisors (product tree, then back-substitution)
+    const T p01 = x0 * x1j, p23 = x2j * x3, p45 = en * denp, p03 = p01 * p23;
+    const T inv = rcp_fast(p03 * p45);
+    const T i45 = inv * p03, i03 = inv * p45;
+    const T eni = i45 * denp, idenp = i45 * en;
+    const T i01 = i03 * p23, i23 = i03 * p01;
+    const T ix0 = i01 * x1j, ix1 = i01 * x0, ix2 = i23 * x3, ix3 = i23 * x2j;
+    // ---- S6: transfer functions (one exponential per jet and one for the sum, see tf_accum)
+    TfAcc<T> tfa{T(0), T(1)};
+    tf_accum(c, ix0, tfa); tf_accum(c, ix1, tfa); tf_accum(c, ix2, tfa); tf_accum(c, ix3, tfa);
+    const T tf = tfa.fac * m_exp(-tfa.esum);
+    const JetR<T> bh = jet_mom(ec + J0, u[0]), bl = jet_mom(ec + J1, u[1]);
+    const JetR<T> q = jet_mom(ec + J2, u[2]), qb = jet_mom(ec + J3, u[3]);
+    // ---- S2: neutrino from the mapped leptonic W mass
     const T t = fma(c.tW_dt, u[5], c.tW_lo);
     const T smm = c.mWGW * m_tan(t);
     const T sW = c.mW2 + smm;
-    const T iden = rcp_fast(den);
+    const T iden = g * idenp;                                                    // 1 / (2 pT_l (cosh - cos))
     const T nuT = sW * iden;
     const T chn = T(0.5) * (en + eni), shn = T(0.5) * (en - eni);
     const T nE = nuT * chn, nx = nuT * ec[CPN], ny = nuT * ec[SPN], nz = nuT * shn;
@@ -277,12 +300,11 @@ struct ProcTTljetsR {
     const T tE = bl.E + ec[LE] + nE, tx = bl.x + ec[LX] + nx, ty = bl.y + ec[LY] + ny, tz = bl.z + ec[LZ] + nz;
     const T aE = bh.E + q.E + qb.E, ax = bh.x + q.x + qb.x, ay = bh.y + q.y + qb.y, az = bh.z + q.z + qb.z;
     const T PE = tE + aE, Px = tx + ax, Py = ty + ay, Pz = tz + az;
-    const T iPE = rcp_fast(PE);
-    const T bx = Px * iPE, by = Py * iPE;
-    const T omb = T(1.0) - (bx * bx + by * by);
-    if (!(omb > T(0))) return T(0);
-    const T gam = m_rsqrt(omb);
-    const T tEb = gam * (tE - bx * tx - by * ty), aEb = gam * (aE - bx * ax - by * ay);
+    // gamma (E - beta.p) = (E P_E - p_T.P_T) / sqrt(P_E^2 - P_T^2): no division by P_E
+    const T M2 = fma(PE, PE, -fma(Px, Px, Py * Py));
+    if (!(M2 > T(0))) return T(0);
+    const T rM = m_rsqrt(M2);
+    const T tEb = rM * fma(tE, PE, -fma(Px, tx, Py * ty)), aEb = rM * fma(aE, PE, -fma(Px, ax, Py * ay));
     const T PEb = tEb + aEb;
     const T x1 = (PEb + Pz) * c.inv_sqrt_s, x2 = (PEb - Pz) * c.inv_sqrt_s;
     if (!(x1 > T(0) && x1 < T(1.0) && x2 > T(0) && x2 < T(1.0))) return T(0);
@@ -401,6 +423,7 @@ __device__ __forceinline__ int quartic_real_roots(double a3, double a2, double a
 
 struct ProcTTdilep {
   using real = double;
+  static constexpr bool kHeavy = true;   // see min_blocks() in mem_kernels.cuh
   static constexpr bool kSplitC0 = false;
   static constexpr int D = 8, NF = 14, NC = 64;
   static constexpr int kNewton = 3;      // Newton steps on the un-squared equations per root
