@@ -62,6 +62,8 @@ def parse_args():
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32],
                     help="32 = fp32 integrand core of config 3 (reading A15)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true",
+                    help="config-5 sweep of BASELINE.json:configs[4]: events x final points, one JSON line")
     return ap.parse_args()
 
 
@@ -340,9 +342,57 @@ def run_b200(args):
     print(json.dumps(line), flush=True)
 
 
+def run_sweep(args):
+    """BASELINE.json:configs[4]: events in {256, 4096, 65536} x N_f in {2^12..2^22}, 5 adaptation passes of
+    N_a = max(N_f / 8, 2^9) points (the base cell's ratio), then the final pass.  One GPU, device-resident
+    inputs, CUDA events, L2 flushed between steps."""
+    import torch
+
+    import paper_1407_7595_b200 as mem
+    from paper_1407_7595_b200 import workloads as wl
+
+    torch.cuda.set_device(0)
+    proc = wl.TT_LJETS
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    cells = []
+    for ne in (256, 4096, 65536):
+        ev_dev = torch.from_numpy(wl.make_events(proc, ne)).cuda()
+        out_p = torch.empty(ne, dtype=torch.float64, device="cuda")
+        out_err = torch.empty_like(out_p)
+        for lg in range(12, 23):
+            n_f = 1 << lg
+            n_a = max(n_f // 8, 1 << 9)
+            over = dict(vegas_iters=VEGAS_ITERS, vegas_points=n_a)
+            if args.precision == 32:
+                over["precision"] = 32
+            with mem.Integrator(proc, **over) as it:
+                it.integrate(ev_dev, n_f, SEED, out_p=out_p, out_err=out_err)       # warm-up, sizes the workspace
+                torch.cuda.synchronize()
+                ms = []
+                for _ in range(max(1, args.steps if ne * n_f < (1 << 34) else 1)):
+                    flush.fill_(0)
+                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record()
+                    it.integrate(ev_dev, n_f, SEED, out_p=out_p, out_err=out_err)
+                    b.record()
+                    b.synchronize()
+                    ms.append(a.elapsed_time(b))
+            t = min(ms)
+            evals = ne * (n_f + VEGAS_ITERS * n_a)
+            cells.append({"events": ne, "final_points": n_f, "adapt_points": n_a, "ms": t,
+                          "evals_per_s": evals / (t * 1e-3), "events_per_s": ne / (t * 1e-3),
+                          "mean_rel_err": float((out_err[out_p > 0] / out_p[out_p > 0]).mean())})
+    print(json.dumps({"metric": "integrand_evals_per_s", "unit": "evals/s", "n_gpus": 1, "data": "synthetic",
+                      "dtype": "f32" if args.precision == 32 else "f64",
+                      "config": {"workload": "config5 sweep: t tbar l+jets 6-D, VEGAS 5 x N_a + N_f, 50 bins/dim"},
+                      "sweep": cells}), flush=True)
+
+
 def main():
     args = parse_args()
-    if args.impl == "reference":
+    if args.sweep:
+        run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_b200(args)
