@@ -684,14 +684,55 @@ template <typename R> R weight_tt_dilep(const orc_params* p, const double* rec, 
   return std::isfinite((double)w) ? w : R(0);
 }
 
+// NEXT-1 (Eq. 7: "The outer sum is over all permutations of assigning measured
+// jets to partons in the matrix element").  The sum over
+// assignments sits outside the integral, i.e. every sample point is evaluated for each assignment:
+// w(u) = sum_sigma w(record with its jets reordered by sigma, u).  Parton role r takes measured jet
+// sigma[r]; the energy variable u_r stays with the role.  Assignments in lexicographic order.
+inline int jet_perms(int process, int n_perm, int perm[24][4]) {
+  static const int id[4] = {0, 1, 2, 3};
+  int n = 0;
+  auto push = [&](int a, int b, int c, int d) { perm[n][0] = a; perm[n][1] = b; perm[n][2] = c; perm[n][3] = d; ++n; };
+  if (process == ORC_TT_LJETS && n_perm == 24) {
+    for (int a = 0; a < 4; ++a) for (int b = 0; b < 4; ++b) for (int c = 0; c < 4; ++c) for (int d = 0; d < 4; ++d)
+      if (a != b && a != c && a != d && b != c && b != d && c != d) push(a, b, c, d);
+  } else if (process == ORC_TT_LJETS && n_perm == 4) {
+    push(0, 1, 2, 3); push(0, 1, 3, 2); push(1, 0, 2, 3); push(1, 0, 3, 2);
+  } else if (process == ORC_TT_DILEP && n_perm == 2) {
+    push(0, 1, 2, 3); push(1, 0, 2, 3);
+  } else {
+    push(id[0], id[1], id[2], id[3]);
+  }
+  return n;
+}
+
+template <typename R> R weight_permuted(int process, const orc_params* p, const double* rec, const double* u,
+                                        double* dbg) {
+  int perm[24][4];
+  const int n = jet_perms(process, p->n_perm, perm);
+  const int first_jet = (process == ORC_TT_LJETS) ? 3 : 6;   // record offset of the first (E, eta, phi) triple
+  const int n_jets = (process == ORC_TT_LJETS) ? 4 : 2;
+  const int nf = (process == ORC_TT_LJETS) ? 17 : 14;
+  R sum = R(0);
+  for (int k = 0; k < n; ++k) {
+    double r2[32];
+    for (int f = 0; f < nf; ++f) r2[f] = rec[f];
+    for (int role = 0; role < n_jets; ++role)
+      for (int c = 0; c < 3; ++c) r2[first_jet + 3 * role + c] = rec[first_jet + 3 * perm[k][role] + c];
+    sum += (process == ORC_TT_LJETS) ? weight_tt_ljets<R>(p, r2, u, k == 0 ? dbg : nullptr)
+                                     : weight_tt_dilep<R>(p, r2, u, k == 0 ? dbg : nullptr);
+  }
+  return sum;
+}
+
 template <typename R> double weight_any(int process, const orc_params* p, const double* rec, const double* u,
                                         double* dbg) {
   R w = R(0);
   switch (process) {
     case ORC_W_ENU: w = weight_w_enu<R>(p, rec, u, dbg); break;
     case ORC_Z_BB: w = weight_z_bb<R>(p, rec, u, dbg); break;
-    case ORC_TT_LJETS: w = weight_tt_ljets<R>(p, rec, u, dbg); break;
-    case ORC_TT_DILEP: w = weight_tt_dilep<R>(p, rec, u, dbg); break;
+    case ORC_TT_LJETS: w = weight_permuted<R>(process, p, rec, u, dbg); break;
+    case ORC_TT_DILEP: w = weight_permuted<R>(process, p, rec, u, dbg); break;
     default: return std::nan("");
   }
   double wd = (double)w;

@@ -37,7 +37,11 @@ typedef struct orc_params {
   double vegas_alpha;
   int64_t vegas_points;
   int32_t vegas_iters, vegas_bins;
-  int32_t n_flav, reserved;
+  int32_t n_flav;
+  /* NEXT-1, Eq. 7 "sum over all permutations of assigning measured jets to partons":
+   * 0 or 1 = the record order only; ORC_TT_LJETS: 4 = b-tags known (the two b jets swapped x the two
+   * light jets swapped), 24 = all assignments; ORC_TT_DILEP: 2 = both b assignments. */
+  int32_t n_perm;
 } orc_params;
 
 int  orc_params_default(int process, orc_params* p);
