@@ -61,6 +61,8 @@ def parse_args():
     ap.add_argument("--points", type=int, default=0, help="override points/event (default: the config's)")
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32],
                     help="32 = fp32 integrand core of config 3 (reading A15)")
+    ap.add_argument("--perm", type=int, default=0,
+                    help="jet-parton assignments summed per point (NEXT-1): config 3/5: 4 or 24, config 4: 2")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true",
                     help="config-5 sweep of BASELINE.json:configs[4]: events x final points, one JSON line")
@@ -77,8 +79,9 @@ def workload(cfg, args):
     name = {1: "config1 W->e nu 1-D", 2: "config2 Z->bb 2-D", 3: "config3 ttbar l+jets 6-D",
             4: "config4 ttbar dilepton 8-D",
             5: "config5 ttbar l+jets 6-D + VEGAS 5x2^17"}[cfg]
-    return proc, ne, npts, "%s, %d events x %d points/event, %s" % (
-        name, ne, npts, "fp32 core (A15)" if args.precision == 32 else "fp64")
+    return proc, ne, npts, "%s, %d events x %d points/event, %s%s" % (
+        name, ne, npts, "fp32 core (A15)" if args.precision == 32 else "fp64",
+        ", %d jet-parton assignments per point" % args.perm if args.perm > 1 else "")
 
 
 # --------------------------------------------------------------------------------------------
@@ -217,6 +220,8 @@ def run_b200(args):
     over = dict(vegas_iters=VEGAS_ITERS, vegas_points=VEGAS_POINTS) if cfg == 5 else {}
     if args.precision == 32:
         over["precision"] = 32
+    if args.perm > 1:
+        over["n_perm"] = args.perm
     it = mem.Integrator(proc, **over)
     it.set_event_offset(lo)
     out_p = torch.empty(ne, dtype=torch.float64, device="cuda")

@@ -66,7 +66,10 @@ typedef struct mem_params {
   int32_t vegas_iters;       /* adaptation passes; 0 = plain Monte Carlo */
   int32_t vegas_bins;        /* bins per dimension, 1..64 */
   int32_t n_flav;            /* light flavours summed in the initial state */
-  int32_t reserved;
+  int32_t n_perm;            /* jet-parton assignments summed per point (Eq. 7 "sum over all
+                              * permutations of assigning measured jets to partons"): 0 or 1 = record order only;
+                              * MEM_PROC_TT_LJETS: 4 = b-tags known (b jets swapped x light jets swapped), 24 = all;
+                              * MEM_PROC_TT_DILEP: 2 = both b assignments.  Anything else: MEM_ERR_INVALID_ARG. */
 } mem_params;
 
 /* Fill *params with the defaults of `process` (precision 64, plain MC). */

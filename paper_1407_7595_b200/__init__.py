@@ -31,7 +31,7 @@ class mem_params(C.Structure):
                     "tf_w_tail", "tf_mu1", "tf_sig1", "tf_mu2", "tf_sig2", "jetE_rlo", "jetE_rhi",
                     "bw_nwidths", "nu_pz_max", "nu_eta_max", "met_sigma", "met_nsigma", "vegas_alpha")] +
                 [("vegas_points", C.c_int64), ("vegas_iters", C.c_int32), ("vegas_bins", C.c_int32),
-                 ("n_flav", C.c_int32), ("reserved", C.c_int32)])
+                 ("n_flav", C.c_int32), ("n_perm", C.c_int32)])
 
 
 class MemError(RuntimeError):

@@ -152,6 +152,7 @@ DevConst make_dev_const(const mem_params& p) {
   c.nu_pz_max = p.nu_pz_max; c.nu_eta_max = p.nu_eta_max;
   c.met_sigma = p.met_sigma; c.met_nsigma = p.met_nsigma;
   c.vegas_bins = p.vegas_bins; c.vegas_alpha = p.vegas_alpha;
+  c.n_perm = p.n_perm > 1 ? p.n_perm : 1;
   return c;
 }
 
@@ -164,7 +165,7 @@ DevConstF to_float(const DevConst& d) {
   CP(gs4); CP(V_ud2); CP(V_tb2); CP(z_cu); CP(z_ct); CP(nu_pz_max); CP(nu_eta_max); CP(met_sigma); CP(met_nsigma);
   CP(vegas_alpha);
 #undef CP
-  f.pdf_fast = d.pdf_fast; f.n_flav = d.n_flav; f.vegas_bins = d.vegas_bins;
+  f.pdf_fast = d.pdf_fast; f.n_flav = d.n_flav; f.vegas_bins = d.vegas_bins; f.n_perm = d.n_perm;
   return f;
 }
 
@@ -194,13 +195,16 @@ mem_status check_params(int process, const mem_params& p) {
     if (p.vegas_points < 2) return fail(MEM_ERR_INVALID_ARG, "vegas_points < 2");
     if (!(p.vegas_alpha >= 0.0)) return fail(MEM_ERR_INVALID_ARG, "vegas_alpha < 0");
   }
-  (void)process;
+  const bool perm_ok = p.n_perm == 0 || p.n_perm == 1 ||
+                       (process == MEM_PROC_TT_LJETS && (p.n_perm == 4 || p.n_perm == 24)) ||
+                       (process == MEM_PROC_TT_DILEP && p.n_perm == 2);
+  if (!perm_ok) return fail(MEM_ERR_INVALID_ARG, "n_perm = %d is not defined for process %d", p.n_perm, process);
   return MEM_OK;
 }
 
 bool aligned8(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 7u) == 0; }
 
-size_t integrate_smem(int NC, int D, int B, int mode) {
+size_t integrate_smem(int NC, int D, int B, int mode) {   // NC = constants per event (all assignments)
   size_t n = (size_t)NC + 2 * kWarps;
   if (mode != MODE_PLAIN) n += (size_t)D * (B + 1);
   if (mode == MODE_ADAPT) n += (size_t)kWarps * D * B;
@@ -209,10 +213,11 @@ size_t integrate_smem(int NC, int D, int B, int mode) {
 
 template <class P>
 mem_status launch_prepare(mem_handle* h, const double* events, int64_t n_events, cudaStream_t st) {
-  mem_status s = ensure(h->ecs, (size_t)n_events * P::NC * sizeof(double), st);
+  const int64_t n_rec = n_events * h->dc.n_perm;            // one block of NC constants per (event, assignment)
+  mem_status s = ensure(h->ecs, (size_t)n_rec * P::NC * sizeof(double), st);
   if (s != MEM_OK) return s;
   const int threads = 128;
-  prepare_kernel<P><<<(unsigned)((n_events + threads - 1) / threads), threads, 0, st>>>(
+  prepare_kernel<P><<<(unsigned)((n_rec + threads - 1) / threads), threads, 0, st>>>(
       h->dc, events, n_events, (double*)h->ecs.p);
   ++h->launches;
   CUDA_TRY(cudaGetLastError());
@@ -224,10 +229,15 @@ mem_status launch_pass(mem_handle* h, int64_t n_events, int64_t n_points, int64_
                        uint64_t seed, uint32_t pass, cudaStream_t st) {
   const int64_t blocks = n_events * n_chunks;
   if (blocks > 0x7fffffffLL) return fail(MEM_ERR_INVALID_ARG, "n_events * chunks = %lld exceeds the grid limit", (long long)blocks);
-  const size_t smem = integrate_smem(P::NC, P::D, h->dc.vegas_bins, MODE);
-  integrate_kernel<P, MODE><<<(unsigned)blocks, kThreads, smem, st>>>(
-      dc_of<typename P::real>(h), (const double*)h->ecs.p, (const double*)h->grids.p, (double*)h->partials.p, (double*)h->hist.p,
-      n_points, chunk, n_chunks, seed, h->event_offset, pass);
+  const size_t smem = integrate_smem(P::NC * h->dc.n_perm, P::D, h->dc.vegas_bins, MODE);
+  if (h->dc.n_perm > 1)
+    integrate_kernel<P, MODE, true><<<(unsigned)blocks, kThreads, smem, st>>>(
+        dc_of<typename P::real>(h), (const double*)h->ecs.p, (const double*)h->grids.p, (double*)h->partials.p,
+        (double*)h->hist.p, n_points, chunk, n_chunks, seed, h->event_offset, pass);
+  else
+    integrate_kernel<P, MODE, false><<<(unsigned)blocks, kThreads, smem, st>>>(
+        dc_of<typename P::real>(h), (const double*)h->ecs.p, (const double*)h->grids.p, (double*)h->partials.p,
+        (double*)h->hist.p, n_points, chunk, n_chunks, seed, h->event_offset, pass);
   ++h->launches;
   CUDA_TRY(cudaGetLastError());
   return MEM_OK;
@@ -301,7 +311,7 @@ mem_status eval_impl(mem_handle* h, const double* events, int64_t n_events, int6
   mem_status s = launch_prepare<P>(h, events, n_events, st);
   if (s != MEM_OK) return s;
   const int threads = 128;
-  const size_t smem = ((size_t)P::NC + (size_t)P::D * (kMaxBins + 1)) * sizeof(double);
+  const size_t smem = ((size_t)P::NC * h->dc.n_perm + (size_t)P::D * (kMaxBins + 1)) * sizeof(double);
   eval_points_kernel<P><<<(unsigned)((n + threads - 1) / threads), threads, smem, st>>>(
       dc_of<typename P::real>(h), (const double*)h->ecs.p, event, grid, first, n, seed, h->event_offset, (uint32_t)iteration, out_w);
   ++h->launches;

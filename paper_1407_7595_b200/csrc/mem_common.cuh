@@ -49,6 +49,7 @@ struct DevConstR {
   // VEGAS
   int vegas_bins;
   T vegas_alpha;
+  int n_perm;                      // jet-parton assignments summed per point (>= 1)
 };
 using DevConst = DevConstR<double>;   // the fp64 path
 using DevConstF = DevConstR<float>;   // fp32 integrand core of config 3 (reading A15)

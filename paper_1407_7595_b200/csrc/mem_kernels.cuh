@@ -15,27 +15,30 @@ enum { MODE_PLAIN = 0, MODE_GRID = 1, MODE_ADAPT = 2 };
 template <class P>
 __global__ void prepare_kernel(const DevConst c, const double* __restrict__ ev, int64_t n_events,
                                double* __restrict__ ecs) {
-  const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (e >= n_events) return;
+  // one thread per (event, jet-parton assignment): ecs = [n_events][n_perm][NC]
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_events * c.n_perm) return;
+  const int64_t e = i / c.n_perm;
+  const int k = (int)(i - e * c.n_perm);
   double ec[P::NC];
-  P::prepare(c, ev, n_events, e, ec);
-  for (int k = 0; k < P::NC; ++k) ecs[e * P::NC + k] = ec[k];
+  P::prepare(c, ev, n_events, e, k, ec);
+  for (int j = 0; j < P::NC; ++j) ecs[i * P::NC + j] = ec[j];
 }
 
 // the integrand at the unit-cube point u.  fp64 processes take u as it is; the fp32 variant
 // (reading A15) rounds u to fp32, clamps it below 1, evaluates the core in fp32 and applies the
 // per-event constant c0 in fp64.
-template <class P, int D>
+template <class P, bool PERM, int D>
 __device__ __forceinline__ double eval_weight(const DevConstR<typename P::real>& c, const typename P::real* ec,
                                               double c0, const double (&u)[D]) {
   using T = typename P::real;
   if constexpr (std::is_same<T, double>::value) {
-    return P::weight(c, ec, u);
+    return P::template weight_t<PERM>(c, ec, u);
   } else {
     T uf[D];
 #pragma unroll
     for (int d = 0; d < D; ++d) uf[d] = fminf((T)u[d], 0x1.fffffep-1f);
-    const double w = (double)P::weight(c, ec, uf) * c0;
+    const double w = (double)P::template weight_t<PERM>(c, ec, uf) * c0;
     return isfinite(w) ? w : 0.0;
   }
 }
@@ -88,7 +91,9 @@ __device__ __forceinline__ void warp_hist_add(double* wh, int k, double v) {
 template <class P, int MODE>
 constexpr int min_blocks() { return (P::kHeavy || MODE != MODE_PLAIN) ? 3 : 0; }   // 0 = no cap
 
-template <class P, int MODE>
+// PERM: sum over c.n_perm jet-parton assignments per point (NEXT-1); the per-event constants are
+// then n_perm blocks of NC.
+template <class P, int MODE, bool PERM>
 __global__ void __launch_bounds__(kThreads, min_blocks<P, MODE>())
 integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__ ecs, const double* __restrict__ grids,
                  double* __restrict__ partials, double* __restrict__ hist, int64_t n_points,
@@ -96,16 +101,17 @@ integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__
   constexpr int D = P::D;
   using T = typename P::real;                         // fp64, or fp32 for the A15 variant
   extern __shared__ double smem[];
-  T* ec = reinterpret_cast<T*>(smem);                 // [NC] (NC doubles are reserved either way)
-  double* red = smem + P::NC;                         // [2 kWarps]
+  const int NCP = PERM ? P::NC * c.n_perm : P::NC;    // constants per event
+  T* ec = reinterpret_cast<T*>(smem);                 // [NCP] (NCP doubles are reserved either way)
+  double* red = smem + NCP;                           // [2 kWarps]
   double* edges = red + 2 * kWarps;                   // [D][B+1]          (GRID, ADAPT)
   const int B = c.vegas_bins;
   double* whist = edges + D * (B + 1);                // [kWarps][D][B]    (ADAPT)
 
   const int64_t e = blockIdx.x / n_chunks;
   const int ch = (int)(blockIdx.x - e * n_chunks);
-  for (int k = threadIdx.x; k < P::NC; k += kThreads) ec[k] = (T)ecs[e * P::NC + k];
-  const double c0 = P::kSplitC0 ? ecs[e * P::NC + P::C0] : 1.0;   // fp32 core x fp64 per-event constant
+  for (int k = threadIdx.x; k < NCP; k += kThreads) ec[k] = (T)ecs[e * NCP + k];
+  const double c0 = P::kSplitC0 ? ecs[e * NCP + P::C0] : 1.0;     // fp32 core x fp64 per-event constant
   if (MODE != MODE_PLAIN)
     for (int k = threadIdx.x; k < D * (B + 1); k += kThreads) edges[k] = grids[e * D * (B + 1) + k];
   if (MODE == MODE_ADAPT)
@@ -126,11 +132,11 @@ integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__
     draw_uniforms<D>(rng, (uint64_t)i, ev_ctr, pass, u);
     double w;
     if (MODE == MODE_PLAIN) {
-      w = eval_weight<P>(c, ec, c0, u);
+      w = eval_weight<P, PERM>(c, ec, c0, u);
     } else {
       int k[D];
       const double jac = vegas_map<D>(edges, B, u, k);
-      w = jac * eval_weight<P>(c, ec, c0, u);
+      w = jac * eval_weight<P, PERM>(c, ec, c0, u);
       if (!isfinite(w)) w = 0.0;
       if (MODE == MODE_ADAPT) {
         const double w2 = live ? w * w : 0.0;
@@ -252,11 +258,12 @@ __global__ void eval_points_kernel(const DevConstR<typename P::real> c, const do
   constexpr int D = P::D;
   using T = typename P::real;
   extern __shared__ double smem[];
+  const int NCP = P::NC * c.n_perm;
   T* ec = reinterpret_cast<T*>(smem);
-  double* edges = smem + P::NC;
+  double* edges = smem + NCP;
   const int B = c.vegas_bins;
-  for (int k = threadIdx.x; k < P::NC; k += blockDim.x) ec[k] = (T)ecs[event * P::NC + k];
-  const double c0 = P::kSplitC0 ? ecs[event * P::NC + P::C0] : 1.0;
+  for (int k = threadIdx.x; k < NCP; k += blockDim.x) ec[k] = (T)ecs[event * NCP + k];
+  const double c0 = P::kSplitC0 ? ecs[event * NCP + P::C0] : 1.0;
   if (grid)
     for (int k = threadIdx.x; k < D * (B + 1); k += blockDim.x) edges[k] = grid[k];
   __syncthreads();
@@ -269,10 +276,10 @@ __global__ void eval_points_kernel(const DevConstR<typename P::real> c, const do
   if (grid) {
     int k[D];
     const double jac = vegas_map<D>(edges, B, u, k);
-    w = jac * eval_weight<P>(c, ec, c0, u);
+    w = jac * eval_weight<P, true>(c, ec, c0, u);
     if (!isfinite(w)) w = 0.0;
   } else {
-    w = eval_weight<P>(c, ec, c0, u);
+    w = eval_weight<P, true>(c, ec, c0, u);
   }
   out_w[i] = w;
 }

@@ -28,6 +28,29 @@ __device__ inline double one_minus_cos(double eta_a, double phi_a, double eta_b,
   return 2.0 * (sh * sh + sn * sn) / (cosh(eta_a) * cosh(eta_b));
 }
 
+// NEXT-1 (Eq. 7): the k-th jet-parton assignment, role r takes measured jet sig[r].
+// n_perm = 24: all permutations of four jets in lexicographic order; 4: b-tags known, order
+// (0123), (0132), (1023), (1032); 2: the two b jets swapped; otherwise the record order.
+__device__ inline void jet_assignment(int n_perm, int k, int (&sig)[4]) {
+  sig[0] = 0; sig[1] = 1; sig[2] = 2; sig[3] = 3;
+  if (n_perm == 24) {
+    int pool[4] = {0, 1, 2, 3};
+    int div = 6, rem = k;
+    for (int r = 0; r < 4; ++r) {
+      const int idx = rem / div;
+      rem -= idx * div;
+      sig[r] = pool[idx];
+      for (int j = idx; j < 3 - r; ++j) pool[j] = pool[j + 1];
+      if (r < 2) div /= (3 - r);
+    }
+  } else if (n_perm == 4) {
+    if (k & 2) { sig[0] = 1; sig[1] = 0; }
+    if (k & 1) { sig[2] = 3; sig[3] = 2; }
+  } else if (n_perm == 2) {
+    if (k & 1) { sig[0] = 1; sig[1] = 0; }
+  }
+}
+
 // =========================================================================================
 // config 1: u dbar -> W+ -> e+ nu, D = 1.  rec = [lep_pT, lep_eta, lep_phi, met_x, met_y]
 // DESIGN.md "Config 1" (reading A5): nu_z in [-P, P] charted by s_W with a Breit-Wigner map,
@@ -40,7 +63,7 @@ struct ProcWenu {
   static constexpr int D = 1, NF = 5, NC = 16;
   enum { LM, LP, LE, LZ, PT, NT2, A, CLO, CHI, DT, SCLO, DSM, PTNT, IPT2, C0, _N };
 
-  __device__ static void prepare(const DevConst& c, const double* ev, int64_t n, int64_t e, double* ec) {
+  __device__ static void prepare(const DevConst& c, const double* ev, int64_t n, int64_t e, int k, double* ec) {
     const double pT = ev[0 * n + e], eta = ev[1 * n + e], phi = ev[2 * n + e];
     const double mx = ev[3 * n + e], my = ev[4 * n + e];
     const double Pz = c.nu_pz_max;
@@ -75,6 +98,9 @@ struct ProcWenu {
     //    * 1 / (8 pi^2 S E_l E_nu) * (jac = E_nu / (2 rt))
     ec[C0] = dt / c.mWGW * c.g4w * c.V_ud2 / 12.0 * c.A_q2 * 4.0 / (8.0 * kPi * kPi * c.S * lE) * 0.5;
   }
+
+  template <bool PERM>
+  __device__ static double weight_t(const DevConst& c, const double* ec, const double (&u)[D]) { return weight(c, ec, u); }
 
   __device__ static double weight(const DevConst& c, const double* ec, const double (&u)[D]) {
     // pi/2 - t = c_lo (1 - u) + c_hi u: positive terms only (1 - u is exact)
@@ -153,7 +179,7 @@ struct ProcZbb {
   static constexpr int D = 2, NF = 6, NC = 12;
   enum { J0 = 0, J1 = 5, C0 = 10, KT = 11 };
 
-  __device__ static void prepare(const DevConst& c, const double* ev, int64_t n, int64_t e, double* ec) {
+  __device__ static void prepare(const DevConst& c, const double* ev, int64_t n, int64_t e, int k, double* ec) {
     double vol = 1.0, sth = 1.0, eta[2], phi[2];
     for (int j = 0; j < 2; ++j) {
       const double Ej = ev[(3 * j) * n + e];
@@ -170,6 +196,9 @@ struct ProcZbb {
     // vol * prod sin(theta)/(2 (2pi)^3) * (2pi)^4 * (2/S) * g_Z^4 * A_q^2 * 4 (flux) * S (u^2, t^2 carry 4 h^2)
     ec[C0] = vol * sth * kTwoPi4 * (2.0 * c.inv_S) * c.gz4 * c.A_q2 * 4.0 * c.S;
   }
+
+  template <bool PERM>
+  __device__ static double weight_t(const DevConst& c, const double* ec, const double (&u)[D]) { return weight(c, ec, u); }
 
   __device__ static double weight(const DevConst& c, const double* ec, const double (&u)[D]) {
     TfAcc<double> tfa{0.0, 1.0};
@@ -217,7 +246,7 @@ struct ProcTTljetsR {
          NA, NB, NC_,                                   // b_lep . nu = E_b nuT (NA e^eta + NB e^-eta - NC_)
          C0, SW0, _N };
 
-  __device__ static void prepare(const DevConst& c, const double* ev, int64_t n, int64_t e, double* ec) {
+  __device__ static void prepare(const DevConst& c, const double* ev, int64_t n, int64_t e, int k, double* ec) {
     const double lpT = ev[0 * n + e], leta = ev[1 * n + e], lphi = ev[2 * n + e];
     const double mphi = ev[16 * n + e];
     const double lE = lpT * cosh(leta);
@@ -227,10 +256,12 @@ struct ProcTTljetsR {
     const double sd = sin(0.5 * (lphi - mphi));
     ec[OMC] = 2.0 * sd * sd;            // 1 - cos(phi_l - phi_nu)
     ec[CPN] = cos(mphi); ec[SPN] = sin(mphi);
+    int sig[4];
+    jet_assignment(c.n_perm, k, sig);                  // role j takes measured jet sig[j]
     double vol = 1.0, sth = 1.0, eta_j[4], phi_j[4];
     for (int j = 0; j < 4; ++j) {
-      const double Ej = ev[(3 + 3 * j) * n + e];
-      eta_j[j] = ev[(4 + 3 * j) * n + e]; phi_j[j] = ev[(5 + 3 * j) * n + e];
+      const double Ej = ev[(3 + 3 * sig[j]) * n + e];
+      eta_j[j] = ev[(4 + 3 * sig[j]) * n + e]; phi_j[j] = ev[(5 + 3 * sig[j]) * n + e];
       jet_prepare(c, Ej, eta_j[j], phi_j[j], ec + J0 + 5 * j);
       vol *= Ej * c.dr;
       sth *= (1.0 / cosh(eta_j[j])) / (2.0 * kTwoPi3);
@@ -258,6 +289,17 @@ struct ProcTTljetsR {
   }
 
   __device__ static T weight(const DevConstR<T>& c, const T* ec, const T (&u)[D]) {
+    return weight_t<false>(c, ec, u);
+  }
+
+  // PERM = false: the record's own jet-parton assignment (ec = one block of NC constants).
+  // PERM = true: NEXT-1, the sum over c.n_perm assignments (Eq. 7), ec = n_perm
+  // blocks.  Everything that depends only on the point -- energy fractions, transfer functions
+  // (functions of E / E_jet alone), the neutrino -- is computed once; only the jet momenta, the
+  // invariants, the boost and the matrix element are repeated per assignment.
+  template <bool PERM>
+  __device__ static T weight_t(const DevConstR<T>& c, const T* ec0, const T (&u)[D]) {
+    const T* ec = ec0;
     // ---- S2: jet energy fractions x_j = E_j / E_jet, neutrino rapidity.
     // g = e^(eta_nu - eta_l); cosh(d eta) - cos(d phi) = ((g-1)^2/2 + (1 - cos d phi) g) / g =: denp / (LPT2 g)
     const T x0 = fma(c.dr, u[0], c.rlo), x1j = fma(c.dr, u[1], c.rlo), x2j = fma(c.dr, u[2], c.rlo), x3 = fma(c.dr, u[3], c.rlo);
@@ -279,8 +321,6 @@ struct ProcTTljetsR {
     TfAcc<T> tfa{T(0), T(1)};
     tf_accum(c, ix0, tfa); tf_accum(c, ix1, tfa); tf_accum(c, ix2, tfa); tf_accum(c, ix3, tfa);
     const T tf = tfa.fac * m_exp(-tfa.esum);
-    const JetR<T> bh = jet_mom(ec + J0, u[0]), bl = jet_mom(ec + J1, u[1]);
-    const JetR<T> q = jet_mom(ec + J2, u[2]), qb = jet_mom(ec + J3, u[3]);
     // ---- S2: neutrino from the mapped leptonic W mass
     const T t = fma(c.tW_dt, u[5], c.tW_lo);
     const T smm = c.mWGW * m_tan(t);
@@ -289,6 +329,11 @@ struct ProcTTljetsR {
     const T nuT = sW * iden;
     const T chn = T(0.5) * (en + eni), shn = T(0.5) * (en - eni);
     const T nE = nuT * chn, nx = nuT * ec[CPN], ny = nuT * ec[SPN], nz = nuT * shn;
+    T sum = T(0);
+    const int n_perm = PERM ? c.n_perm : 1;
+    for (int k = 0; k < n_perm; ++k, ec += NC) {
+    const JetR<T> bh = jet_mom(ec + J0, u[0]), bl = jet_mom(ec + J1, u[1]);
+    const JetR<T> q = jet_mom(ec + J2, u[2]), qb = jet_mom(ec + J3, u[3]);
     // ---- S3: invariants through per-event angular constants
     const T bl_nu = bl.E * nuT * (fma(ec[NA], en, ec[NB] * eni) - ec[NC_]);
     const T bl_l = bl.E * ec[KBL];
@@ -302,14 +347,14 @@ struct ProcTTljetsR {
     const T PE = tE + aE, Px = tx + ax, Py = ty + ay, Pz = tz + az;
     // gamma (E - beta.p) = (E P_E - p_T.P_T) / sqrt(P_E^2 - P_T^2): no division by P_E
     const T M2 = fma(PE, PE, -fma(Px, Px, Py * Py));
-    if (!(M2 > T(0))) return T(0);
+    if (!(M2 > T(0))) continue;
     const T rM = m_rsqrt(M2);
     const T tEb = rM * fma(tE, PE, -fma(Px, tx, Py * ty)), aEb = rM * fma(aE, PE, -fma(Px, ax, Py * ay));
     const T PEb = tEb + aEb;
     const T x1 = (PEb + Pz) * c.inv_sqrt_s, x2 = (PEb - Pz) * c.inv_sqrt_s;
-    if (!(x1 > T(0) && x1 < T(1.0) && x2 > T(0) && x2 < T(1.0))) return T(0);
+    if (!(x1 > T(0) && x1 < T(1.0) && x2 > T(0) && x2 < T(1.0))) continue;
     const T xx = x1 * x2, shat = xx * c.S;
-    if (!(T(4.0) * c.mt2 < shat)) return T(0);                                       // reading A9
+    if (!(T(4.0) * c.mt2 < shat)) continue;                                       // reading A9
     // ---- S5: production.  tau1 = (q1.pt + q2.ptb)/s-hat, tau2 = (q2.pt + q1.ptb)/s-hat
     const T ish = rcp_fast(shat);
     const T hs = T(0.5) * c.sqrt_s * ish;
@@ -334,9 +379,13 @@ struct ProcTTljetsR {
       decprop = t_l * bl_nu * a_q * bh_qb * rcp_fast(dens);
     }
     // ---- S4, S7
-    const T core = tf * (nuT * iden) * (pdf_pair(c, x1, x2) * ish) * prod * decprop;
-    // fp64: the per-event constant is applied here; fp32: by the caller in fp64 (it would underflow)
-    const T w = kSplitC0 ? core : ec[C0] * core;
+    const T core = (pdf_pair(c, x1, x2) * ish) * prod * decprop;
+    if (isfinite(core)) sum += core;
+    }
+    const T pt = tf * (nuT * iden) * sum;
+    // fp64: the per-event constant (identical for every assignment) is applied here; fp32: by the
+    // caller in fp64 (it would underflow)
+    const T w = kSplitC0 ? pt : ec0[C0] * pt;
     return isfinite(w) ? w : T(0);
   }
 };
@@ -445,12 +494,14 @@ struct ProcTTdilep {
          IEJ0 = 54, IEJ1,                                   // 1 / E_jet
          METX = 56, METY, MSPAN, MEXP, C0, PTX, PTY, _N };  // 56..62
 
-  __device__ static void prepare(const DevConst& c, const double* ev, int64_t n, int64_t e, double* ec) {
+  __device__ static void prepare(const DevConst& c, const double* ev, int64_t n, int64_t e, int k, double* ec) {
     for (int k = 0; k < NC; ++k) ec[k] = 0.0;
+    int sig[4];
+    jet_assignment(c.n_perm, k, sig);                  // top side s pairs its lepton with measured jet sig[s]
     double vol = 1.0, sth = 1.0, ptx = 0.0, pty = 0.0, lE[2];
     for (int s = 0; s < 2; ++s) {
       const double pT = ev[(3 * s) * n + e], eta = ev[(3 * s + 1) * n + e], phi = ev[(3 * s + 2) * n + e];
-      const double Ej = ev[(6 + 3 * s) * n + e], jeta = ev[(7 + 3 * s) * n + e], jphi = ev[(8 + 3 * s) * n + e];
+      const double Ej = ev[(6 + 3 * sig[s]) * n + e], jeta = ev[(7 + 3 * sig[s]) * n + e], jphi = ev[(8 + 3 * sig[s]) * n + e];
       double* o = ec + S0 + SIDE * s;
       const double E = pT * cosh(eta);
       lE[s] = E;
@@ -495,6 +546,16 @@ struct ProcTTdilep {
              (2.0 * lE[0] * kTwoPi3) / (2.0 * lE[1] * kTwoPi3) * kTwoPi4 * (2.0 * c.inv_S) /
              (c.mWGW * c.mWGW * c.mtGt * c.mtGt) / (kTwoPi3 * kTwoPi3 * 4.0) / (16.0 * lE[0] * lE[1]) * 4.0 /
              (2.0 * kPi * c.met_sigma * c.met_sigma) * c.gs4 * (2.0 * c.g4w * c.V_tb2) * (2.0 * c.g4w * c.V_tb2);
+  }
+
+  // PERM = true: NEXT-1, both assignments of the two b jets (ec = 2 blocks of NC constants)
+  template <bool PERM>
+  __device__ static double weight_t(const DevConst& c, const double* ec, const double (&u)[D]) {
+    if (!PERM) return weight(c, ec, u);
+    double w = 0.0;
+#pragma unroll 1
+    for (int k = 0; k < c.n_perm; ++k) w += weight(c, ec + k * NC, u);
+    return w;
   }
 
   __device__ static double weight(const DevConst& c, const double* ec, const double (&u)[D]) {
