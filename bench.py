@@ -32,22 +32,24 @@ SEED = 20140729
 # thread-level DFMA / DMUL / DADD per point from the ncu captures in profiles/ (r01_ncu_config3.md,
 # r01_fp64_counts.md): smsp__sass_thread_inst_executed_op_{dfma,dmul,dadd}_pred_on.sum / points.
 # flop = 2 DFMA + DMUL + DADD.  Key = config; config 5's dominant kernel is the grid-mapped final pass.
-FP64_PER_CALL = {
-    1: {"dfma": 87.3, "dmul": 47.0, "dadd": 17.9},
-    2: {"dfma": 116.0, "dmul": 37.0, "dadd": 14.2},
-    3: {"dfma": 261.2, "dmul": 77.7, "dadd": 40.8},
-    4: {"dfma": 300.0, "dmul": 100.0, "dadd": 50.0},
-    5: {"dfma": 268.4, "dmul": 96.7, "dadd": 53.1},
+FP64_PER_CALL = {           # key = (config, jet-parton assignments per point)
+    (1, 1): {"dfma": 87.3, "dmul": 47.0, "dadd": 17.9},
+    (2, 1): {"dfma": 104.0, "dmul": 34.0, "dadd": 15.2},
+    (3, 1): {"dfma": 193.4, "dmul": 86.3, "dadd": 42.8},
+    (3, 24): {"dfma": 1442.3, "dmul": 1258.6, "dadd": 593.8},
+    (4, 1): {"dfma": 248.3, "dmul": 67.7, "dadd": 44.2},
+    (4, 2): {"dfma": 426.7, "dmul": 136.2, "dadd": 80.0},
+    (5, 1): {"dfma": 200.6, "dmul": 106.2, "dadd": 58.1},
 }
-# fp32 variant of config 3 (reading A15): executed FFMA / FMUL / FADD per call (ncu, r01_fp64_counts.md)
-FP32_PER_CALL = {3: {"ffma": 150.0, "fmul": 60.0, "fadd": 30.0}, 5: {"ffma": 150.0, "fmul": 60.0, "fadd": 30.0}}
+# fp32 variant of config 3 (reading A15): executed FFMA / FMUL / FADD per call (same ncu pass)
+FP32_PER_CALL = {3: {"ffma": 82.7, "fmul": 90.3, "fadd": 32.7}, 5: {"ffma": 82.7, "fmul": 90.3, "fadd": 32.7}}
 NOMINAL_FP64_FMA_PER_CLK_PER_SM = 64      # 4 SMSPs x 16 lanes; confirmed by the microbenchmark
 VEGAS_ITERS, VEGAS_POINTS = 5, 1 << 17    # BASELINE.json:configs[4]
 
 
-def flops_per_call(cfg):
-    c = FP64_PER_CALL[cfg]
-    return 2.0 * c["dfma"] + c["dmul"] + c["dadd"]
+def flops_per_call(cfg, perm=1):
+    c = FP64_PER_CALL.get((cfg, max(perm, 1)))
+    return None if c is None else 2.0 * c["dfma"] + c["dmul"] + c["dadd"]
 
 
 def parse_args():
@@ -285,9 +287,11 @@ def run_b200(args):
     k_ms = sum(kms) / len(kms)
     k_evals = ne * n_points
     peak_meas = mem.mem_measure_fp64_peak(5)
-    fl = flops_per_call(cfg)
+    fl = flops_per_call(cfg, args.perm)
+    c = FP64_PER_CALL.get((cfg, max(args.perm, 1)))
+    if fl is None:          # no ncu count for this combination yet: report the single-assignment floor
+        fl, c = flops_per_call(cfg), FP64_PER_CALL[(cfg, 1)]
     achieved = k_evals * fl / (k_ms * 1e-3) / 1e12
-    c = FP64_PER_CALL[cfg]
     pipe_inst = c["dfma"] + c["dmul"] + c["dadd"]
     sms = torch.cuda.get_device_properties(0).multi_processor_count
     sm_mhz = (clocks or {}).get("sm_mhz") or 0.0
