@@ -95,12 +95,20 @@ class ClockSampler:
 
     def __init__(self, index):
         self.proc = None
+        self.index = index
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
                                           "--format=csv,noheader,nounits", "-lms", "100"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
         except OSError:
             self.proc = None
+
+    def _one_shot(self):
+        try:
+            return subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                   "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=10).stdout
+        except (OSError, subprocess.SubprocessError):
+            return ""
 
     def stop(self):
         if self.proc is None:
@@ -111,6 +119,8 @@ class ClockSampler:
         except subprocess.TimeoutExpired:
             self.proc.kill()
             out, _ = self.proc.communicate()
+        if not out.strip():          # timed region shorter than one sampling period: query once, right after it
+            out = self._one_shot()
         sm, mx, reasons = [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for line in out.strip().splitlines():
@@ -317,6 +327,8 @@ def run_b200(args):
                          "peak": peak32, "frac": ach32 / peak32, "flop_per_call": fl32,
                          "peak_source": "derived: 128 FP32 FMA/clk/SM x SMs x sampled SM clock (DESIGN.md)",
                          "fp64_flop_per_call_kept": fl})
+        roofline.pop("fp64_pipe_frac", None)
+        roofline.pop("fp64_inst_per_call", None)
     h2d = ne * mem.mem_event_fields(proc) * 8
     d2h = 2 * ne * 8
     line = {
