@@ -619,10 +619,10 @@ struct ProcTTdilep {
     const double tvx = ec[S0 + LX] + Eb0 * ec[J0 + 2], tvy = ec[S0 + LY] + Eb0 * ec[J0 + 3];
     const double avx = ec[S1 + LX] + Eb1 * ec[J1 + 2], avy = ec[S1 + LY] + Eb1 * ec[J1 + 3];
     double sum = 0.0;
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-      if (k >= nr) break;
-      double x = xr[k];
+    // one copy of the per-solution code (the roots stay in registers: selected, not indexed)
+#pragma unroll 1
+    for (int k = 0; k < nr; ++k) {
+      double x = (k == 0) ? xr[0] : (k == 1) ? xr[1] : (k == 2) ? xr[2] : xr[3];
       const double V = fma(vv1, x, V0);
       if (!(V != 0.0)) continue;
       double y = -fma(fma(uu2, x, U1), x, U0) / V;
