@@ -80,6 +80,7 @@ def lib():
         L.orc_boost_transverse.restype = None
         L.orc_quartic_real_roots.argtypes = [_dp, _dp]
         L.orc_dilep_solve.argtypes = [_dp] * 4 + [C.c_double] * 6 + [_dp, _dp]
+        L.orc_parton_weights.argtypes = [C.c_int, C.POINTER(Params), _dp, C.c_int64, C.c_int, _dp]
         L.orc_weight.argtypes = [C.c_int, C.POINTER(Params), _dp, _dp, _dp]
         L.orc_weight.restype = C.c_double
         L.orc_eval_points.argtypes = [C.c_int, C.POINTER(Params), _dp, C.c_int64, C.c_int64, C.c_uint64,
@@ -211,6 +212,15 @@ def dilep_solve(lp, b, lm, bb, sWp, st, sWm, stb, Sx, Sy):
     sol, jac = np.empty(32), np.empty(4)
     n = lib().orc_dilep_solve(_p(a[0]), _p(a[1]), _p(a[2]), _p(a[3]), sWp, st, sWm, stb, Sx, Sy, _p(sol), _p(jac))
     return sol[:8 * n].reshape(n, 2, 4).copy(), jac[:n].copy()
+
+
+def parton_weights(process, p, mom, extended=False):
+    """NEXT-2: parton-level weights; mom = [24, n_events] (l, nu, b_had, b_lep, q, qbar')"""
+    m = _f64(mom)
+    out = np.empty(m.shape[1])
+    if lib().orc_parton_weights(process, C.byref(p), _p(m), m.shape[1], int(extended), _p(out)) != 0:
+        raise ValueError("orc_parton_weights failed")
+    return out
 
 
 def weight(process, p, rec, u, debug=False):

@@ -725,6 +725,54 @@ template <typename R> R weight_permuted(int process, const orc_params* p, const 
   return sum;
 }
 
+// NEXT-2, parton-level mode (Table 2): "the transfer functions are delta
+// functions", no integration -- the integrand of Eq. 1 without dPhi at a fully specified partonic
+// configuration, summed over the jet-parton assignments (n_perm) and the initial-state flavours:
+//   w = sum_sigma  f(x1) f(x2) / (|q1||q2|) * |M|^2(l, nu, b_had, b_lep, q, qbar' [jets reordered by sigma])
+// mom = six four-vectors (E, px, py, pz) in the order l, nu, b_had, b_lep, q, qbar'.  The transverse
+// boost O7 is applied (identity for a balanced event); all four propagators come from the momenta.
+template <typename R> R parton_weight_tt_ljets(const orc_params* p, const double* mom_in) {
+  const R S = R(p->sqrt_s) * R(p->sqrt_s), mt = p->m_t, Gt = p->Gam_t;
+  int perm[24][4];
+  const int n = jet_perms(ORC_TT_LJETS, p->n_perm, perm);
+  R sum = R(0);
+  for (int k = 0; k < n; ++k) {
+    // internal order for the boost: l, nu, b_lep, b_had, q, qbar'
+    R mom[24];
+    const int role_src[4] = {2 + perm[k][0], 2 + perm[k][1], 2 + perm[k][2], 2 + perm[k][3]};   // b_had, b_lep, q, qbar'
+    for (int c = 0; c < 4; ++c) {
+      mom[c] = mom_in[c]; mom[4 + c] = mom_in[4 + c];
+      mom[8 + c] = mom_in[4 * role_src[1] + c];     // b_lep
+      mom[12 + c] = mom_in[4 * role_src[0] + c];    // b_had
+      mom[16 + c] = mom_in[4 * role_src[2] + c];    // q
+      mom[20 + c] = mom_in[4 * role_src[3] + c];    // qbar'
+    }
+    R P[4] = {0, 0, 0, 0};
+    for (int i = 0; i < 6; ++i) for (int c = 0; c < 4; ++c) P[c] += mom[4 * i + c];
+    if (!(P[1] * P[1] + P[2] * P[2] < P[0] * P[0])) continue;
+    boost_transverse<R>(P, 6, mom);
+    R PE = 0, Pz = 0;
+    for (int i = 0; i < 6; ++i) { PE += mom[4 * i]; Pz += mom[4 * i + 3]; }
+    R x1, x2;
+    if (!beam_fractions<R>(p, PE, Pz, &x1, &x2)) continue;
+    const R shat = x1 * x2 * S;
+    if (!(R(4) * mt * mt < shat)) continue;                          // A9
+    R q1[4], q2[4], pt[4], ptb[4];
+    beams<R>(p, x1, x2, q1, q2);
+    for (int c = 0; c < 4; ++c) { pt[c] = mom[c] + mom[4 + c] + mom[8 + c]; ptb[c] = mom[12 + c] + mom[16 + c] + mom[20 + c]; }
+    const R prod = R(p->pdf_A_g) * R(p->pdf_A_g) * me_tt_gg<R>(p, q1, q2, pt, ptb) +
+                   R(2) * R(p->n_flav) * R(p->pdf_A_q) * R(p->pdf_A_q) * me_tt_qq<R>(p, q1, q2, pt, ptb);
+    const R dec_lep = R(0.5) * me_top_decay<R>(p, R(1), pt, mom + 8, mom, mom + 4);
+    const R dec_had = R(0.5) * R(p->V_ud) * R(p->V_ud) * me_top_decay<R>(p, R(3), ptb, mom + 12, mom + 16, mom + 20);
+    V4<R> t4 = from_arr(pt), tb4 = from_arr(ptb);
+    const R Dt = bw_D<R>(dot(t4, t4) - mt * mt, mt, Gt), Dtb = bw_D<R>(dot(tb4, tb4) - mt * mt, mt, Gt);
+    const R ff = pdf_shape<R>(p, x1) * pdf_shape<R>(p, x2);
+    const R w = ff * prod * Dt * Dtb * dec_lep * dec_had / (x1 * x2 * S / R(4));
+    if (std::isfinite((double)w)) sum += w;
+  }
+  return sum;
+}
+
 template <typename R> double weight_any(int process, const orc_params* p, const double* rec, const double* u,
                                         double* dbg) {
   R w = R(0);
@@ -877,6 +925,19 @@ int orc_dilep_solve(const double lp[4], const double b[4], const double lm[4], c
     jac[k] = dilep_jacobian<double>(a, c, d, e, s[k]);
   }
   return n;
+}
+
+// NEXT-2: parton-level weights of n_events configurations, SoA field-major [24][n_events]
+int orc_parton_weights(int process, const orc_params* p, const double* mom, int64_t n_events, int extended,
+                       double* out_w) {
+  if (process != ORC_TT_LJETS || !p || !mom || !out_w) return 1;
+  for (int64_t e = 0; e < n_events; ++e) {
+    double m[24];
+    for (int f = 0; f < 24; ++f) m[f] = mom[(size_t)f * n_events + e];
+    double w = extended ? (double)parton_weight_tt_ljets<long double>(p, m) : (double)parton_weight_tt_ljets<double>(p, m);
+    out_w[e] = std::isfinite(w) ? w : 0.0;
+  }
+  return 0;
 }
 
 double orc_weight(int process, const orc_params* p, const double* rec, const double* u, double* dbg) {

@@ -101,6 +101,13 @@ int orc_integrate(int process, const orc_params* p, const double* events, int64_
                   uint64_t event_offset, int64_t n_points, uint64_t seed,
                   double* out_p, double* out_err);
 
+/* --- NEXT-2, parton-level mode (Table 2): delta transfer functions, no integration.
+ * mom: SoA field-major [24][n_events] = (E,px,py,pz) of l, nu, b_had, b_lep, q, qbar'.
+ * out_w[e] = sum over the n_perm jet assignments of f f / (|q1||q2|) |M|^2.  extended != 0: the
+ * long-double referee. */
+int orc_parton_weights(int process, const orc_params* p, const double* mom, int64_t n_events, int extended,
+                       double* out_w);
+
 /* --- VEGAS (DESIGN.md config 5, reading A14) --- */
 void orc_vegas_map(const double* edges /* [D][bins+1] */, int bins, int n_dims, const double* u,
                    double* z, int* k, double* jac);

@@ -86,3 +86,60 @@ def shard_range(n_events: int, rank: int, world: int):
     base, rem = divmod(int(n_events), int(world))
     lo = rank * base + min(rank, rem)
     return lo, lo + base + (1 if rank < rem else 0)
+
+
+# ------------------------------------------------------------------------------------------
+# NEXT-2, parton-level mode (Table 2): fully specified partonic
+# t tbar -> b l nu bbar q qbar' configurations.  Pure kinematics: Breit-Wigner distributed top and
+# W masses, isotropic two-body decays, a longitudinal boost.  Stands in for the paper's MadGraph
+# parton-level samples.
+# ------------------------------------------------------------------------------------------
+def _boost(p, b):
+    """boost four-vectors p [4, n] by velocities b [3, n]"""
+    b2 = np.sum(b * b, axis=0)
+    g = 1.0 / np.sqrt(1.0 - b2)
+    bp = np.sum(b * p[1:], axis=0)
+    k = np.where(b2 > 0, (g - 1.0) * bp / np.where(b2 > 0, b2, 1.0), 0.0) + g * p[0]
+    return np.concatenate([(g * (p[0] + bp))[None], p[1:] + k * b], axis=0)
+
+
+def _two_body(r, P, m1, m2):
+    """isotropic decay of P [4, n] into masses m1, m2 (arrays or scalars)"""
+    n = P.shape[1]
+    M2 = P[0] ** 2 - P[1] ** 2 - P[2] ** 2 - P[3] ** 2
+    M = np.sqrt(M2)
+    k = np.sqrt(np.maximum(0.0, (M2 - (m1 + m2) ** 2) * (M2 - (m1 - m2) ** 2))) / (2.0 * M)
+    c = 2.0 * r.random(n) - 1.0
+    ph = 2.0 * np.pi * r.random(n)
+    s = np.sqrt(1.0 - c * c)
+    d = np.stack([s * np.cos(ph), s * np.sin(ph), c])
+    p1 = np.concatenate([np.sqrt(k * k + m1 * m1)[None], k * d])
+    p2 = np.concatenate([np.sqrt(k * k + m2 * m2)[None], -k * d])
+    b = P[1:] / P[0]
+    return _boost(p1, b), _boost(p2, b)
+
+
+def _breit_wigner(r, n, m, G, nwidths):
+    lo, hi = np.arctan(((m - nwidths * G) ** 2 - m * m) / (m * G)), np.arctan(((m + nwidths * G) ** 2 - m * m) / (m * G))
+    return np.sqrt(m * m + m * G * np.tan(lo + (hi - lo) * r.random(n)))
+
+
+def make_parton_events(n_events: int, seed: int = DEFAULT_SEED, sqrt_s: float = 14000.0, m_t: float = 173.0,
+                       Gam_t: float = 1.4, m_W: float = 80.4, Gam_W: float = 2.09) -> np.ndarray:
+    """[24, n_events]: (E, px, py, pz) of l, nu, b_had, b_lep, q, qbar' with t = b_lep + l + nu and
+    tbar = b_had + q + qbar'; sqrt(s-hat) = 2 m_t + 30 + Exp(150) GeV, rapidity of the pair U(-1.5, 1.5)."""
+    r = np.random.Generator(np.random.PCG64([int(seed), 1407]))
+    n = int(n_events)
+    mt1, mt2 = _breit_wigner(r, n, m_t, Gam_t, 15.0), _breit_wigner(r, n, m_t, Gam_t, 15.0)
+    mw1, mw2 = _breit_wigner(r, n, m_W, Gam_W, 15.0), _breit_wigner(r, n, m_W, Gam_W, 15.0)
+    rs = 2.0 * m_t + 30.0 + _exp(r.random(n), 150.0)
+    y = -1.5 + 3.0 * r.random(n)
+    rs = np.minimum(rs, 0.9 * sqrt_s * np.exp(-np.abs(y)))          # keep x1, x2 below 1
+    P = np.stack([rs * np.cosh(y), np.zeros(n), np.zeros(n), rs * np.sinh(y)])
+    t, tb = _two_body(r, P, mt1, mt2)
+    W1, b_lep = _two_body(r, t, mw1, np.zeros(n))
+    lep, nu = _two_body(r, W1, np.zeros(n), np.zeros(n))
+    W2, b_had = _two_body(r, tb, mw2, np.zeros(n))
+    q, qb = _two_body(r, W2, np.zeros(n), np.zeros(n))
+    ev = np.concatenate([lep, nu, b_had, b_lep, q, qb], axis=0)
+    return np.ascontiguousarray(ev, dtype=np.float64)
