@@ -66,6 +66,8 @@ def parse_args():
     ap.add_argument("--perm", type=int, default=0,
                     help="jet-parton assignments summed per point (NEXT-1): config 3/5: 4 or 24, config 4: 2")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--parton", action="store_true",
+                    help="NEXT-2 parton-level mode: ME evaluations of --events configurations (default 10^5)")
     ap.add_argument("--sweep", action="store_true",
                     help="config-5 sweep of BASELINE.json:configs[4]: events x final points, one JSON line")
     return ap.parse_args()
@@ -409,9 +411,74 @@ def run_sweep(args):
                       "sweep": cells}), flush=True)
 
 
+def run_parton(args):
+    """NEXT-2 (Table 2): parton-level weights of N fully specified t tbar -> 6 parton
+    configurations, summed over --perm assignments.  One step = one mem_eval_parton call.  The kernel reads
+    192 B and writes 8 B per event: at one assignment it is HBM/latency bound, at 24 FP64 bound."""
+    import torch
+
+    import paper_1407_7595_b200 as mem
+    from paper_1407_7595_b200 import workloads as wl
+
+    torch.cuda.set_device(0)
+    n = args.events or 100000
+    perm = max(args.perm, 1)
+    ev_host = torch.from_numpy(wl.make_parton_events(n)).pin_memory()
+    ev = ev_host.cuda()
+    out = torch.empty(n, dtype=torch.float64, device="cuda")
+    out_host = torch.empty(n, dtype=torch.float64).pin_memory()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    with mem.Integrator(wl.TT_LJETS, **({"n_perm": perm} if perm > 1 else {})) as it:
+        def dev_step():
+            it.eval_parton(ev, out_w=out)
+
+        def host_step():
+            d = ev_host.cuda(non_blocking=True)
+            it.eval_parton(d, out_w=out)
+            out_host.copy_(out, non_blocking=True)
+            torch.cuda.synchronize()
+
+        for _ in range(max(args.warmup, 3)):
+            dev_step()
+        host_step()
+        res = {}
+        for name, fn in (("dev", dev_step), ("host", host_step)):
+            ms = []
+            for _ in range(args.steps):
+                flush.fill_(0)
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record()
+                fn()
+                b.record()
+                b.synchronize()
+                ms.append(a.elapsed_time(b))
+            res[name] = sum(ms) / len(ms)
+    t = res["dev"] * 1e-3
+    traffic = n * (24 + 1) * 8
+    peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(
+        os.path.join(ROOT, "MEASURED_PEAKS.json")) else {}
+    hbm = peaks.get("hbm_gbs", 6650.0)
+    line = {"metric": "parton_level_me_evals_per_s", "value": n * perm / t, "unit": "assignment evaluations/s",
+            "events_per_s": n / t, "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": res["dev"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "parton-level t tbar l+jets (NEXT-2), %d events x %d assignments" % (n, perm),
+                       "l2": "flushed between timed steps (256 MiB fill)"},
+            "e2e": {"value": n * perm / (res["host"] * 1e-3), "unit": "assignment evaluations/s",
+                    "h2d_bytes_per_step": n * 24 * 8, "d2h_bytes_per_step": n * 8, "ms_per_step": res["host"]},
+            "gpu_launches": args.steps,
+            "roofline": {"bound": "hbm", "kernel": "parton_ttljets_kernel", "achieved": traffic / t / 1e9, "peak": hbm,
+                         "unit": "GB/s", "frac": traffic / t / 1e9 / hbm, "traffic": None,
+                         "peak_source": "MEASURED_PEAKS.json hbm_gbs" if peaks else "fallback 6650 GB/s",
+                         "note": "200 B/event algorithmic; with 24 assignments the kernel is FP64 bound instead"}}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     args = parse_args()
-    if args.sweep:
+    if args.parton:
+        run_parton(args)
+    elif args.sweep:
         run_sweep(args)
     elif args.impl == "reference":
         run_reference(args)

@@ -128,6 +128,19 @@ mem_status mem_eval_points(mem_handle* h, const double* events, int64_t n_events
                            int64_t first_point, int64_t n, uint64_t seed, int32_t iteration,
                            const double* grid, double* out_w, void* cuda_stream);
 
+/* Parton-level mode (NEXT-2; Table 2): the transfer functions are delta
+ * functions and nothing is integrated.  For each fully specified partonic configuration
+ *   out_w[e] = sum over the handle's n_perm jet-parton assignments and the initial-state flavours of
+ *              f(x1) f(x2) / (|q1||q2|) * |M|^2(l, nu, b_had, b_lep, q, qbar')
+ * i.e. the integrand of PAPER.md:45 Eq. 1 without dPhi (transverse boost O7 applied, propagators
+ * from the momenta; kinematically forbidden configurations give 0).
+ * momenta : device, float64, SoA field-major [24][n_events] = (E, px, py, pz) of l, nu, b_had, b_lep,
+ *           q, qbar' (t = b_lep + l + nu, tbar = b_had + q + qbar'); read-only
+ * out_w   : device, float64 [n_events]; overwritten.  Asynchronous on cuda_stream.
+ * MEM_PROC_TT_LJETS handles with precision 64 only (MEM_ERR_UNSUPPORTED otherwise). */
+mem_status mem_eval_parton(mem_handle* h, const double* momenta, int64_t n_events, double* out_w,
+                           void* cuda_stream);
+
 /* Diagnostic: copy the VEGAS grids left by the last mem_integrate with
  * vegas_iters > 0 into out_grid (device, float64 [n_events][D][vegas_bins+1]). */
 mem_status mem_get_grid(mem_handle* h, int64_t n_events, double* out_grid, void* cuda_stream);

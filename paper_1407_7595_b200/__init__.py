@@ -19,7 +19,7 @@ MEM_PROC_W_ENU, MEM_PROC_Z_BB, MEM_PROC_TT_LJETS, MEM_PROC_TT_DILEP = 1, 2, 3, 4
 
 EXPORTS = ("mem_params_default", "mem_event_fields", "mem_n_dims", "mem_create", "mem_destroy",
            "mem_set_event_offset", "mem_integrate", "mem_integrate_host", "mem_eval_points",
-           "mem_get_grid", "mem_launch_count", "mem_last_error", "mem_last_pass_ms", "mem_measure_fp64_peak")
+           "mem_eval_parton", "mem_get_grid", "mem_launch_count", "mem_last_error", "mem_last_pass_ms", "mem_measure_fp64_peak")
 
 
 class mem_params(C.Structure):
@@ -64,6 +64,7 @@ def lib():
         L.mem_integrate.argtypes = [vp, dp, i64, i64, u64, dp, dp, vp]
         L.mem_integrate_host.argtypes = [vp, dp, i64, i64, u64, dp, dp]
         L.mem_eval_points.argtypes = [vp, dp, i64, i64, i64, i64, u64, C.c_int32, dp, dp, vp]
+        L.mem_eval_parton.argtypes = [vp, dp, i64, dp, vp]
         L.mem_get_grid.argtypes = [vp, i64, dp, vp]
         L.mem_launch_count.argtypes = [vp]
         L.mem_launch_count.restype = i64
@@ -193,6 +194,17 @@ def mem_eval_points(handle, events, event: int, first_point: int, n: int, seed: 
     return out_w
 
 
+def mem_eval_parton(handle, momenta, out_w=None, stream=None):
+    """Parton-level mode (NEXT-2): momenta = CUDA float64 tensor [24, n_events]; returns out_w [n_events]."""
+    import torch
+    n_events = int(momenta.shape[1])
+    if out_w is None:
+        out_w = torch.empty(n_events, dtype=torch.float64, device=momenta.device)
+    _check(lib().mem_eval_parton(handle, _dev_f64(momenta, "momenta"), n_events,
+                                 _dev_f64(out_w, "out_w", (n_events,)), _stream_ptr(stream)))
+    return out_w
+
+
 def mem_get_grid(handle, n_events: int, n_dims: int, bins: int, device=None, stream=None):
     """Diagnostic: VEGAS grids of the last mem_integrate, CUDA tensor [n_events, D, bins + 1]."""
     import torch
@@ -222,6 +234,9 @@ class Integrator:
 
     def eval_points(self, events, event, first_point, n, seed, **kw):
         return mem_eval_points(self.handle, events, event, first_point, n, seed, **kw)
+
+    def eval_parton(self, momenta, **kw):
+        return mem_eval_parton(self.handle, momenta, **kw)
 
     def grid(self, n_events, **kw):
         return mem_get_grid(self.handle, n_events, mem_n_dims(self.process), self.params.vegas_bins, **kw)

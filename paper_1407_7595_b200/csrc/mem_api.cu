@@ -9,6 +9,7 @@
 #include <new>
 
 #include "mem_kernels.cuh"
+#include "mem_parton.cuh"
 
 using namespace memb200;
 
@@ -515,6 +516,23 @@ mem_status mem_eval_points(mem_handle* h, const double* events, int64_t n_events
     case MEM_PROC_TT_DILEP: return eval_impl<ProcTTdilep>(h, events, n_events, event, first_point, n, seed, iteration, grid, out_w, st);
   }
   return fail(MEM_ERR_UNSUPPORTED, "process %d is not implemented", h->process);
+}
+
+mem_status mem_eval_parton(mem_handle* h, const double* momenta, int64_t n_events, double* out_w, void* cuda_stream) {
+  if (!h) return fail(MEM_ERR_INVALID_ARG, "handle is NULL");
+  if (h->process != MEM_PROC_TT_LJETS || h->params.precision != 64)
+    return fail(MEM_ERR_UNSUPPORTED, "parton-level mode is implemented for MEM_PROC_TT_LJETS in fp64");
+  if (n_events < 0) return fail(MEM_ERR_INVALID_ARG, "n_events < 0");
+  if (n_events == 0) return MEM_OK;
+  if (!momenta || !out_w) return fail(MEM_ERR_INVALID_ARG, "momenta / out_w is NULL");
+  if (!aligned8(momenta) || !aligned8(out_w)) return fail(MEM_ERR_INVALID_ARG, "device pointers must be 8-byte aligned");
+  const int threads = 128;
+  const int64_t blocks = (n_events + threads - 1) / threads;
+  if (blocks > 0x7fffffffLL) return fail(MEM_ERR_INVALID_ARG, "n_events exceeds the grid limit");
+  parton_ttljets_kernel<<<(unsigned)blocks, threads, 0, (cudaStream_t)cuda_stream>>>(h->dc, momenta, n_events, out_w);
+  ++h->launches;
+  CUDA_TRY(cudaGetLastError());
+  return MEM_OK;
 }
 
 mem_status mem_get_grid(mem_handle* h, int64_t n_events, double* out_grid, void* cuda_stream) {
