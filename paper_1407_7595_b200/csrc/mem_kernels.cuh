@@ -123,6 +123,61 @@ integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__
   const int64_t lo = (int64_t)ch * chunk;
   const int64_t hi = (lo + chunk < n_points) ? lo + chunk : n_points;
   double s1 = 0.0, s2 = 0.0;
+  if constexpr (P::kCompact && MODE == MODE_PLAIN && !PERM) {
+    // Lane compaction (config 4).  Most points have no kinematic solution, and the ones that do are
+    // scattered over the warp, so the long per-solution part would run with a few lanes active.
+    // Pass A: every lane takes one point up to the quartic and learns its number of real roots.
+    // Points with roots are queued per warp (two queues: 2 roots, 4 roots, so that a batch has a
+    // uniform trip count) as 32-bit offsets; whenever a queue holds 32 entries the warp runs the
+    // full integrand on them, all lanes active (pass B recomputes the point from its counter:
+    // cheaper than carrying 13 doubles of state per entry through shared memory).  The order in
+    // which a lane meets its points depends only on the data, so the sums stay reproducible.
+    // Measured on config 4: +9.5 % (1.50e10 -> 1.64e10 evaluations/s); with two assignments per point
+    // pass A doubles and the scheme loses 30 %, so the assignment sum keeps the plain loop.
+    uint32_t* q = reinterpret_cast<uint32_t*>(edges) + (threadIdx.x >> 5) * 128;   // [2][64] per warp
+    const int lane = threadIdx.x & 31;
+    const unsigned lt = (1u << lane) - 1u;
+    int cnt2 = 0, cnt4 = 0, head2 = 0, head4 = 0;                                   // warp-uniform
+    int64_t base = lo;
+    bool draining = false;
+    while (true) {
+      if (!draining) {
+        // pass A: one point per lane up to the quartic
+        const int64_t i = base + threadIdx.x;
+        int nr = 0;
+        if (i < hi) {
+          double u[D];
+          draw_uniforms<D>(rng, (uint64_t)i, ev_ctr, pass, u);
+          nr = P::template n_roots<PERM>(c, ec, u);
+        }
+        const unsigned m2 = __ballot_sync(0xffffffffu, nr > 0 && nr <= 2), m4 = __ballot_sync(0xffffffffu, nr > 2);
+        if (nr > 2) q[64 + ((head4 + cnt4 + __popc(m4 & lt)) & 63)] = (uint32_t)(i - lo);
+        else if (nr > 0) q[(head2 + cnt2 + __popc(m2 & lt)) & 63] = (uint32_t)(i - lo);
+        cnt2 += __popc(m2); cnt4 += __popc(m4);
+        base += kThreads;
+        draining = base >= hi;
+        __syncwarp();
+      }
+      // pass B: full batches, and whatever is left once the chunk is exhausted (one call site)
+      while (true) {
+        int which = -1;
+        if (cnt2 >= 32 || (draining && cnt2 > 0)) which = 0;
+        else if (cnt4 >= 32 || (draining && cnt4 > 0)) which = 1;
+        if (which < 0) break;
+        const int n_live = min(32, which ? cnt4 : cnt2), hd = which ? head4 : head2;
+        if (lane < n_live) {
+          const int64_t i = lo + q[which * 64 + ((hd + lane) & 63)];
+          double u[D];
+          draw_uniforms<D>(rng, (uint64_t)i, ev_ctr, pass, u);
+          const double w = eval_weight<P, PERM>(c, ec, c0, u);
+          s1 += w; s2 = fma(w, w, s2);
+        }
+        if (which) { head4 += n_live; cnt4 -= n_live; } else { head2 += n_live; cnt2 -= n_live; }
+        __syncwarp();
+      }
+      if (draining) break;
+    }
+  } else {
   double* wh = whist + (threadIdx.x >> 5) * D * B;
   // uniform trip count across the block so that the warp-wide histogram update is convergent
   for (int64_t base = lo; base < hi; base += kThreads) {
@@ -145,6 +200,7 @@ integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__
       }
     }
     if (live) { s1 += w; s2 = fma(w, w, s2); }
+  }
   }
   block_sum2(s1, s2, red);
   if (threadIdx.x == 0) {

@@ -58,6 +58,7 @@ __device__ inline void jet_assignment(int n_perm, int k, int (&sig)[4]) {
 // =========================================================================================
 struct ProcWenu {
   using real = double;
+  static constexpr bool kCompact = false;   // lane compaction in the plain integrate kernel
   static constexpr bool kHeavy = false;   // see min_blocks() in mem_kernels.cuh
   static constexpr bool kSplitC0 = false;
   static constexpr int D = 1, NF = 5, NC = 16;
@@ -174,6 +175,7 @@ __device__ __forceinline__ JetR<T> jet_mom(const T* o, T u) {
 // =========================================================================================
 struct ProcZbb {
   using real = double;
+  static constexpr bool kCompact = false;   // lane compaction in the plain integrate kernel
   static constexpr bool kHeavy = false;   // see min_blocks() in mem_kernels.cuh
   static constexpr bool kSplitC0 = false;
   static constexpr int D = 2, NF = 6, NC = 12;
@@ -236,6 +238,7 @@ struct ProcZbb {
 template <typename T>
 struct ProcTTljetsR {
   using real = T;
+  static constexpr bool kCompact = false;
   static constexpr bool kHeavy = false;
   static constexpr int D = 6, NF = 17, NC = 44;
   static constexpr bool kSplitC0 = !std::is_same<T, double>::value;
@@ -472,6 +475,7 @@ __device__ __forceinline__ int quartic_real_roots(double a3, double a2, double a
 
 struct ProcTTdilep {
   using real = double;
+  static constexpr bool kCompact = true;   // lane compaction in the plain integrate kernel
   static constexpr bool kHeavy = true;   // see min_blocks() in mem_kernels.cuh
   static constexpr bool kSplitC0 = false;
   static constexpr int D = 8, NF = 14, NC = 64;
@@ -559,6 +563,25 @@ struct ProcTTdilep {
   }
 
   __device__ static double weight(const DevConst& c, const double* ec, const double (&u)[D]) {
+    return weight_impl<false>(c, ec, u);
+  }
+
+  // The number of real roots of the resultant quartic (0, 2, 4) at this point, the largest over the
+  // assignments: what the lane-compacting kernel (mem_kernels.cuh) sorts points by before it runs the
+  // expensive per-solution part on full warps.  Same code as weight(): the prelude is shared.
+  template <bool PERM>
+  __device__ static int n_roots(const DevConst& c, const double* ec, const double (&u)[D]) {
+    int nr = (int)weight_impl<true>(c, ec, u);
+    if (PERM) {
+#pragma unroll 1
+      for (int k = 1; k < c.n_perm; ++k) nr = max(nr, (int)weight_impl<true>(c, ec + k * NC, u));
+    }
+    return nr;
+  }
+
+  // COUNT_ONLY: stop after the quartic and return its number of real roots
+  template <bool COUNT_ONLY>
+  __device__ static double weight_impl(const DevConst& c, const double* ec, const double (&u)[D]) {
     // ---- S2: jets, transfer functions
     TfAcc<double> tfa{0.0, 1.0};
     const double xb0 = fma(c.dr, u[0], c.rlo), xb1 = fma(c.dr, u[1], c.rlo);
@@ -610,6 +633,7 @@ struct ProcTTdilep {
     double xr[4];
     const int nr = quartic_real_roots(R3 * ir4, R2 * ir4, R1 * ir4, R0 * ir4, xr);
     if (nr == 0) return 0.0;
+    if (COUNT_ONLY) return (double)nr;
     // ---- solution-independent pieces
     const double ptx = ec[PTX] + Eb0 * ec[J0 + 2] + Eb1 * ec[J1 + 2] + Sx;     // total transverse momentum
     const double pty = ec[PTY] + Eb0 * ec[J0 + 3] + Eb1 * ec[J1 + 3] + Sy;
