@@ -299,6 +299,7 @@ def run_b200(args):
     k_ms = sum(kms) / len(kms)
     k_evals = ne * n_points
     peak_meas = mem.mem_measure_fp64_peak(5)
+    peak_rrr = mem.mem_measure_fp64_peak_rrr(5)
     fl = flops_per_call(cfg, args.perm)
     c = FP64_PER_CALL.get((cfg, max(args.perm, 1)))
     if fl is None:          # no ncu count for this combination yet: report the single-assignment floor
@@ -311,6 +312,9 @@ def run_b200(args):
         "bound": "alu", "kernel": "integrate_kernel<%s>" % ("ProcTTljets,GRID" if cfg == 5 else "proc%d,PLAIN" % proc),
         "achieved": achieved, "peak": peak_meas, "unit": "TFLOP/s", "frac": achieved / peak_meas,
         "peak_source": "measured in this run: independent DFMA chains on all SMs (mem_measure_fp64_peak)",
+        "peak_three_register_operands": peak_rrr,
+        "peak_three_register_operands_note": "same microbenchmark with x = fma(x, y, z), y and z in registers: the "
+                                             "register file feeds such DFMAs at ~2/3 of the pipe's nominal rate",
         "peak_nominal_at_observed_clock": 2e-6 * NOMINAL_FP64_FMA_PER_CLK_PER_SM * sms * sm_mhz,
         "fp64_pipe_frac": (k_evals * pipe_inst / (k_ms * 1e-3)) / (peak_meas * 1e12 / 2.0),
         "flop_per_call": fl, "fp64_inst_per_call": pipe_inst, "kernel_ms": k_ms,

@@ -159,6 +159,11 @@ mem_status mem_last_pass_ms(mem_handle* h, double* ms, int64_t* evals);
  * The denominator of the "alu" roofline (MEASURED_PEAKS.json has no FP64 figure). */
 mem_status mem_measure_fp64_peak(int32_t repeats, double* tflops, void* cuda_stream);
 
+/* The same measurement with three distinct 64-bit register operands per DFMA (x = fma(x, y, z), y and z in
+ * registers): what the register file sustains for generic fused multiply-adds, about 2/3 of the figure
+ * above on B200.  Reported beside the roofline as the ceiling of register-operand code. */
+mem_status mem_measure_fp64_peak_rrr(int32_t repeats, double* tflops, void* cuda_stream);
+
 /* Thread-local description of the last error on this thread ("" if none). */
 const char* mem_last_error(void);
 

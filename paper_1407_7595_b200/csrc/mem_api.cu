@@ -414,7 +414,7 @@ mem_status mem_last_pass_ms(mem_handle* h, double* ms, int64_t* evals) {
   return MEM_OK;
 }
 
-mem_status mem_measure_fp64_peak(int32_t repeats, double* tflops, void* cuda_stream) {
+static mem_status measure_fp64(bool rrr, int32_t repeats, double* tflops, void* cuda_stream) {
   if (!tflops || repeats < 1) return fail(MEM_ERR_INVALID_ARG, "tflops is NULL or repeats < 1");
   cudaStream_t st = (cudaStream_t)cuda_stream;
   int dev = 0, sms = 0;
@@ -429,7 +429,8 @@ mem_status mem_measure_fp64_peak(int32_t repeats, double* tflops, void* cuda_str
   double best = 0.0;
   for (int r = 0; r < repeats + 1; ++r) {                  // first launch is the warm-up
     cudaEventRecord(a, st);
-    fp64_peak_kernel<<<blocks, threads, 0, st>>>(sink, 0.999999, 1e-9);
+    if (rrr) fp64_peak_kernel<true><<<blocks, threads, 0, st>>>(sink, 0.999999, 1e-9);
+    else fp64_peak_kernel<false><<<blocks, threads, 0, st>>>(sink, 0.999999, 1e-9);
     cudaEventRecord(b, st);
     cudaError_t e = cudaEventSynchronize(b);
     float ms = 0.f;
@@ -444,6 +445,14 @@ mem_status mem_measure_fp64_peak(int32_t repeats, double* tflops, void* cuda_str
   cudaFree(sink); cudaEventDestroy(a); cudaEventDestroy(b);
   *tflops = best;
   return MEM_OK;
+}
+
+mem_status mem_measure_fp64_peak(int32_t repeats, double* tflops, void* cuda_stream) {
+  return measure_fp64(false, repeats, tflops, cuda_stream);
+}
+
+mem_status mem_measure_fp64_peak_rrr(int32_t repeats, double* tflops, void* cuda_stream) {
+  return measure_fp64(true, repeats, tflops, cuda_stream);
 }
 
 mem_status mem_integrate(mem_handle* h, const double* events, int64_t n_events, int64_t n_points, uint64_t seed,

@@ -110,6 +110,48 @@ __device__ __forceinline__ double rcp_fast(double x) {
   return fma(y, e, y);
 }
 
+// tan(t) for the Breit-Wigner maps (O6): t = atan(..) lies strictly inside (-pi/2, pi/2), so no
+// general range reduction (and none of libdevice's large-argument path) is needed.  |t| <= pi/4:
+// tan = S(t)/C(t); otherwise with r = pi/2 - |t| (pi/2 in two parts): tan = C(r)/S(r).  S, C are
+// degree-13 / degree-12 polynomials (Chebyshev interpolants in r^2 on 1.02 [0, (pi/4)^2]; the quotient
+// is within 2.0e-17 of tan before rounding), one reciprocal.  tan_bw_n evaluates N arguments with
+// the Horner steps interleaved so that each coefficient is fetched once for all of them.
+template <int N>
+__device__ __forceinline__ void tan_bw_n(const double (&t)[N], double (&out)[N]) {
+  constexpr double kS[6] = {-0x1.5555555555554p-3, 0x1.1111111110a86p-7, -0x1.a01a019e3e0afp-13,
+                            0x1.71de373e0fee6p-19, -0x1.ae5fb0a5df712p-26, 0x1.5deb31d167e93p-33};
+  constexpr double kC[6] = {0x1.5555555555555p-5, -0x1.6c16c16c168d0p-10, 0x1.a01a019f2bd7bp-16,
+                            -0x1.27e4f9eb9238ep-22, 0x1.1eeb3bafbb15dp-29, -0x1.905db35e3086ap-37};
+  double r[N], z[N], ps[N], pc[N];
+  bool big[N];
+#pragma unroll
+  for (int j = 0; j < N; ++j) {
+    const double a = fabs(t[j]);
+    big[j] = a > 0.78539816339744830962;
+    r[j] = big[j] ? (1.57079632679489655800e+00 - a) + 6.12323399573676603587e-17 : a;
+    z[j] = r[j] * r[j];
+    ps[j] = kS[5]; pc[j] = kC[5];
+  }
+#pragma unroll
+  for (int i = 4; i >= 0; --i) {
+#pragma unroll
+    for (int j = 0; j < N; ++j) { ps[j] = fma(ps[j], z[j], kS[i]); pc[j] = fma(pc[j], z[j], kC[i]); }
+  }
+#pragma unroll
+  for (int j = 0; j < N; ++j) {
+    const double sn = fma(r[j] * z[j], ps[j], r[j]);
+    const double cs = fma(z[j] * z[j], pc[j], fma(-0.5, z[j], 1.0));
+    const double q = (big[j] ? cs : sn) * rcp_fast(big[j] ? sn : cs);
+    out[j] = copysign(q, t[j]);
+  }
+}
+__device__ __forceinline__ double tan_bw(double t) {
+  const double a[1] = {t};
+  double o[1];
+  tan_bw_n<1>(a, o);
+  return o[0];
+}
+
 // toy PDF shape product f(x1) f(x2) / A^2 = (x1 x2)^pow_x ((1-x1)(1-x2))^pow_1mx (O4)
 __device__ __forceinline__ double pdf_pair(const DevConst& c, double x1, double x2) {
   const double xx = x1 * x2, yy = (1.0 - x1) * (1.0 - x2);
@@ -133,7 +175,7 @@ template <typename T> struct TfAcc { T esum, fac; };
 __device__ __forceinline__ float rcp_fast(float x) { return __frcp_rn(x); }
 __device__ __forceinline__ double m_exp(double x) { return exp(x); }
 __device__ __forceinline__ float m_exp(float x) { return __expf(x); }
-__device__ __forceinline__ double m_tan(double x) { return tan(x); }
+__device__ __forceinline__ double m_tan(double x) { return tan_bw(x); }
 __device__ __forceinline__ float m_tan(float x) { return tanf(x); }
 __device__ __forceinline__ double m_rsqrt(double x) { return rsqrt(x); }
 __device__ __forceinline__ float m_rsqrt(float x) { return rsqrtf(x); }

@@ -341,16 +341,26 @@ __global__ void eval_points_kernel(const DevConstR<typename P::real> c, const do
 }
 
 // FP64 peak microbenchmark: 8 independent DFMA chains per thread, kPeakIters x 8 FMAs each.
+// RRR = false: x = fma(x, a, b) with uniform a, b -- one register operand per instruction, the pipe's
+// nominal 64 DFMA/clk/SM.  RRR = true: x = fma(x, y, z) with y, z in registers -- three distinct
+// 64-bit register operands per instruction, which the register file feeds at only 2/3 of that rate
+// (measured: 12.3 vs 18.45 T inst/s); DMUL and DADD with two register operands run at the full rate.
 constexpr int kPeakIters = 4096;
+template <bool RRR>
 __global__ void __launch_bounds__(256) fp64_peak_kernel(double* __restrict__ sink, double a, double b) {
-  double x0 = threadIdx.x, x1 = x0 + 1.0, x2 = x0 + 2.0, x3 = x0 + 3.0, x4 = x0 + 4.0, x5 = x0 + 5.0, x6 = x0 + 6.0,
-         x7 = x0 + 7.0;
-#pragma unroll 8
-  for (int i = 0; i < kPeakIters; ++i) {
-    x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
-    x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+  double x[8], y[8], z[8];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    x[j] = threadIdx.x + j;
+    y[j] = a - 1e-12 * (double)(threadIdx.x + j);
+    z[j] = b * (double)(j + 1 + threadIdx.x);
   }
-  const double s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+#pragma unroll 2
+  for (int i = 0; i < kPeakIters; ++i) {
+#pragma unroll
+    for (int j = 0; j < 8; ++j) x[j] = RRR ? fma(x[j], y[j], z[j]) : fma(x[j], a, b);
+  }
+  const double s = ((x[0] + x[1]) + (x[2] + x[3])) + ((x[4] + x[5]) + (x[6] + x[7]));
   if (s == 12345.678) sink[0] = s;     // never true for the arguments used; keeps the chains alive
 }
 

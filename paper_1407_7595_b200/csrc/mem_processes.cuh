@@ -591,10 +591,11 @@ struct ProcTTdilep {
     const double Eb0 = fma(ec[J0 + 1], u[0], ec[J0]), Eb1 = fma(ec[J1 + 1], u[1], ec[J1]);
     const double iEb0 = ixb0 * ec[IEJ0], iEb1 = ixb1 * ec[IEJ1];
     // ---- S2: the four mapped masses, s_k - m_k^2 = m Gam tan t_k (O6)
-    const double smW0 = c.mWGW * tan(fma(c.tW_dt, u[2], c.tW_lo));
-    const double smT0 = c.mtGt * tan(fma(c.tT_dt, u[3], c.tT_lo));
-    const double smW1 = c.mWGW * tan(fma(c.tW_dt, u[4], c.tW_lo));
-    const double smT1 = c.mtGt * tan(fma(c.tT_dt, u[5], c.tT_lo));
+    const double tk[4] = {fma(c.tW_dt, u[2], c.tW_lo), fma(c.tT_dt, u[3], c.tT_lo), fma(c.tW_dt, u[4], c.tW_lo),
+                          fma(c.tT_dt, u[5], c.tT_lo)};
+    double tn[4];
+    tan_bw_n<4>(tk, tn);
+    const double smW0 = c.mWGW * tn[0], smT0 = c.mtGt * tn[1], smW1 = c.mWGW * tn[2], smT1 = c.mtGt * tn[3];
     const double sW0 = c.mW2 + smW0, sW1 = c.mW2 + smW1;
     const double dm2 = c.mt2 - c.mW2;
     // Delta/(2 E_b) = b.nu / E_b = ((s_t - s_W)/2 - b.l) / E_b must be positive
