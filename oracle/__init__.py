@@ -39,7 +39,10 @@ class Params(C.Structure):
         "tf_w_tail", "tf_mu1", "tf_sig1", "tf_mu2", "tf_sig2",
         "jetE_rlo", "jetE_rhi", "bw_nwidths", "nu_pz_max", "nu_eta_max", "met_sigma", "met_nsigma",
         "vegas_alpha")] + [("vegas_points", C.c_int64), ("vegas_iters", C.c_int32),
-                           ("vegas_bins", C.c_int32), ("n_flav", C.c_int32), ("n_perm", C.c_int32)]
+                           ("vegas_bins", C.c_int32), ("n_flav", C.c_int32), ("n_perm", C.c_int32),
+                           ("pdf_mode", C.c_int32), ("pdf_nx", C.c_int32), ("pdf_nq", C.c_int32), ("pdf_pad", C.c_int32),
+                           ("pdf_lxmin", C.c_double), ("pdf_lxmax", C.c_double), ("pdf_lqmin", C.c_double),
+                           ("pdf_lqmax", C.c_double), ("pdf_Q", C.c_double), ("pdf_data", C.c_void_p)]
 
 
 _lib = None
@@ -63,6 +66,8 @@ def lib():
         L.orc_pdf_shape.restype = C.c_double
         L.orc_tf_jet.argtypes = [C.POINTER(Params), C.c_double, C.c_double]
         L.orc_tf_jet.restype = C.c_double
+        L.orc_pdf_grid.argtypes = [C.POINTER(Params), C.c_int, C.c_double, C.c_double]
+        L.orc_pdf_grid.restype = C.c_double
         L.orc_bw_window.argtypes = [C.c_double] * 4 + [_dp, _dp]
         L.orc_bw_window.restype = None
         L.orc_bw_point.argtypes = [C.c_double] * 3 + [_dp, _dp, _dp]
@@ -114,6 +119,21 @@ def params_default(process: int) -> Params:
     if lib().orc_params_default(process, C.byref(p)) != 0:
         raise ValueError("unknown process %r" % process)
     return p
+
+
+def set_pdf_grid(p: Params, table, lxmin, lxmax, lqmin, lqmax, Q):
+    """NEXT-3: switch p to grid PDFs.  table = float64 [6, NQ, NX]; the array is kept alive on p."""
+    t = np.ascontiguousarray(table, dtype=np.float64)
+    assert t.ndim == 3 and t.shape[0] == 6
+    p._pdf_keepalive = t
+    p.pdf_mode, p.pdf_nq, p.pdf_nx = 1, t.shape[1], t.shape[2]
+    p.pdf_lxmin, p.pdf_lxmax, p.pdf_lqmin, p.pdf_lqmax, p.pdf_Q = lxmin, lxmax, lqmin, lqmax, Q
+    p.pdf_data = t.ctypes.data
+    return p
+
+
+def pdf_grid(p, species, x, Q):
+    return lib().orc_pdf_grid(C.byref(p), int(species), float(x), float(Q))
 
 
 def n_fields(process):

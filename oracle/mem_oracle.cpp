@@ -107,6 +107,46 @@ template <typename R> R tf_jet(const orc_params* p, R E_jet, R E) {
          R(p->tf_w_tail) * gauss<R>(d, R(p->tf_mu2) * E, R(p->tf_sig2) * E);
 }
 
+// NEXT-3, grid PDFs ("stored in (x, Q^2) grids for each parton flavor ... evaluated using
+// bilinear interpolation within the kernel"; listing PAPER.md:274-306 Fig. A.5, reading A17): uniform
+// grid in (ln x, ln Q) with NX x NQ samples per species, sample i at min + i (max - min)/N (the
+// listing's step), cell index clamped to [0, N-2] (so points outside the grid extrapolate the edge
+// cell), value = sum of the four corners weighted by the opposite areas / (dx dq).
+// species: 0 = gluon, 1..5 = d, u, s, c, b (antiquark = quark in the synthesised tables).
+template <typename R> R pdf_grid(const orc_params* p, int species, R x, R Q) {
+  const int NX = p->pdf_nx, NQ = p->pdf_nq;
+  if (species < 0 || species > 5) return R(0);
+  const double* data = p->pdf_data + (size_t)species * NX * NQ;
+  const R lx = std::log(x), lq = std::log(Q);
+  const R dx = (R(p->pdf_lxmax) - R(p->pdf_lxmin)) / R(NX), dq = (R(p->pdf_lqmax) - R(p->pdf_lqmin)) / R(NQ);
+  int ix = 0, iq = 0;
+  if (R(p->pdf_lxmin) < lx) ix = (int)((lx - R(p->pdf_lxmin)) / dx);
+  ix = ix < NX - 1 ? ix : NX - 2;
+  if (R(p->pdf_lqmin) < lq) iq = (int)((lq - R(p->pdf_lqmin)) / dq);
+  iq = iq < NQ - 1 ? iq : NQ - 2;
+  const R c11x = R(p->pdf_lxmin) + dx * R(ix), c11q = R(p->pdf_lqmin) + dq * R(iq);
+  const R c22x = R(p->pdf_lxmin) + dx * R(ix + 1), c22q = R(p->pdf_lqmin) + dq * R(iq + 1);
+  const R norm = dx * dq;
+  const R d00 = data[(size_t)iq * NX + ix], d10 = data[(size_t)(iq + 1) * NX + ix];
+  const R d01 = data[(size_t)iq * NX + ix + 1], d11 = data[(size_t)(iq + 1) * NX + ix + 1];
+  return d00 / norm * (c22x - lx) * (c22q - lq) + d01 / norm * (lx - c11x) * (c22q - lq) +
+         d10 / norm * (c22x - lx) * (lq - c11q) + d11 / norm * (lx - c11x) * (lq - c11q);
+}
+
+// sum over initial-state flavours of f_a(x1) f_b(x2) |M_ab|^2 for t tbar production:
+// g g, and q qbar + qbar q for the first n_flav quark species.  Toy mode (O4): every species has
+// the shape A x^a (1-x)^b; grid mode: pdf_grid at the fixed scale pdf_Q.
+template <typename R> R tt_flavour_sum(const orc_params* p, R x1, R x2, R me_gg, R me_qq) {
+  if (!p->pdf_mode) {
+    const R ff = pdf_shape<R>(p, x1) * pdf_shape<R>(p, x2);
+    return ff * (R(p->pdf_A_g) * R(p->pdf_A_g) * me_gg + R(2) * R(p->n_flav) * R(p->pdf_A_q) * R(p->pdf_A_q) * me_qq);
+  }
+  const R Q = p->pdf_Q;
+  R lqq = R(0);
+  for (int f = 1; f <= p->n_flav; ++f) lqq += R(2) * pdf_grid<R>(p, f, x1, Q) * pdf_grid<R>(p, f, x2, Q);
+  return pdf_grid<R>(p, 0, x1, Q) * pdf_grid<R>(p, 0, x2, Q) * me_gg + lqq * me_qq;
+}
+
 // integrate over q^2 of the propagators.  s = m^2 + m Gam tan t.
 template <typename R> void bw_window(R m, R Gam, R s_lo, R s_hi, R* t_lo, R* t_hi) {
   *t_lo = std::atan((s_lo - m * m) / (m * Gam));
@@ -384,8 +424,7 @@ template <typename R> R weight_tt_ljets(const orc_params* p, const double* rec, 
   R q1[4], q2[4], pta[4], ptba[4];
   beams<R>(p, x1, x2, q1, q2);
   for (int k = 0; k < 4; ++k) { pta[k] = mom[k] + mom[4 + k] + mom[8 + k]; ptba[k] = mom[12 + k] + mom[16 + k] + mom[20 + k]; }
-  R prod = R(p->pdf_A_g) * R(p->pdf_A_g) * me_tt_gg<R>(p, q1, q2, pta, ptba) +
-           R(2) * R(p->n_flav) * R(p->pdf_A_q) * R(p->pdf_A_q) * me_tt_qq<R>(p, q1, q2, pta, ptba);
+  R prod = tt_flavour_sum<R>(p, x1, x2, me_tt_gg<R>(p, q1, q2, pta, ptba), me_tt_qq<R>(p, q1, q2, pta, ptba));   // includes the PDFs
   // narrow-width factorised decays, 1/2 = average over the decaying top's spin.  The leptonic
   // W mass is the mapped variable: its propagator is D(m Gam tan t) (reading O6).
   R dec_lep = R(0.5) * me_top_decay_D<R>(p, R(1), pta, mom + 8, mom, mom + 4, DW_lep);
@@ -393,7 +432,7 @@ template <typename R> R weight_tt_ljets(const orc_params* p, const double* rec, 
   R mt = p->m_t, Gt = p->Gam_t;
   R Dt = bw_D<R>(st - mt * mt, mt, Gt), Dtb = bw_D<R>(stb - mt * mt, mt, Gt);
   R me = prod * Dt * Dtb * dec_lep * dec_had;
-  R ff = pdf_shape<R>(p, x1) * pdf_shape<R>(p, x2);
+  R ff = R(1);                                  // PDFs are inside prod (tt_flavour_sum)
   R flux = x1 * x2 * S / R(4);
   dbg_store<R>(dbg, 0, 6, x1, x2, mom);
   if (dbg) dbg[0] = 1;
@@ -664,13 +703,12 @@ template <typename R> R weight_tt_dilep(const orc_params* p, const double* rec, 
     R q1[4], q2[4], pta[4], ptba[4];
     beams<R>(p, x1, x2, q1, q2);
     for (int c = 0; c < 4; ++c) { pta[c] = mom[c] + mom[4 + c] + mom[8 + c]; ptba[c] = mom[12 + c] + mom[16 + c] + mom[20 + c]; }
-    const R prod = R(p->pdf_A_g) * R(p->pdf_A_g) * me_tt_gg<R>(p, q1, q2, pta, ptba) +
-                   R(2) * R(p->n_flav) * R(p->pdf_A_q) * R(p->pdf_A_q) * me_tt_qq<R>(p, q1, q2, pta, ptba);
+    const R prod = tt_flavour_sum<R>(p, x1, x2, me_tt_gg<R>(p, q1, q2, pta, ptba), me_tt_qq<R>(p, q1, q2, pta, ptba));   // includes the PDFs
     // t -> b l+ nu: (p_t.p_l+)(p_b.p_nu);  tbar -> bbar l- nubar: (p_tbar.p_l-)(p_bbar.p_nubar)
     const R dec1 = R(0.5) * me_top_decay_D<R>(p, R(1), pta, mom + 8, mom, mom + 4, Dk[0]);
     const R dec2 = R(0.5) * me_top_decay_D<R>(p, R(1), ptba, mom + 20, mom + 12, mom + 16, Dk[2]);
     const R me = prod * Dk[1] * Dk[3] * dec1 * dec2;
-    const R ff = pdf_shape<R>(p, x1) * pdf_shape<R>(p, x2);
+    const R ff = R(1);                                  // PDFs are inside prod (tt_flavour_sum)
     const R flux = x1 * x2 * S / R(4);
     const R ws = J / (twopi3 * twopi3 * R(4) * nu.E * nub.E) * ff * me / flux;
     if (!std::isfinite((double)ws)) continue;
@@ -760,13 +798,12 @@ template <typename R> R parton_weight_tt_ljets(const orc_params* p, const double
     R q1[4], q2[4], pt[4], ptb[4];
     beams<R>(p, x1, x2, q1, q2);
     for (int c = 0; c < 4; ++c) { pt[c] = mom[c] + mom[4 + c] + mom[8 + c]; ptb[c] = mom[12 + c] + mom[16 + c] + mom[20 + c]; }
-    const R prod = R(p->pdf_A_g) * R(p->pdf_A_g) * me_tt_gg<R>(p, q1, q2, pt, ptb) +
-                   R(2) * R(p->n_flav) * R(p->pdf_A_q) * R(p->pdf_A_q) * me_tt_qq<R>(p, q1, q2, pt, ptb);
+    const R prod = tt_flavour_sum<R>(p, x1, x2, me_tt_gg<R>(p, q1, q2, pt, ptb), me_tt_qq<R>(p, q1, q2, pt, ptb));   // includes the PDFs
     const R dec_lep = R(0.5) * me_top_decay<R>(p, R(1), pt, mom + 8, mom, mom + 4);
     const R dec_had = R(0.5) * R(p->V_ud) * R(p->V_ud) * me_top_decay<R>(p, R(3), ptb, mom + 12, mom + 16, mom + 20);
     V4<R> t4 = from_arr(pt), tb4 = from_arr(ptb);
     const R Dt = bw_D<R>(dot(t4, t4) - mt * mt, mt, Gt), Dtb = bw_D<R>(dot(tb4, tb4) - mt * mt, mt, Gt);
-    const R ff = pdf_shape<R>(p, x1) * pdf_shape<R>(p, x2);
+    const R ff = R(1);                                  // PDFs are inside prod (tt_flavour_sum)
     const R w = ff * prod * Dt * Dtb * dec_lep * dec_had / (x1 * x2 * S / R(4));
     if (std::isfinite((double)w)) sum += w;
   }
@@ -939,6 +976,8 @@ int orc_parton_weights(int process, const orc_params* p, const double* mom, int6
   }
   return 0;
 }
+
+double orc_pdf_grid(const orc_params* p, int species, double x, double Q) { return pdf_grid<double>(p, species, x, Q); }
 
 double orc_weight(int process, const orc_params* p, const double* rec, const double* u, double* dbg) {
   return weight_any<double>(process, p, rec, u, dbg);

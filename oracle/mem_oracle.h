@@ -42,6 +42,12 @@ typedef struct orc_params {
    * 0 or 1 = the record order only; ORC_TT_LJETS: 4 = b-tags known (the two b jets swapped x the two
    * light jets swapped), 24 = all assignments; ORC_TT_DILEP: 2 = both b assignments. */
   int32_t n_perm;
+  /* NEXT-3, grid PDFs (PAPER.md:141, :274-306 Fig. A.5): pdf_mode != 0 replaces the toy PDF by bilinear
+   * interpolation of pdf_data[species][iq][ix] (species 0 = g, 1..5 = d,u,s,c,b; NQ x NX samples on a
+   * uniform grid in ln x, ln Q) at the fixed scale pdf_Q.  t tbar processes only. */
+  int32_t pdf_mode, pdf_nx, pdf_nq, pdf_pad;
+  double pdf_lxmin, pdf_lxmax, pdf_lqmin, pdf_lqmax, pdf_Q;
+  const double* pdf_data;
 } orc_params;
 
 int  orc_params_default(int process, orc_params* p);
@@ -57,6 +63,7 @@ void   orc_uniforms(uint64_t seed, uint64_t event, uint64_t point, uint32_t iter
 /* --- building blocks, exposed so that the tests can pin each one --- */
 double orc_pdf_shape(const orc_params* p, double x);
 double orc_tf_jet(const orc_params* p, double E_jet, double E_parton);
+double orc_pdf_grid(const orc_params* p, int species, double x, double Q);   /* NEXT-3 */
 /* Breit-Wigner map: t-window of [s_lo, s_hi]; at t: s - m^2, ds/dt, D(s). */
 void   orc_bw_window(double m, double Gam, double s_lo, double s_hi, double* t_lo, double* t_hi);
 void   orc_bw_point(double m, double Gam, double t, double* s_minus_m2, double* dsdt, double* D);

@@ -143,3 +143,28 @@ def make_parton_events(n_events: int, seed: int = DEFAULT_SEED, sqrt_s: float = 
     q, qb = _two_body(r, W2, np.zeros(n), np.zeros(n))
     ev = np.concatenate([lep, nu, b_had, b_lep, q, qb], axis=0)
     return np.ascontiguousarray(ev, dtype=np.float64)
+
+
+# ------------------------------------------------------------------------------------------
+# NEXT-3, grid PDFs: the paper fills per-flavour (x, Q) tables by querying
+# LHAPDF / CTEQ, which are not available; these tables are synthesised from BASELINE's toy shape
+# A x^a (1-x)^b (times a mild, made-up ln Q slope so that the Q interpolation is exercised) and
+# stand in for them.  Sample i sits at min + i (max - min) / N, the listing's convention.
+# ------------------------------------------------------------------------------------------
+PDF_GRID = dict(nx=256, nq=16, lxmin=float(np.log(1e-6)), lxmax=0.0, lqmin=float(np.log(10.0)),
+                lqmax=float(np.log(1000.0)))
+
+
+def make_pdf_table(A_g: float = 1.0, A_q: float = 1.0, pow_x: float = -0.5, pow_1mx: float = 3.0,
+                   q_slope: float = 0.0, Q0: float = 173.0, **grid) -> np.ndarray:
+    """float64 [6, NQ, NX]: species 0 = gluon, 1..5 = d, u, s, c, b."""
+    g = dict(PDF_GRID, **grid)
+    lx = g["lxmin"] + (g["lxmax"] - g["lxmin"]) / g["nx"] * np.arange(g["nx"])
+    lq = g["lqmin"] + (g["lqmax"] - g["lqmin"]) / g["nq"] * np.arange(g["nq"])
+    x = np.exp(lx)
+    shape = x ** pow_x * (1.0 - x) ** pow_1mx
+    qfac = 1.0 + q_slope * (lq - np.log(Q0))
+    tab = np.empty((6, g["nq"], g["nx"]))
+    for s in range(6):
+        tab[s] = (A_g if s == 0 else A_q) * qfac[:, None] * shape[None, :]
+    return tab
