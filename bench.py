@@ -65,6 +65,8 @@ def parse_args():
                     help="32 = fp32 integrand core of config 3 (reading A15)")
     ap.add_argument("--perm", type=int, default=0,
                     help="jet-parton assignments summed per point (NEXT-1): config 3/5: 4 or 24, config 4: 2")
+    ap.add_argument("--pdf", default="toy", choices=["toy", "grid"],
+                    help="grid = NEXT-3: bilinear (ln x, ln Q) tables synthesised from the toy PDF (configs 3-5)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--parton", action="store_true",
                     help="NEXT-2 parton-level mode: ME evaluations of --events configurations (default 10^5)")
@@ -85,7 +87,8 @@ def workload(cfg, args):
             5: "config5 ttbar l+jets 6-D + VEGAS 5x2^17"}[cfg]
     return proc, ne, npts, "%s, %d events x %d points/event, %s%s" % (
         name, ne, npts, "fp32 core (A15)" if args.precision == 32 else "fp64",
-        ", %d jet-parton assignments per point" % args.perm if args.perm > 1 else "")
+        (", %d jet-parton assignments per point" % args.perm if args.perm > 1 else "") +
+        (", grid PDFs" if args.pdf == "grid" else ""))
 
 
 # --------------------------------------------------------------------------------------------
@@ -237,6 +240,9 @@ def run_b200(args):
     if args.perm > 1:
         over["n_perm"] = args.perm
     it = mem.Integrator(proc, **over)
+    if args.pdf == "grid":
+        g = wl.PDF_GRID
+        it.set_pdf_grid(wl.make_pdf_table(), g["lxmin"], g["lxmax"], g["lqmin"], g["lqmax"], 173.0)
     it.set_event_offset(lo)
     out_p = torch.empty(ne, dtype=torch.float64, device="cuda")
     out_err = torch.empty_like(out_p)

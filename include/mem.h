@@ -128,6 +128,20 @@ mem_status mem_eval_points(mem_handle* h, const double* events, int64_t n_events
                            int64_t first_point, int64_t n, uint64_t seed, int32_t iteration,
                            const double* grid, double* out_w, void* cuda_stream);
 
+/* Grid PDFs (NEXT-3; "stored in (x, Q^2) grids for each parton flavor ... bilinear interpolation
+ * within the kernel", listing PAPER.md:274-306 Fig. A.5).  Replaces the toy PDF of this handle by tables:
+ * table : host, float64 [6][nq][nx]: species 0 = gluon, 1..5 = d, u, s, c, b (antiquark = quark); sample
+ *         (iq, ix) at ln Q = lqmin + iq (lqmax - lqmin)/nq, ln x = lxmin + ix (lxmax - lxmin)/nx (the listing's
+ *         step); copied, the caller keeps ownership.  NULL switches back to the toy PDF.
+ * Q     : the fixed factorisation scale (BASELINE: "at fixed Q"); the ln Q direction of the bilinear formula is
+ *         folded into one row per species here, the kernels interpolate in ln x; cell indices are clamped to
+ *         [0, n - 2] as in the listing, so points outside the grid extrapolate the edge cell.
+ * The flavour sum of t tbar production becomes f_g f_g |M_gg|^2 + sum over the first n_flav quark species of
+ * 2 f_q f_q |M_qq|^2.  MEM_PROC_TT_LJETS / MEM_PROC_TT_DILEP with precision 64 only (MEM_ERR_UNSUPPORTED
+ * otherwise).  Synchronises the device copy; call it between, not during, integrations. */
+mem_status mem_set_pdf_grid(mem_handle* h, const double* table, int32_t nx, int32_t nq, double lxmin, double lxmax,
+                            double lqmin, double lqmax, double Q);
+
 /* Parton-level mode (NEXT-2; Table 2): the transfer functions are delta
  * functions and nothing is integrated.  For each fully specified partonic configuration
  *   out_w[e] = sum over the handle's n_perm jet-parton assignments and the initial-state flavours of

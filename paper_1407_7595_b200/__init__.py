@@ -19,7 +19,7 @@ MEM_PROC_W_ENU, MEM_PROC_Z_BB, MEM_PROC_TT_LJETS, MEM_PROC_TT_DILEP = 1, 2, 3, 4
 
 EXPORTS = ("mem_params_default", "mem_event_fields", "mem_n_dims", "mem_create", "mem_destroy",
            "mem_set_event_offset", "mem_integrate", "mem_integrate_host", "mem_eval_points",
-           "mem_eval_parton", "mem_get_grid", "mem_launch_count", "mem_last_error", "mem_last_pass_ms", "mem_measure_fp64_peak",
+           "mem_eval_parton", "mem_set_pdf_grid", "mem_get_grid", "mem_launch_count", "mem_last_error", "mem_last_pass_ms", "mem_measure_fp64_peak",
            "mem_measure_fp64_peak_rrr")
 
 
@@ -66,6 +66,7 @@ def lib():
         L.mem_integrate_host.argtypes = [vp, dp, i64, i64, u64, dp, dp]
         L.mem_eval_points.argtypes = [vp, dp, i64, i64, i64, i64, u64, C.c_int32, dp, dp, vp]
         L.mem_eval_parton.argtypes = [vp, dp, i64, dp, vp]
+        L.mem_set_pdf_grid.argtypes = [vp, dp, C.c_int32, C.c_int32] + [C.c_double] * 5
         L.mem_get_grid.argtypes = [vp, i64, dp, vp]
         L.mem_launch_count.argtypes = [vp]
         L.mem_launch_count.restype = i64
@@ -203,6 +204,19 @@ def mem_eval_points(handle, events, event: int, first_point: int, n: int, seed: 
     return out_w
 
 
+def mem_set_pdf_grid(handle, table, lxmin, lxmax, lqmin, lqmax, Q):
+    """NEXT-3: table = float64 host array [6, NQ, NX] (None: back to the toy PDF)."""
+    import numpy as np
+    if table is None:
+        _check(lib().mem_set_pdf_grid(handle, None, 0, 0, 0.0, 0.0, 0.0, 0.0, 0.0))
+        return
+    t = np.ascontiguousarray(table, dtype=np.float64)
+    if t.ndim != 3 or t.shape[0] != 6:
+        raise ValueError("table must have shape [6, NQ, NX]")
+    _check(lib().mem_set_pdf_grid(handle, C.c_void_p(t.ctypes.data), t.shape[2], t.shape[1], float(lxmin), float(lxmax),
+                                  float(lqmin), float(lqmax), float(Q)))
+
+
 def mem_eval_parton(handle, momenta, out_w=None, stream=None):
     """Parton-level mode (NEXT-2): momenta = CUDA float64 tensor [24, n_events]; returns out_w [n_events]."""
     import torch
@@ -243,6 +257,9 @@ class Integrator:
 
     def eval_points(self, events, event, first_point, n, seed, **kw):
         return mem_eval_points(self.handle, events, event, first_point, n, seed, **kw)
+
+    def set_pdf_grid(self, table, lxmin=0.0, lxmax=0.0, lqmin=0.0, lqmax=0.0, Q=0.0):
+        mem_set_pdf_grid(self.handle, table, lxmin, lxmax, lqmin, lqmax, Q)
 
     def eval_parton(self, momenta, **kw):
         return mem_eval_parton(self.handle, momenta, **kw)

@@ -77,7 +77,7 @@ struct mem_handle {
   uint64_t event_offset;
   int64_t launches;
   int64_t grid_events;      // events covered by the grids of the last VEGAS call
-  Buffer ecs, partials, grids, hist, stage_in, stage_out;
+  Buffer ecs, partials, grids, hist, stage_in, stage_out, pdf_tab;
   cudaEvent_t ev_begin, ev_end;  // around the dominant kernel of the last mem_integrate
   int64_t last_evals;            // integrand evaluations of that kernel; 0 = none yet
 };
@@ -154,6 +154,7 @@ DevConst make_dev_const(const mem_params& p) {
   c.met_sigma = p.met_sigma; c.met_nsigma = p.met_nsigma;
   c.vegas_bins = p.vegas_bins; c.vegas_alpha = p.vegas_alpha;
   c.n_perm = p.n_perm > 1 ? p.n_perm : 1;
+  c.pdf_tab = nullptr; c.pdf_nx = 0; c.pdf_lxmin = c.pdf_dx = c.pdf_inv_dx = 0.0;
   return c;
 }
 
@@ -167,6 +168,7 @@ DevConstF to_float(const DevConst& d) {
   CP(vegas_alpha);
 #undef CP
   f.pdf_fast = d.pdf_fast; f.n_flav = d.n_flav; f.vegas_bins = d.vegas_bins; f.n_perm = d.n_perm;
+  f.pdf_tab = nullptr; f.pdf_nx = 0; f.pdf_lxmin = f.pdf_dx = f.pdf_inv_dx = 0.0;      // grid PDFs are fp64 only
   return f;
 }
 
@@ -386,7 +388,7 @@ mem_status mem_create(mem_process process, const mem_params* params, mem_handle*
 mem_status mem_destroy(mem_handle* h) {
   if (!h) return MEM_OK;
   cudaDeviceSynchronize();
-  Buffer* bs[] = {&h->ecs, &h->partials, &h->grids, &h->hist, &h->stage_in, &h->stage_out};
+  Buffer* bs[] = {&h->ecs, &h->partials, &h->grids, &h->hist, &h->stage_in, &h->stage_out, &h->pdf_tab};
   for (Buffer* b : bs)
     if (b->p) cudaFree(b->p);
   cudaEventDestroy(h->ev_begin);
@@ -527,6 +529,47 @@ mem_status mem_eval_points(mem_handle* h, const double* events, int64_t n_events
     case MEM_PROC_TT_DILEP: return eval_impl<ProcTTdilep>(h, events, n_events, event, first_point, n, seed, iteration, grid, out_w, st);
   }
   return fail(MEM_ERR_UNSUPPORTED, "process %d is not implemented", h->process);
+}
+
+mem_status mem_set_pdf_grid(mem_handle* h, const double* table, int32_t nx, int32_t nq, double lxmin, double lxmax,
+                            double lqmin, double lqmax, double Q) {
+  if (!h) return fail(MEM_ERR_INVALID_ARG, "handle is NULL");
+  if (!table) {                                             // back to the toy PDF
+    h->dc.pdf_tab = nullptr;
+    return MEM_OK;
+  }
+  if ((h->process != MEM_PROC_TT_LJETS && h->process != MEM_PROC_TT_DILEP) || h->params.precision != 64)
+    return fail(MEM_ERR_UNSUPPORTED, "grid PDFs are implemented for the t tbar processes in fp64");
+  if (nx < 2 || nq < 2 || nx > 65536 || nq > 65536) return fail(MEM_ERR_INVALID_ARG, "nx, nq outside 2..65536");
+  if (!(lxmax > lxmin) || !(lqmax > lqmin) || !(Q > 0.0)) return fail(MEM_ERR_INVALID_ARG, "empty grid range or Q <= 0");
+  // fold the ln Q direction of the bilinear interpolation (listing PAPER.md:274-306) into one row per species
+  const double lq = std::log(Q), dq = (lqmax - lqmin) / nq;
+  int iq = 0;
+  if (lqmin < lq) iq = (int)((lq - lqmin) / dq);
+  iq = iq < nq - 1 ? iq : nq - 2;
+  const double c11q = lqmin + dq * iq, c22q = lqmin + dq * (iq + 1);
+  double* row = new (std::nothrow) double[(size_t)6 * nx];
+  if (!row) return fail(MEM_ERR_NOMEM, "out of host memory");
+  for (int s = 0; s < 6; ++s)
+    for (int ix = 0; ix < nx; ++ix) {
+      const double d0 = table[((size_t)s * nq + iq) * nx + ix], d1 = table[((size_t)s * nq + iq + 1) * nx + ix];
+      row[(size_t)s * nx + ix] = (d0 * (c22q - lq) + d1 * (lq - c11q)) / dq;
+    }
+  cudaStream_t st = 0;
+  mem_status r = ensure(h->pdf_tab, (size_t)6 * nx * sizeof(double), st);
+  cudaError_t e = cudaSuccess;
+  if (r == MEM_OK) {
+    e = cudaMemcpy(h->pdf_tab.p, row, (size_t)6 * nx * sizeof(double), cudaMemcpyHostToDevice);   // synchronous
+  }
+  delete[] row;
+  if (r != MEM_OK) return r;
+  if (e != cudaSuccess) return fail(MEM_ERR_CUDA, "cudaMemcpy(pdf table): %s", cudaGetErrorString(e));
+  h->dc.pdf_tab = (const double*)h->pdf_tab.p;
+  h->dc.pdf_nx = nx;
+  h->dc.pdf_lxmin = lxmin;
+  h->dc.pdf_dx = (lxmax - lxmin) / nx;
+  h->dc.pdf_inv_dx = 1.0 / h->dc.pdf_dx;
+  return MEM_OK;
 }
 
 mem_status mem_eval_parton(mem_handle* h, const double* momenta, int64_t n_events, double* out_w, void* cuda_stream) {

@@ -50,6 +50,11 @@ struct DevConstR {
   int vegas_bins;
   T vegas_alpha;
   int n_perm;                      // jet-parton assignments summed per point (>= 1)
+  // NEXT-3 grid PDFs: tables already interpolated in ln Q at the handle's fixed scale, [6][pdf_nx]
+  // (species 0 = g, 1..5 = d,u,s,c,b), sample i at pdf_lxmin + i pdf_dx; nullptr = toy PDF
+  const double* pdf_tab;
+  int pdf_nx;
+  double pdf_lxmin, pdf_dx, pdf_inv_dx;
 };
 using DevConst = DevConstR<double>;   // the fp64 path
 using DevConstF = DevConstR<float>;   // fp32 integrand core of config 3 (reading A15)
@@ -179,6 +184,39 @@ __device__ __forceinline__ double m_tan(double x) { return tan_bw(x); }
 __device__ __forceinline__ float m_tan(float x) { return tanf(x); }
 __device__ __forceinline__ double m_rsqrt(double x) { return rsqrt(x); }
 __device__ __forceinline__ float m_rsqrt(float x) { return rsqrtf(x); }
+
+// NEXT-3 (listing :274-306, reading A17): one species of the grid PDF at ln x = L.
+// Cell index as in the listing: 0 below the grid, clamped to nx - 2 above (the edge cell is
+// extrapolated); linear in ln x between the two samples (the ln Q direction was folded in on the host).
+__device__ __forceinline__ double pdf_grid_1d(const double* __restrict__ tab, int nx, double lxmin, double dx,
+                                              double inv_dx, double L) {
+  int ix = 0;
+  if (lxmin < L) ix = (int)((L - lxmin) * inv_dx);
+  ix = ix < nx - 1 ? ix : nx - 2;
+  const double c11 = fma(dx, (double)ix, lxmin), c22 = fma(dx, (double)(ix + 1), lxmin);
+  return fma(__ldg(tab + ix), c22 - L, __ldg(tab + ix + 1) * (L - c11)) * inv_dx;
+}
+
+// Flavour sum of t tbar production: sum_ab f_a(x1) f_b(x2) |M_ab|^2 = Lgg Mgg + Lqq Mqq with
+// Mqq = tau1^2 + tau2^2 + rho/2 (the colour factor 4/9 is folded into Lqq).  Toy mode (O4): every
+// species has the same shape; grid mode: g g, and q qbar + qbar q for the first n_flav species.
+template <typename T> struct TtLumi { T gg, qq; };
+template <typename T>
+__device__ __forceinline__ TtLumi<T> tt_lumi(const DevConstR<T>& c, T x1, T x2) {
+  if (c.pdf_tab == nullptr) {
+    const T ff = pdf_pair(c, x1, x2);
+    return {ff * c.A_g2, ff * ((T(2.0) * c.n_flav * (T(4.0) / T(9.0))) * c.A_q2)};
+  }
+  const double L1 = log((double)x1), L2 = log((double)x2);
+  const double* t = c.pdf_tab;
+  const double gg = pdf_grid_1d(t, c.pdf_nx, c.pdf_lxmin, c.pdf_dx, c.pdf_inv_dx, L1) *
+                    pdf_grid_1d(t, c.pdf_nx, c.pdf_lxmin, c.pdf_dx, c.pdf_inv_dx, L2);
+  double qq = 0.0;
+  for (int f = 1; f <= c.n_flav; ++f)
+    qq = fma(pdf_grid_1d(t + f * c.pdf_nx, c.pdf_nx, c.pdf_lxmin, c.pdf_dx, c.pdf_inv_dx, L1),
+             pdf_grid_1d(t + f * c.pdf_nx, c.pdf_nx, c.pdf_lxmin, c.pdf_dx, c.pdf_inv_dx, L2), qq);
+  return {(T)gg, (T)(qq * (2.0 * 4.0 / 9.0))};
+}
 
 template <typename T>
 __device__ __forceinline__ void tf_accum(const DevConstR<T>& c, T inv_x, TfAcc<T>& acc) {

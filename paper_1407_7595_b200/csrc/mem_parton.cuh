@@ -47,6 +47,7 @@ parton_ttljets_kernel(const DevConst c, const double* __restrict__ mom, int64_t 
   const double shat = x1 * x2 * c.S;
   if (!(4.0 * c.mt2 < shat)) return;                               // reading A9
   const double h = 0.5 * c.sqrt_s, ish = 1.0 / shat, rho = 4.0 * c.mt2 * ish;
+  const TtLumi<double> lum = tt_lumi(c, x1, x2);                   // the same for every assignment
   const P4 l = p[0], nu = p[1];
   const P4 Wl = l + nu;
   const double swl_m = mdot(Wl, Wl) - c.mW2;
@@ -69,8 +70,8 @@ parton_ttljets_kernel(const DevConst c, const double* __restrict__ mom, int64_t 
     const double tau2 = h * ish * fma(x2, pt.E + pt.z, x1 * (ptb.E - ptb.z));
     const double iT = 1.0 / (tau1 * tau2), tt = fma(tau1, tau1, tau2 * tau2);
     const double Mgg = (iT * (1.0 / 6.0) - 0.375) * (tt + rho - 0.25 * rho * rho * iT);
-    const double Mqq = (4.0 / 9.0) * (tt + 0.5 * rho);
-    const double prod = c.gs4 * fma(c.A_g2, Mgg, 2.0 * c.n_flav * c.A_q2 * Mqq);
+    const double Mqq = tt + 0.5 * rho;
+    const double prod = c.gs4 * fma(lum.gg, Mgg, lum.qq * Mqq);    // flavour sum incl. the PDFs
     // propagators from the momenta
     const double st_m = mdot(pt, pt) - c.mt2, stb_m = mdot(ptb, ptb) - c.mt2, swh_m = mdot(Wh, Wh) - c.mW2;
     const double props = DWl / (fma(st_m, st_m, c.mtGt2) * fma(stb_m, stb_m, c.mtGt2) * fma(swh_m, swh_m, c.mWGW2));
@@ -80,7 +81,7 @@ parton_ttljets_kernel(const DevConst c, const double* __restrict__ mom, int64_t 
     const double me = prod * props * dec;
     if (isfinite(me)) sum += me;
   }
-  const double w = pdf_pair(c, x1, x2) * 4.0 * ish * sum;           // f f / (x1 x2 S / 4)
+  const double w = 4.0 * ish * sum;                                 // 1 / (x1 x2 S / 4)
   out_w[e] = isfinite(w) ? w : 0.0;
 }
 

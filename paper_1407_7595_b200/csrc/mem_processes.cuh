@@ -368,7 +368,8 @@ struct ProcTTljetsR {
     const T tt = fma(tau1, tau1, tau2 * tau2);
     const T Mgg = fma(iT, T(1.0) / T(6.0), -T(0.375)) * (tt + rho - T(0.25) * rho * rho * iT);
     const T Mqq = tt + T(0.5) * rho;
-    const T prod = fma(c.A_g2, Mgg, (T(2.0) * c.n_flav * (T(4.0) / T(9.0))) * c.A_q2 * Mqq);
+    const TtLumi<T> lum = tt_lumi(c, x1, x2);
+    const T prod = fma(lum.gg, Mgg, lum.qq * Mqq);                             // flavour sum incl. the PDFs
     // ---- S5: propagators and decays
     const T t_l = fma(T(0.5), sW, bl_l);                                       // p_t . l
     const T a_q = bh_q + q_qb;                                                 // p_tbar . q
@@ -382,7 +383,7 @@ struct ProcTTljetsR {
       decprop = t_l * bl_nu * a_q * bh_qb * rcp_fast(dens);
     }
     // ---- S4, S7
-    const T core = (pdf_pair(c, x1, x2) * ish) * prod * decprop;
+    const T core = ish * prod * decprop;
     if (isfinite(core)) sum += core;
     }
     const T pt = tf * (nuT * iden) * sum;
@@ -709,8 +710,8 @@ struct ProcTTdilep {
       const double tt = fma(tau1, tau1, tau2 * tau2);
       const double Mgg = fma(iT, 1.0 / 6.0, -0.375) * (tt + rho - 0.25 * rho * rho * iT);
       const double Mqq = tt + 0.5 * rho;
-      const double prod = fma(c.A_g2, Mgg, (2.0 * c.n_flav * (4.0 / 9.0)) * c.A_q2 * Mqq);
-      const double ws = pdf_pair(c, x1, x2) * ish * prod / xz;
+      const TtLumi<double> lum = tt_lumi(c, x1, x2);
+      const double ws = fma(lum.gg, Mgg, lum.qq * Mqq) * ish / xz;            // flavour sum incl. the PDFs
       if (isfinite(ws)) sum += ws;
     }
     // ---- S5: decays (p_t.p_l)(p_b.p_nu) per side; S6: MET TF; S7
