@@ -35,14 +35,14 @@ SEED = 20140729
 FP64_PER_CALL = {           # key = (config, jet-parton assignments per point)
     (1, 1): {"dfma": 87.3, "dmul": 47.0, "dadd": 17.9},
     (2, 1): {"dfma": 104.0, "dmul": 34.0, "dadd": 15.2},
-    (3, 1): {"dfma": 193.4, "dmul": 86.3, "dadd": 42.8},
-    (3, 24): {"dfma": 1442.3, "dmul": 1258.6, "dadd": 593.8},
-    (4, 1): {"dfma": 248.3, "dmul": 67.7, "dadd": 44.2},
-    (4, 2): {"dfma": 426.7, "dmul": 136.2, "dadd": 80.0},
-    (5, 1): {"dfma": 200.6, "dmul": 106.2, "dadd": 58.1},
+    (3, 1): {"dfma": 189.9, "dmul": 89.2, "dadd": 44.3},
+    (3, 24): {"dfma": 1438.9, "dmul": 1323.5, "dadd": 617.6},
+    (4, 1): {"dfma": 221.3, "dmul": 77.0, "dadd": 55.0},
+    (4, 2): {"dfma": 337.3, "dmul": 119.7, "dadd": 81.9},
+    (5, 1): {"dfma": 197.0, "dmul": 108.1, "dadd": 60.6},
 }
 # fp32 variant of config 3 (reading A15): executed FFMA / FMUL / FADD per call (same ncu pass)
-FP32_PER_CALL = {3: {"ffma": 82.7, "fmul": 90.3, "fadd": 32.7}, 5: {"ffma": 82.7, "fmul": 90.3, "fadd": 32.7}}
+FP32_PER_CALL = {3: {"ffma": 82.7, "fmul": 91.3, "fadd": 33.7}, 5: {"ffma": 82.7, "fmul": 91.3, "fadd": 33.7}}
 NOMINAL_FP64_FMA_PER_CLK_PER_SM = 64      # 4 SMSPs x 16 lanes; confirmed by the microbenchmark
 VEGAS_ITERS, VEGAS_POINTS = 5, 1 << 17    # BASELINE.json:configs[4]
 
