@@ -134,3 +134,41 @@ def test_parton_events_are_physical():
     t = ev[0] + ev[1] + ev[3]
     mt = np.sqrt(t[0] ** 2 - t[1] ** 2 - t[2] ** 2 - t[3] ** 2)
     assert np.all(np.abs(mt - 173.0) < 15 * 1.4 + 1e-6)
+
+
+def _record_from_partons(ev, e, swap=None):
+    """config-3 record [lep (pT, eta, phi), (E, eta, phi) x {b_had, b_lep, q, qbar'}, met, met_phi] from a parton
+    configuration with perfect jets (E_jet = E_parton); swap = (i, j) exchanges two jets of the record"""
+    m = ev[:, e].reshape(6, 4)
+
+    def pt_eta_phi(p):
+        pt = math.hypot(p[1], p[2])
+        return pt, math.asinh(p[3] / pt), math.atan2(p[2], p[1]) % (2 * math.pi)
+    lep, nu = m[0], m[1]
+    jets = [m[2], m[3], m[4], m[5]]
+    if swap:
+        jets[swap[0]], jets[swap[1]] = jets[swap[1]], jets[swap[0]]
+    rec = list(pt_eta_phi(lep))
+    for j in jets:
+        _, eta, phi = pt_eta_phi(j)
+        rec += [j[0], eta, phi]
+    npt, _, nphi = pt_eta_phi(nu)
+    return np.array(rec + [npt, nphi])
+
+
+def test_closure_the_integrand_peaks_on_physical_events():
+    """SURVEY.md 8(d) closure check: records built from on-shell t tbar configurations (perfect jets, MET
+    azimuth = neutrino azimuth) give likelihoods orders of magnitude above those of records in which a b jet
+    and a light jet are exchanged, and the true point (u = 1/3 for every jet: E = E_jet) is live."""
+    ev = wl.make_parton_events(12, seed=31)
+    p = oracle.params_default(3)
+    ratios = []
+    for e in range(12):
+        good = _record_from_partons(ev, e)
+        bad = _record_from_partons(ev, e, swap=(0, 2))          # b_had <-> q: wrong top and W masses
+        pg, _ = oracle.integrate(3, p, good.reshape(17, 1), 6000, 5)
+        pb, _ = oracle.integrate(3, p, bad.reshape(17, 1), 6000, 5)
+        assert pg[0] > 0
+        ratios.append(pg[0] / max(pb[0], 1e-300))
+    assert np.median(ratios) > 30.0
+    assert np.mean(np.array(ratios) > 1.0) >= 0.9
