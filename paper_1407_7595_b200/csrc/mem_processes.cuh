@@ -350,14 +350,14 @@ struct ProcTTljetsR {
     const T PE = tE + aE, Px = tx + ax, Py = ty + ay, Pz = tz + az;
     // gamma (E - beta.p) = (E P_E - p_T.P_T) / sqrt(P_E^2 - P_T^2): no division by P_E
     const T M2 = fma(PE, PE, -fma(Px, Px, Py * Py));
-    if (!(M2 > T(0))) continue;
+    bool ok = M2 > T(0);                     // cuts are predicates: the select at the end discards the point
     const T rM = m_rsqrt(M2);
     const T tEb = rM * fma(tE, PE, -fma(Px, tx, Py * ty)), aEb = rM * fma(aE, PE, -fma(Px, ax, Py * ay));
     const T PEb = tEb + aEb;
     const T x1 = (PEb + Pz) * c.inv_sqrt_s, x2 = (PEb - Pz) * c.inv_sqrt_s;
-    if (!(x1 > T(0) && x1 < T(1.0) && x2 > T(0) && x2 < T(1.0))) continue;
+    ok = ok && x1 > T(0) && x1 < T(1.0) && x2 > T(0) && x2 < T(1.0);
     const T xx = x1 * x2, shat = xx * c.S;
-    if (!(T(4.0) * c.mt2 < shat)) continue;                                       // reading A9
+    ok = ok && T(4.0) * c.mt2 < shat;                                             // reading A9
     // ---- S5: production.  tau1 = (q1.pt + q2.ptb)/s-hat, tau2 = (q2.pt + q1.ptb)/s-hat
     const T ish = rcp_fast(shat);
     const T hs = T(0.5) * c.sqrt_s * ish;
@@ -384,7 +384,7 @@ struct ProcTTljetsR {
     }
     // ---- S4, S7
     const T core = ish * prod * decprop;
-    if (isfinite(core)) sum += core;
+    if (ok && isfinite(core)) sum += core;
     }
     const T pt = tf * (nuT * iden) * sum;
     // fp64: the per-event constant (identical for every assignment) is applied here; fp32: by the
