@@ -106,7 +106,8 @@ mem_status mem_set_event_offset(mem_handle* h, uint64_t first_event);
  * cuda_stream : a cudaStream_t (NULL = legacy default stream).  All work is
  *   enqueued on it and the call returns without synchronising.  The handle's
  *   workspace grows on demand (a growth step synchronises that stream).
- * n_events == 0 is MEM_OK with no launch; n_points < 2 is MEM_ERR_INVALID_ARG.
+ * n_events == 0 is MEM_OK with no launch; n_points < 2 is MEM_ERR_INVALID_ARG; so is a call made while
+ * another CUDA device than the handle's is current.
  * Kinematically forbidden or non-finite points contribute w = 0 and still count in N. */
 mem_status mem_integrate(mem_handle* h, const double* events, int64_t n_events,
                          int64_t n_points, uint64_t seed,

@@ -466,6 +466,12 @@ mem_status mem_integrate(mem_handle* h, const double* events, int64_t n_events, 
   if (!events || !out_p || !out_err) return fail(MEM_ERR_INVALID_ARG, "events / out_p / out_err is NULL");
   if (!aligned8(events) || !aligned8(out_p) || !aligned8(out_err))
     return fail(MEM_ERR_INVALID_ARG, "device pointers must be 8-byte aligned");
+  {
+    int dev = -1;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev != h->device)
+      return fail(MEM_ERR_INVALID_ARG, "handle was created on device %d, the current device is %d", h->device, dev);
+  }
   if (h->event_offset + (uint64_t)n_events > 0x100000000ULL)
     return fail(MEM_ERR_INVALID_ARG, "event index exceeds the 32-bit Philox counter word");
   cudaStream_t st = (cudaStream_t)cuda_stream;
