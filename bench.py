@@ -43,6 +43,9 @@ FP64_PER_CALL = {           # key = (config, jet-parton assignments per point)
 }
 # fp32 variant of config 3 (reading A15): executed FFMA / FMUL / FADD per call (same ncu pass)
 FP32_PER_CALL = {3: {"ffma": 82.7, "fmul": 91.3, "fadd": 33.7}, 5: {"ffma": 82.7, "fmul": 91.3, "fadd": 33.7}}
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant launch at full size, from an ncu metric pass
+# of the same command (profiles/r01_ncu_config3.md); key = (config, events, points/event, assignments, precision)
+TRAFFIC_BYTES = {(3, 4096, 1 << 20, 1, 64): 1571584}
 NOMINAL_FP64_FMA_PER_CLK_PER_SM = 64      # 4 SMSPs x 16 lanes; confirmed by the microbenchmark
 VEGAS_ITERS, VEGAS_POINTS = 5, 1 << 17    # BASELINE.json:configs[4]
 
@@ -327,7 +330,7 @@ def run_b200(args):
         "fp64_pipe_frac": (k_evals * pipe_inst / (k_ms * 1e-3)) / (peak_meas * 1e12 / 2.0),
         "flop_per_call": fl, "fp64_inst_per_call": pipe_inst, "kernel_ms": k_ms,
         "kernel_share_of_step": k_ms * len(kms) / sum(ms),
-        "traffic": None,
+        "traffic": TRAFFIC_BYTES.get((cfg, ne, n_points, max(args.perm, 1), args.precision)) if args.pdf == "toy" else None,
         "hbm_gbs_event_result_path": (ne * mem.mem_event_fields(proc) * 8 + ne * 16) / (sum(ms) / len(ms) * 1e-3) / 1e9,
     }
     if args.precision == 32:
