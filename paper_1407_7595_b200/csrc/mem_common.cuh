@@ -150,6 +150,19 @@ __device__ __forceinline__ void tan_bw_n(const double (&t)[N], double (&out)[N])
     out[j] = copysign(q, t[j]);
   }
 }
+// cos(x) for 0 <= x <= pi/3 (the trigonometric form of the resolvent cubic): 1 - 2 sin^2(x/2) with the
+// sine polynomial of tan_bw_n on |x/2| <= pi/6; no range reduction, no large-argument path.
+__device__ __forceinline__ double cos_third(double x) {
+  constexpr double kS[6] = {-0x1.5555555555554p-3, 0x1.1111111110a86p-7, -0x1.a01a019e3e0afp-13,
+                            0x1.71de373e0fee6p-19, -0x1.ae5fb0a5df712p-26, 0x1.5deb31d167e93p-33};
+  const double h = 0.5 * x, z = h * h;
+  double ps = kS[5];
+#pragma unroll
+  for (int i = 4; i >= 0; --i) ps = fma(ps, z, kS[i]);
+  const double sn = fma(h * z, ps, h);
+  return fma(-2.0 * sn, sn, 1.0);
+}
+
 __device__ __forceinline__ double tan_bw(double t) {
   const double a[1] = {t};
   double o[1];

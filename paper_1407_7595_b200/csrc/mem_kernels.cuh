@@ -139,43 +139,45 @@ integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__
     const unsigned lt = (1u << lane) - 1u;
     int cnt2 = 0, cnt4 = 0, head2 = 0, head4 = 0;                                   // warp-uniform
     int64_t base = lo;
-    bool draining = false;
+    bool draining = base >= hi;
+    // One loop body serves both passes (the mode is warp-uniform): pass B whenever a queue holds a
+    // full batch, or anything at all once the chunk is exhausted; pass A otherwise.
     while (true) {
-      if (!draining) {
-        // pass A: one point per lane up to the quartic
-        const int64_t i = base + threadIdx.x;
-        int nr = 0;
-        if (i < hi) {
-          double u[D];
-          draw_uniforms<D>(rng, (uint64_t)i, ev_ctr, pass, u);
-          nr = P::template n_roots<PERM>(c, ec, u);
-        }
+      int which = -1;
+      if (cnt2 >= 32 || (draining && cnt2 > 0)) which = 0;
+      else if (cnt4 >= 32 || (draining && cnt4 > 0)) which = 1;
+      if (which < 0 && draining) break;
+      const bool pass_b = which >= 0;
+      int64_t i;
+      bool active;
+      if (pass_b) {
+        const int n_live = min(32, which ? cnt4 : cnt2), hd = which ? head4 : head2;
+        active = lane < n_live;
+        i = lo + q[which * 64 + ((hd + lane) & 63)];
+        if (which) { head4 += n_live; cnt4 -= n_live; } else { head2 += n_live; cnt2 -= n_live; }
+      } else {
+        i = base + threadIdx.x;
+        active = i < hi;
+        base += kThreads;
+        draining = base >= hi;
+      }
+      double r = 0.0;
+      if (active) {
+        double u[D];
+        draw_uniforms<D>(rng, (uint64_t)i, ev_ctr, pass, u);
+        r = P::weight_rt(c, ec, u, !pass_b);              // pass A: number of real roots; pass B: the weight
+      }
+      __syncwarp();                                        // the batch has been read before anything is queued
+      if (pass_b) {
+        s1 += r; s2 = fma(r, r, s2);
+      } else {
+        const int nr = (int)r;
         const unsigned m2 = __ballot_sync(0xffffffffu, nr > 0 && nr <= 2), m4 = __ballot_sync(0xffffffffu, nr > 2);
         if (nr > 2) q[64 + ((head4 + cnt4 + __popc(m4 & lt)) & 63)] = (uint32_t)(i - lo);
         else if (nr > 0) q[(head2 + cnt2 + __popc(m2 & lt)) & 63] = (uint32_t)(i - lo);
         cnt2 += __popc(m2); cnt4 += __popc(m4);
-        base += kThreads;
-        draining = base >= hi;
-        __syncwarp();
       }
-      // pass B: full batches, and whatever is left once the chunk is exhausted (one call site)
-      while (true) {
-        int which = -1;
-        if (cnt2 >= 32 || (draining && cnt2 > 0)) which = 0;
-        else if (cnt4 >= 32 || (draining && cnt4 > 0)) which = 1;
-        if (which < 0) break;
-        const int n_live = min(32, which ? cnt4 : cnt2), hd = which ? head4 : head2;
-        if (lane < n_live) {
-          const int64_t i = lo + q[which * 64 + ((hd + lane) & 63)];
-          double u[D];
-          draw_uniforms<D>(rng, (uint64_t)i, ev_ctr, pass, u);
-          const double w = eval_weight<P, PERM>(c, ec, c0, u);
-          s1 += w; s2 = fma(w, w, s2);
-        }
-        if (which) { head4 += n_live; cnt4 -= n_live; } else { head2 += n_live; cnt2 -= n_live; }
-        __syncwarp();
-      }
-      if (draining) break;
+      __syncwarp();
     }
   } else {
   double* wh = whist + (threadIdx.x >> 5) * D * B;

@@ -420,15 +420,15 @@ __device__ __forceinline__ double cubic_largest_root(double c2, double c1, doubl
   if (disc > 0.0) {
     const double sq = sqrt(disc);
     const double A = (Qh > 0.0) ? -cbrt(Qh + sq) : cbrt(sq - Qh);
-    w = (A != 0.0) ? A - P3 / A : 0.0;
+    w = (A != 0.0) ? fma(-P3, rcp_fast(A), A) : 0.0;
   } else {
     const double m2 = -P3, m = sqrt(m2);
     if (m == 0.0) {
       w = 0.0;
     } else {
-      double c = -Qh / (m2 * m);
+      double c = -Qh * rcp_fast(m2 * m);
       c = fmin(1.0, fmax(-1.0, c));
-      w = 2.0 * m * cos(acos(c) * (1.0 / 3.0));
+      w = 2.0 * m * cos_third(acos(c) * (1.0 / 3.0));
     }
   }
   double z = w - sh;
@@ -436,7 +436,7 @@ __device__ __forceinline__ double cubic_largest_root(double c2, double c1, doubl
   for (int it = 0; it < 2; ++it) {
     const double f = fma(fma(z + c2, z, c1), z, c0);
     const double fp = fma(fma(3.0, z, 2.0 * c2), z, c1);
-    const double zn = z - f / fp;
+    const double zn = fma(-f, rcp_fast(fp), z);
     if (isfinite(zn)) z = zn;
   }
   return z;
@@ -454,19 +454,19 @@ __device__ __forceinline__ int quartic_real_roots(double a3, double a2, double a
   if (!(z0 > 0.0)) z0 = 0.0;
   const double s = sqrt(z0);
   double qs;
-  if (s > 0.0) qs = q / s;
+  if (s > 0.0) qs = q * rcp_fast(s);
   else { const double t = fma(p, p, -4.0 * r); qs = (t > 0.0) ? sqrt(t) : 0.0; }
   const double m = 0.5 * (p + z0 - qs), n = 0.5 * (p + z0 + qs);
   int cnt = 0;
   const double d1 = fma(-4.0, m, z0), d2 = fma(-4.0, n, z0);
   if (d1 >= 0.0) {
     const double ya = 0.5 * (-s - sqrt(d1));
-    const double yb = (ya != 0.0) ? m / ya : 0.5 * (-s + sqrt(d1));
+    const double yb = (ya != 0.0) ? m * rcp_fast(ya) : 0.5 * (-s + sqrt(d1));
     x[0] = ya + shift; x[1] = yb + shift; cnt = 2;
   }
   if (d2 >= 0.0) {
     const double ya = 0.5 * (s + sqrt(d2));
-    const double yb = (ya != 0.0) ? n / ya : 0.5 * (s - sqrt(d2));
+    const double yb = (ya != 0.0) ? n * rcp_fast(ya) : 0.5 * (s - sqrt(d2));
     if (cnt == 0) { x[0] = ya + shift; x[1] = yb + shift; }
     else { x[2] = ya + shift; x[3] = yb + shift; }
     cnt += 2;
@@ -564,25 +564,14 @@ struct ProcTTdilep {
   }
 
   __device__ static double weight(const DevConst& c, const double* ec, const double (&u)[D]) {
-    return weight_impl<false>(c, ec, u);
+    return weight_rt(c, ec, u, false);
   }
 
-  // The number of real roots of the resultant quartic (0, 2, 4) at this point, the largest over the
-  // assignments: what the lane-compacting kernel (mem_kernels.cuh) sorts points by before it runs the
-  // expensive per-solution part on full warps.  Same code as weight(): the prelude is shared.
-  template <bool PERM>
-  __device__ static int n_roots(const DevConst& c, const double* ec, const double (&u)[D]) {
-    int nr = (int)weight_impl<true>(c, ec, u);
-    if (PERM) {
-#pragma unroll 1
-      for (int k = 1; k < c.n_perm; ++k) nr = max(nr, (int)weight_impl<true>(c, ec + k * NC, u));
-    }
-    return nr;
-  }
-
-  // COUNT_ONLY: stop after the quartic and return its number of real roots
-  template <bool COUNT_ONLY>
-  __device__ static double weight_impl(const DevConst& c, const double* ec, const double (&u)[D]) {
+  // count_only (a warp-uniform run-time flag, so that the prelude exists once in the kernel: the
+  // config-4 kernel is instruction-cache bound, profiles/r01_ncu_config4.md): stop after the resultant
+  // quartic and return its number of real roots (0, 2, 4) -- what the lane-compacting loop
+  // (mem_kernels.cuh) sorts points by before it runs the per-solution part on full warps.
+  __device__ static double weight_rt(const DevConst& c, const double* ec, const double (&u)[D], bool count_only) {
     // ---- S2: jets, transfer functions
     TfAcc<double> tfa{0.0, 1.0};
     const double xb0 = fma(c.dr, u[0], c.rlo), xb1 = fma(c.dr, u[1], c.rlo);
@@ -635,7 +624,7 @@ struct ProcTTdilep {
     double xr[4];
     const int nr = quartic_real_roots(R3 * ir4, R2 * ir4, R1 * ir4, R0 * ir4, xr);
     if (nr == 0) return 0.0;
-    if (COUNT_ONLY) return (double)nr;
+    if (count_only) return (double)nr;
     // ---- solution-independent pieces
     const double ptx = ec[PTX] + Eb0 * ec[J0 + 2] + Eb1 * ec[J1 + 2] + Sx;     // total transverse momentum
     const double pty = ec[PTY] + Eb0 * ec[J0 + 3] + Eb1 * ec[J1 + 3] + Sy;
@@ -651,7 +640,7 @@ struct ProcTTdilep {
       double x = (k == 0) ? xr[0] : (k == 1) ? xr[1] : (k == 2) ? xr[2] : xr[3];
       const double V = fma(vv1, x, V0);
       if (!(V != 0.0)) continue;
-      double y = -fma(fma(uu2, x, U1), x, U0) / V;
+      double y = -fma(fma(uu2, x, U1), x, U0) * rcp_fast(V);
       // Newton on g1 = |nu| - E_nu(x, y), g2 = |nubar| - E_nubar(Sx - x, Sy - y)
       double nz, nbz, xb, yb;
 #pragma unroll
@@ -667,7 +656,7 @@ struct ProcTTdilep {
         const double j12 = fma(fma(nz, ec[S0 + AY], y), iEn, -ec[S0 + LAY]);
         const double j21 = -fma(fma(nbz, ec[S1 + AX], xb), iEnb, -ec[S1 + LAX]);
         const double j22 = -fma(fma(nbz, ec[S1 + AY], yb), iEnb, -ec[S1 + LAY]);
-        const double idet = 1.0 / fma(j11, j22, -j12 * j21);
+        const double idet = rcp_fast(fma(j11, j22, -j12 * j21));
         x -= fma(g1, j22, -g2 * j12) * idet;
         y -= fma(j11, g2, -j21 * g1) * idet;
       }
@@ -711,7 +700,7 @@ struct ProcTTdilep {
       const double Mgg = fma(iT, 1.0 / 6.0, -0.375) * (tt + rho - 0.25 * rho * rho * iT);
       const double Mqq = tt + 0.5 * rho;
       const TtLumi<double> lum = tt_lumi(c, x1, x2);
-      const double ws = fma(lum.gg, Mgg, lum.qq * Mqq) * ish / xz;            // flavour sum incl. the PDFs
+      const double ws = fma(lum.gg, Mgg, lum.qq * Mqq) * ish * rcp_fast(xz);  // flavour sum incl. the PDFs
       if (isfinite(ws)) sum += ws;
     }
     // ---- S5: decays (p_t.p_l)(p_b.p_nu) per side; S6: MET TF; S7
