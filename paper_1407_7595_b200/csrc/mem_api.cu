@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <type_traits>
 
 #include "mem_kernels.cuh"
 #include "mem_parton.cuh"
@@ -235,14 +236,16 @@ mem_status launch_pass(mem_handle* h, int64_t n_events, int64_t n_points, int64_
   // lane-compacting kernels keep two queues of 64 32-bit point offsets per warp
   const size_t smem = integrate_smem(P::NC * h->dc.n_perm, P::D, h->dc.vegas_bins, MODE) +
                       ((P::kCompact && MODE == MODE_PLAIN) ? (size_t)kWarps * 128 * sizeof(uint32_t) : 0);
-  if (h->dc.n_perm > 1)
-    integrate_kernel<P, MODE, true><<<(unsigned)blocks, kThreads, smem, st>>>(
+  auto launch = [&](auto perm, auto grid) {
+    integrate_kernel<P, MODE, decltype(perm)::value, decltype(grid)::value><<<(unsigned)blocks, kThreads, smem, st>>>(
         dc_of<typename P::real>(h), (const double*)h->ecs.p, (const double*)h->grids.p, (double*)h->partials.p,
         (double*)h->hist.p, n_points, chunk, n_chunks, seed, h->event_offset, pass);
-  else
-    integrate_kernel<P, MODE, false><<<(unsigned)blocks, kThreads, smem, st>>>(
-        dc_of<typename P::real>(h), (const double*)h->ecs.p, (const double*)h->grids.p, (double*)h->partials.p,
-        (double*)h->hist.p, n_points, chunk, n_chunks, seed, h->event_offset, pass);
+  };
+  const bool perm = h->dc.n_perm > 1, grid = h->dc.pdf_tab != nullptr;
+  if (perm && grid) launch(std::true_type{}, std::true_type{});
+  else if (perm) launch(std::true_type{}, std::false_type{});
+  else if (grid) launch(std::false_type{}, std::true_type{});
+  else launch(std::false_type{}, std::false_type{});
   ++h->launches;
   CUDA_TRY(cudaGetLastError());
   return MEM_OK;

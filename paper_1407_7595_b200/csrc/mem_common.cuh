@@ -213,10 +213,12 @@ __device__ __forceinline__ double pdf_grid_1d(const double* __restrict__ tab, in
 // Flavour sum of t tbar production: sum_ab f_a(x1) f_b(x2) |M_ab|^2 = Lgg Mgg + Lqq Mqq with
 // Mqq = tau1^2 + tau2^2 + rho/2 (the colour factor 4/9 is folded into Lqq).  Toy mode (O4): every
 // species has the same shape; grid mode: g g, and q qbar + qbar q for the first n_flav species.
+// GRIDPDF = false compiles the toy branch only (the hot kernels are instantiated both ways and the
+// launch picks one: carrying the table code costs 1-4 % even when it is not taken).
 template <typename T> struct TtLumi { T gg, qq; };
-template <typename T>
+template <bool GRIDPDF, typename T>
 __device__ __forceinline__ TtLumi<T> tt_lumi(const DevConstR<T>& c, T x1, T x2) {
-  if (c.pdf_tab == nullptr) {
+  if (!GRIDPDF || c.pdf_tab == nullptr) {
     const T ff = pdf_pair(c, x1, x2);
     return {ff * c.A_g2, ff * ((T(2.0) * c.n_flav * (T(4.0) / T(9.0))) * c.A_q2)};
   }

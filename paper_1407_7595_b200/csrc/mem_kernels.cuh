@@ -28,17 +28,17 @@ __global__ void prepare_kernel(const DevConst c, const double* __restrict__ ev, 
 // the integrand at the unit-cube point u.  fp64 processes take u as it is; the fp32 variant
 // (reading A15) rounds u to fp32, clamps it below 1, evaluates the core in fp32 and applies the
 // per-event constant c0 in fp64.
-template <class P, bool PERM, int D>
+template <class P, bool PERM, bool GRIDPDF, int D>
 __device__ __forceinline__ double eval_weight(const DevConstR<typename P::real>& c, const typename P::real* ec,
                                               double c0, const double (&u)[D]) {
   using T = typename P::real;
   if constexpr (std::is_same<T, double>::value) {
-    return P::template weight_t<PERM>(c, ec, u);
+    return P::template weight_t<PERM, GRIDPDF>(c, ec, u);
   } else {
     T uf[D];
 #pragma unroll
     for (int d = 0; d < D; ++d) uf[d] = fminf((T)u[d], 0x1.fffffep-1f);
-    const double w = (double)P::template weight_t<PERM>(c, ec, uf) * c0;
+    const double w = (double)P::template weight_t<PERM, GRIDPDF>(c, ec, uf) * c0;
     return isfinite(w) ? w : 0.0;
   }
 }
@@ -92,8 +92,8 @@ template <class P, int MODE>
 constexpr int min_blocks() { return (P::kHeavy || MODE != MODE_PLAIN) ? 3 : 0; }   // 0 = no cap
 
 // PERM: sum over c.n_perm jet-parton assignments per point (NEXT-1); the per-event constants are
-// then n_perm blocks of NC.
-template <class P, int MODE, bool PERM>
+// then n_perm blocks of NC.  GRIDPDF: the flavour sum may use interpolated tables (NEXT-3).
+template <class P, int MODE, bool PERM, bool GRIDPDF>
 __global__ void __launch_bounds__(kThreads, min_blocks<P, MODE>())
 integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__ ecs, const double* __restrict__ grids,
                  double* __restrict__ partials, double* __restrict__ hist, int64_t n_points,
@@ -165,7 +165,7 @@ integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__
       if (active) {
         double u[D];
         draw_uniforms<D>(rng, (uint64_t)i, ev_ctr, pass, u);
-        r = P::weight_rt(c, ec, u, !pass_b);              // pass A: number of real roots; pass B: the weight
+        r = P::template weight_rt<GRIDPDF>(c, ec, u, !pass_b);              // pass A: number of real roots; pass B: the weight
       }
       __syncwarp();                                        // the batch has been read before anything is queued
       if (pass_b) {
@@ -189,11 +189,11 @@ integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__
     draw_uniforms<D>(rng, (uint64_t)i, ev_ctr, pass, u);
     double w;
     if (MODE == MODE_PLAIN) {
-      w = eval_weight<P, PERM>(c, ec, c0, u);
+      w = eval_weight<P, PERM, GRIDPDF>(c, ec, c0, u);
     } else {
       int k[D];
       const double jac = vegas_map<D>(edges, B, u, k);
-      w = jac * eval_weight<P, PERM>(c, ec, c0, u);
+      w = jac * eval_weight<P, PERM, GRIDPDF>(c, ec, c0, u);
       if (!isfinite(w)) w = 0.0;
       if (MODE == MODE_ADAPT) {
         const double w2 = live ? w * w : 0.0;
@@ -334,10 +334,10 @@ __global__ void eval_points_kernel(const DevConstR<typename P::real> c, const do
   if (grid) {
     int k[D];
     const double jac = vegas_map<D>(edges, B, u, k);
-    w = jac * eval_weight<P, true>(c, ec, c0, u);
+    w = jac * eval_weight<P, true, true>(c, ec, c0, u);
     if (!isfinite(w)) w = 0.0;
   } else {
-    w = eval_weight<P, true>(c, ec, c0, u);
+    w = eval_weight<P, true, true>(c, ec, c0, u);
   }
   out_w[i] = w;
 }

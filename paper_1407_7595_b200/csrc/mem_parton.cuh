@@ -47,7 +47,7 @@ parton_ttljets_kernel(const DevConst c, const double* __restrict__ mom, int64_t 
   const double shat = x1 * x2 * c.S;
   if (!(4.0 * c.mt2 < shat)) return;                               // reading A9
   const double h = 0.5 * c.sqrt_s, ish = 1.0 / shat, rho = 4.0 * c.mt2 * ish;
-  const TtLumi<double> lum = tt_lumi(c, x1, x2);                   // the same for every assignment
+  const TtLumi<double> lum = tt_lumi<true>(c, x1, x2);                   // the same for every assignment
   const P4 l = p[0], nu = p[1];
   const P4 Wl = l + nu;
   const double swl_m = mdot(Wl, Wl) - c.mW2;

@@ -100,7 +100,7 @@ struct ProcWenu {
     ec[C0] = dt / c.mWGW * c.g4w * c.V_ud2 / 12.0 * c.A_q2 * 4.0 / (8.0 * kPi * kPi * c.S * lE) * 0.5;
   }
 
-  template <bool PERM>
+  template <bool PERM, bool GRIDPDF>
   __device__ static double weight_t(const DevConst& c, const double* ec, const double (&u)[D]) { return weight(c, ec, u); }
 
   __device__ static double weight(const DevConst& c, const double* ec, const double (&u)[D]) {
@@ -199,7 +199,7 @@ struct ProcZbb {
     ec[C0] = vol * sth * kTwoPi4 * (2.0 * c.inv_S) * c.gz4 * c.A_q2 * 4.0 * c.S;
   }
 
-  template <bool PERM>
+  template <bool PERM, bool GRIDPDF>
   __device__ static double weight_t(const DevConst& c, const double* ec, const double (&u)[D]) { return weight(c, ec, u); }
 
   __device__ static double weight(const DevConst& c, const double* ec, const double (&u)[D]) {
@@ -292,7 +292,7 @@ struct ProcTTljetsR {
   }
 
   __device__ static T weight(const DevConstR<T>& c, const T* ec, const T (&u)[D]) {
-    return weight_t<false>(c, ec, u);
+    return weight_t<false, false>(c, ec, u);
   }
 
   // PERM = false: the record's own jet-parton assignment (ec = one block of NC constants).
@@ -300,7 +300,7 @@ struct ProcTTljetsR {
   // blocks.  Everything that depends only on the point -- energy fractions, transfer functions
   // (functions of E / E_jet alone), the neutrino -- is computed once; only the jet momenta, the
   // invariants, the boost and the matrix element are repeated per assignment.
-  template <bool PERM>
+  template <bool PERM, bool GRIDPDF>
   __device__ static T weight_t(const DevConstR<T>& c, const T* ec0, const T (&u)[D]) {
     const T* ec = ec0;
     // ---- S2: jet energy fractions x_j = E_j / E_jet, neutrino rapidity.
@@ -368,7 +368,7 @@ struct ProcTTljetsR {
     const T tt = fma(tau1, tau1, tau2 * tau2);
     const T Mgg = fma(iT, T(1.0) / T(6.0), -T(0.375)) * (tt + rho - T(0.25) * rho * rho * iT);
     const T Mqq = tt + T(0.5) * rho;
-    const TtLumi<T> lum = tt_lumi(c, x1, x2);
+    const TtLumi<T> lum = tt_lumi<GRIDPDF>(c, x1, x2);
     const T prod = fma(lum.gg, Mgg, lum.qq * Mqq);                             // flavour sum incl. the PDFs
     // ---- S5: propagators and decays
     const T t_l = fma(T(0.5), sW, bl_l);                                       // p_t . l
@@ -554,23 +554,24 @@ struct ProcTTdilep {
   }
 
   // PERM = true: NEXT-1, both assignments of the two b jets (ec = 2 blocks of NC constants)
-  template <bool PERM>
+  template <bool PERM, bool GRIDPDF>
   __device__ static double weight_t(const DevConst& c, const double* ec, const double (&u)[D]) {
-    if (!PERM) return weight(c, ec, u);
+    if (!PERM) return weight_rt<GRIDPDF>(c, ec, u, false);
     double w = 0.0;
 #pragma unroll 1
-    for (int k = 0; k < c.n_perm; ++k) w += weight(c, ec + k * NC, u);
+    for (int k = 0; k < c.n_perm; ++k) w += weight_rt<GRIDPDF>(c, ec + k * NC, u, false);
     return w;
   }
 
   __device__ static double weight(const DevConst& c, const double* ec, const double (&u)[D]) {
-    return weight_rt(c, ec, u, false);
+    return weight_rt<false>(c, ec, u, false);
   }
 
   // count_only (a warp-uniform run-time flag, so that the prelude exists once in the kernel: the
   // config-4 kernel is instruction-cache bound, profiles/r01_ncu_config4.md): stop after the resultant
   // quartic and return its number of real roots (0, 2, 4) -- what the lane-compacting loop
   // (mem_kernels.cuh) sorts points by before it runs the per-solution part on full warps.
+  template <bool GRIDPDF>
   __device__ static double weight_rt(const DevConst& c, const double* ec, const double (&u)[D], bool count_only) {
     // ---- S2: jets, transfer functions
     TfAcc<double> tfa{0.0, 1.0};
@@ -699,7 +700,7 @@ struct ProcTTdilep {
       const double tt = fma(tau1, tau1, tau2 * tau2);
       const double Mgg = fma(iT, 1.0 / 6.0, -0.375) * (tt + rho - 0.25 * rho * rho * iT);
       const double Mqq = tt + 0.5 * rho;
-      const TtLumi<double> lum = tt_lumi(c, x1, x2);
+      const TtLumi<double> lum = tt_lumi<GRIDPDF>(c, x1, x2);
       const double ws = fma(lum.gg, Mgg, lum.qq * Mqq) * ish * rcp_fast(xz);  // flavour sum incl. the PDFs
       if (isfinite(ws)) sum += ws;
     }
