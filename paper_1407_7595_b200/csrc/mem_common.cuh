@@ -190,11 +190,29 @@ template <typename T> struct TfAcc { T esum, fac; };
 // per-event constants, the overall constant C0 and the sums stay in fp64).  MUFU-based
 // reciprocal / rsqrt / exp2; no --use_fast_math anywhere, these are chosen per call site.
 // ---------------------------------------------------------------------------------------
-__device__ __forceinline__ float rcp_fast(float x) { return __frcp_rn(x); }
+__device__ __forceinline__ float rcp_fast(float x) {
+  float y;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));      // one MUFU, 1 ulp: ample for the 1e-4 bar
+  return y;
+}
+// tan for the Breit-Wigner map in fp32: same scheme as tan_bw_n (no range reduction beyond pi/2 - |t|),
+// degree-9 / degree-8 polynomials (Taylor coefficients; the remainders are below 2e-8 on |r| <= pi/4)
+__device__ __forceinline__ float tan_bw(float t) {
+  const float a = fabsf(t);
+  const bool big = a > 0.78539816f;
+  const float r = big ? (1.57079637f - a) - 4.37113883e-8f : a, z = r * r;
+  float ps = 2.75573192e-6f, pc = 2.48015873e-5f;
+  ps = fmaf(ps, z, -1.98412698e-4f); pc = fmaf(pc, z, -1.38888889e-3f);
+  ps = fmaf(ps, z, 8.33333333e-3f);  pc = fmaf(pc, z, 4.16666667e-2f);
+  ps = fmaf(ps, z, -1.66666667e-1f);
+  const float sn = fmaf(r * z, ps, r), cs = fmaf(z * z, pc, fmaf(-0.5f, z, 1.0f));
+  const float q = (big ? cs : sn) * rcp_fast(big ? sn : cs);
+  return copysignf(q, t);
+}
 __device__ __forceinline__ double m_exp(double x) { return exp(x); }
 __device__ __forceinline__ float m_exp(float x) { return __expf(x); }
 __device__ __forceinline__ double m_tan(double x) { return tan_bw(x); }
-__device__ __forceinline__ float m_tan(float x) { return tanf(x); }
+__device__ __forceinline__ float m_tan(float x) { return tan_bw(x); }
 __device__ __forceinline__ double m_rsqrt(double x) { return rsqrt(x); }
 __device__ __forceinline__ float m_rsqrt(float x) { return rsqrtf(x); }
 
