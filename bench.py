@@ -35,17 +35,17 @@ SEED = 20140729
 FP64_PER_CALL = {           # key = (config, jet-parton assignments per point)
     (1, 1): {"dfma": 87.3, "dmul": 47.0, "dadd": 17.9},
     (2, 1): {"dfma": 104.0, "dmul": 34.0, "dadd": 15.2},
-    (3, 1): {"dfma": 189.9, "dmul": 89.2, "dadd": 44.3},
-    (3, 24): {"dfma": 1438.9, "dmul": 1323.5, "dadd": 617.6},
-    (4, 1): {"dfma": 221.3, "dmul": 77.0, "dadd": 55.0},
-    (4, 2): {"dfma": 337.3, "dmul": 119.7, "dadd": 81.9},
-    (5, 1): {"dfma": 197.0, "dmul": 108.1, "dadd": 60.6},
+    (3, 1): {"dfma": 196.0, "dmul": 90.0, "dadd": 41.2},
+    (3, 24): {"dfma": 1597.0, "dmul": 1335.0, "dadd": 551.2},
+    (4, 1): {"dfma": 255.0, "dmul": 80.5, "dadd": 57.4},
+    (4, 2): {"dfma": 327.2, "dmul": 120.1, "dadd": 79.2},
+    (5, 1): {"dfma": 202.0, "dmul": 109.0, "dadd": 55.2},
 }
 # fp32 variant of config 3 (reading A15): executed FFMA / FMUL / FADD per call (same ncu pass)
-FP32_PER_CALL = {3: {"ffma": 82.7, "fmul": 91.3, "fadd": 33.7}, 5: {"ffma": 82.7, "fmul": 91.3, "fadd": 33.7}}
+FP32_PER_CALL = {3: {"ffma": 75.0, "fmul": 93.1, "fadd": 27.1}, 5: {"ffma": 75.0, "fmul": 93.1, "fadd": 27.1}}
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant launch at full size, from an ncu metric pass
 # of the same command (profiles/r01_ncu_config3.md); key = (config, events, points/event, assignments, precision)
-TRAFFIC_BYTES = {(3, 4096, 1 << 20, 1, 64): 1571584}
+TRAFFIC_BYTES = {(3, 4096, 1 << 20, 1, 64): 1821696}
 NOMINAL_FP64_FMA_PER_CLK_PER_SM = 64      # 4 SMSPs x 16 lanes; confirmed by the microbenchmark
 VEGAS_ITERS, VEGAS_POINTS = 5, 1 << 17    # BASELINE.json:configs[4]
 
