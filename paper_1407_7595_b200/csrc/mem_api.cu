@@ -251,12 +251,22 @@ mem_status launch_pass(mem_handle* h, int64_t n_events, int64_t n_points, int64_
   return MEM_OK;
 }
 
+// Points per (event, chunk) block of the pass that produces the outputs: kChunk, or less for short
+// integrations so that a few events still fill the GPU (config 1: 64 events x 2^16 points).  A
+// function of n_points alone -- never of the number of events -- so that the reduction order, and
+// with it every bit of the result, is the same however the event list is sharded.
+int64_t chunk_for(int64_t n_points) {
+  int64_t c = kChunk;
+  while (c > 1024 && c * 16 > n_points) c >>= 1;
+  return c;
+}
+
 // the pass that produces the outputs, bracketed by the handle's events
 template <class P, int MODE>
 mem_status launch_timed_pass(mem_handle* h, int64_t n_events, int64_t n_points, int n_chunks, uint64_t seed,
                              uint32_t pass, cudaStream_t st) {
   CUDA_TRY(cudaEventRecord(h->ev_begin, st));
-  mem_status s = launch_pass<P, MODE>(h, n_events, n_points, kChunk, n_chunks, seed, pass, st);
+  mem_status s = launch_pass<P, MODE>(h, n_events, n_points, chunk_for(n_points), n_chunks, seed, pass, st);
   if (s != MEM_OK) return s;
   CUDA_TRY(cudaEventRecord(h->ev_end, st));
   h->last_evals = n_events * n_points;
@@ -268,7 +278,8 @@ mem_status integrate_impl(mem_handle* h, const double* events, int64_t n_events,
                           double* out_p, double* out_err, cudaStream_t st) {
   mem_status s = launch_prepare<P>(h, events, n_events, st);
   if (s != MEM_OK) return s;
-  const int n_chunks = (int)((n_points + kChunk - 1) / kChunk);
+  const int64_t chunk = chunk_for(n_points);
+  const int n_chunks = (int)((n_points + chunk - 1) / chunk);
   s = ensure(h->partials, (size_t)n_events * n_chunks * 2 * sizeof(double), st);
   if (s != MEM_OK) return s;
   const mem_params& p = h->params;
