@@ -287,7 +287,7 @@ mem_status integrate_impl(mem_handle* h, const double* events, int64_t n_events,
     const int D = P::D, B = p.vegas_bins;
     // adaptation passes: at most kMaxAdaptChunks blocks per event, chunk a multiple of kThreads
     int64_t a_chunk = (p.vegas_points + kMaxAdaptChunks - 1) / kMaxAdaptChunks;
-    if (a_chunk < kChunk) a_chunk = kChunk;
+    if (a_chunk < chunk_for(p.vegas_points)) a_chunk = chunk_for(p.vegas_points);
     a_chunk = (a_chunk + kThreads - 1) / kThreads * kThreads;
     const int a_chunks = (int)((p.vegas_points + a_chunk - 1) / a_chunk);
     s = ensure(h->grids, (size_t)n_events * D * (B + 1) * sizeof(double), st);
