@@ -165,7 +165,7 @@ integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__
       if (active) {
         double u[D];
         draw_uniforms<D>(rng, (uint64_t)i, ev_ctr, pass, u);
-        r = P::template weight_rt<GRIDPDF>(c, ec, u, !pass_b);              // pass A: number of real roots; pass B: the weight
+        r = P::template weight_rt<GRIDPDF, true>(c, ec, u, !pass_b);              // pass A: number of real roots; pass B: the weight
       }
       __syncwarp();                                        // the batch has been read before anything is queued
       if (pass_b) {

@@ -153,7 +153,7 @@ __device__ inline void jet_prepare(const DevConst& c, double Ej, double eta, dou
 template <typename T>
 __device__ __forceinline__ JetR<T> jet_point(const DevConstR<T>& c, const T* o, T u, TfAcc<T>& tf) {
   const T x = fma(c.dr, u, c.rlo);
-  tf_accum(c, rcp_fast(x), tf);
+  tf_accum<true>(c, rcp_fast(x), tf);
   JetR<T> j;
   j.E = fma(o[1], u, o[0]);
   j.x = j.E * o[2]; j.y = j.E * o[3]; j.z = j.E * o[4];
@@ -205,7 +205,7 @@ struct ProcZbb {
   __device__ static double weight(const DevConst& c, const double* ec, const double (&u)[D]) {
     TfAcc<double> tfa{0.0, 1.0};
     const Jet p1 = jet_point(c, ec + J0, u[0], tfa), p2 = jet_point(c, ec + J1, u[1], tfa);
-    const double tf = tfa.fac * exp(-tfa.esum);
+    const double tf = tfa.fac * exp_tab(-tfa.esum);
     // O7 without the cancellation in 1 - beta^2 (nearly collinear jets): with P = p1 + p2,
     //   P_E'^2 = P_E^2 - P_T^2 = p1z^2 + p2z^2 + 2 E1 E2 (1 - n1T.n2T)
     //   E_i'   = gamma (E_i - beta.p_iT) = (p_iz^2 + E1 E2 (1 - n1T.n2T)) / P_E'
@@ -556,29 +556,31 @@ struct ProcTTdilep {
   // PERM = true: NEXT-1, both assignments of the two b jets (ec = 2 blocks of NC constants)
   template <bool PERM, bool GRIDPDF>
   __device__ static double weight_t(const DevConst& c, const double* ec, const double (&u)[D]) {
-    if (!PERM) return weight_rt<GRIDPDF>(c, ec, u, false);
+    if (!PERM) return weight_rt<GRIDPDF, true>(c, ec, u, false);
     double w = 0.0;
 #pragma unroll 1
-    for (int k = 0; k < c.n_perm; ++k) w += weight_rt<GRIDPDF>(c, ec + k * NC, u, false);
+    for (int k = 0; k < c.n_perm; ++k) w += weight_rt<GRIDPDF, false>(c, ec + k * NC, u, false);
     return w;
   }
 
   __device__ static double weight(const DevConst& c, const double* ec, const double (&u)[D]) {
-    return weight_rt<false>(c, ec, u, false);
+    return weight_rt<false, true>(c, ec, u, false);
   }
 
   // count_only (a warp-uniform run-time flag, so that the prelude exists once in the kernel: the
   // config-4 kernel is instruction-cache bound, profiles/r01_ncu_config4.md): stop after the resultant
   // quartic and return its number of real roots (0, 2, 4) -- what the lane-compacting loop
   // (mem_kernels.cuh) sorts points by before it runs the per-solution part on full warps.
-  template <bool GRIDPDF>
+  // TAB: table-driven exp (+5.8 % in the single-assignment kernel; the two-assignment kernel, tighter on
+  // registers, loses 9 % with it and keeps libdevice's exp)
+  template <bool GRIDPDF, bool TAB>
   __device__ static double weight_rt(const DevConst& c, const double* ec, const double (&u)[D], bool count_only) {
     // ---- S2: jets, transfer functions
     TfAcc<double> tfa{0.0, 1.0};
     const double xb0 = fma(c.dr, u[0], c.rlo), xb1 = fma(c.dr, u[1], c.rlo);
     const double ixb0 = rcp_fast(xb0), ixb1 = rcp_fast(xb1);
-    tf_accum(c, ixb0, tfa);
-    tf_accum(c, ixb1, tfa);
+    tf_accum<TAB>(c, ixb0, tfa);
+    tf_accum<TAB>(c, ixb1, tfa);
     const double Eb0 = fma(ec[J0 + 1], u[0], ec[J0]), Eb1 = fma(ec[J1 + 1], u[1], ec[J1]);
     const double iEb0 = ixb0 * ec[IEJ0], iEb1 = ixb1 * ec[IEJ1];
     // ---- S2: the four mapped masses, s_k - m_k^2 = m Gam tan t_k (O6)
@@ -707,7 +709,8 @@ struct ProcTTdilep {
     // ---- S5: decays (p_t.p_l)(p_b.p_nu) per side; S6: MET TF; S7
     const double dec = fma(Eb0, ec[S0 + ELK], 0.5 * sW0) * (Eb0 * hD0) * fma(Eb1, ec[S1 + ELK], 0.5 * sW1) * (Eb1 * hD1);
     // jets' Gaussians and the MET Gaussian share one exponential
-    const double tf_tmet = tfa.fac * exp(fma(ec[MEXP], fma(g6, g6, g7 * g7), -tfa.esum));
+    const double targ = fma(ec[MEXP], fma(g6, g6, g7 * g7), -tfa.esum);
+    const double tf_tmet = tfa.fac * (TAB ? exp_tab(targ) : exp(targ));
     const double w = ec[C0] * tf_tmet * dec * (iEb0 * iEb1) * sum;
     return isfinite(w) ? w : 0.0;
   }
