@@ -33,12 +33,12 @@ SEED = 20140729
 # r01_fp64_counts.md): smsp__sass_thread_inst_executed_op_{dfma,dmul,dadd}_pred_on.sum / points.
 # flop = 2 DFMA + DMUL + DADD.  Key = config; config 5's dominant kernel is the grid-mapped final pass.
 FP64_PER_CALL = {           # key = (config, jet-parton assignments per point)
-    (1, 1): {"dfma": 87.3, "dmul": 47.0, "dadd": 17.9},
-    (2, 1): {"dfma": 104.0, "dmul": 34.0, "dadd": 15.2},
+    (1, 1): {"dfma": 87.3, "dmul": 47.0, "dadd": 18.4},
+    (2, 1): {"dfma": 86.0, "dmul": 37.0, "dadd": 15.6},
     (3, 1): {"dfma": 196.0, "dmul": 90.0, "dadd": 41.2},
     (3, 24): {"dfma": 1597.0, "dmul": 1335.0, "dadd": 551.2},
-    (4, 1): {"dfma": 255.0, "dmul": 80.5, "dadd": 57.4},
-    (4, 2): {"dfma": 327.2, "dmul": 120.1, "dadd": 79.2},
+    (4, 1): {"dfma": 241.0, "dmul": 82.9, "dadd": 57.9},
+    (4, 2): {"dfma": 327.2, "dmul": 120.2, "dadd": 79.8},
     (5, 1): {"dfma": 202.0, "dmul": 109.0, "dadd": 55.2},
 }
 # fp32 variant of config 3 (reading A15): executed FFMA / FMUL / FADD per call (same ncu pass)
