@@ -293,6 +293,9 @@ __device__ __forceinline__ TtLumi<T> tt_lumi(const DevConstR<T>& c, T x1, T x2) 
   return {(T)gg, (T)(qq * (2.0 * 4.0 / 9.0))};
 }
 
+template <bool TAB> __device__ __forceinline__ double x_exp(double x) { return TAB ? exp_tab(x) : exp(x); }
+template <bool TAB> __device__ __forceinline__ float x_exp(float x) { return m_exp(x); }
+
 // TAB: exp_tab instead of libdevice's exp (fp64 only).  Measured: configs 2 and 4 gain 5.7 % and 5.8 %;
 // config 3's time does not move (its plain kernel sits on the mixed-operand FP64 ceiling either way) while
 // its executed flop count, hence the reported roofline fraction, would drop: it keeps libdevice's exp.

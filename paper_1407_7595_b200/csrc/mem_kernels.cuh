@@ -28,17 +28,17 @@ __global__ void prepare_kernel(const DevConst c, const double* __restrict__ ev, 
 // the integrand at the unit-cube point u.  fp64 processes take u as it is; the fp32 variant
 // (reading A15) rounds u to fp32, clamps it below 1, evaluates the core in fp32 and applies the
 // per-event constant c0 in fp64.
-template <class P, bool PERM, bool GRIDPDF, int D>
+template <class P, bool PERM, bool GRIDPDF, bool TAB, int D>
 __device__ __forceinline__ double eval_weight(const DevConstR<typename P::real>& c, const typename P::real* ec,
                                               double c0, const double (&u)[D]) {
   using T = typename P::real;
   if constexpr (std::is_same<T, double>::value) {
-    return P::template weight_t<PERM, GRIDPDF>(c, ec, u);
+    return P::template weight_t<PERM, GRIDPDF, TAB>(c, ec, u);
   } else {
     T uf[D];
 #pragma unroll
     for (int d = 0; d < D; ++d) uf[d] = fminf((T)u[d], 0x1.fffffep-1f);
-    const double w = (double)P::template weight_t<PERM, GRIDPDF>(c, ec, uf) * c0;
+    const double w = (double)P::template weight_t<PERM, GRIDPDF, TAB>(c, ec, uf) * c0;
     return isfinite(w) ? w : 0.0;
   }
 }
@@ -189,11 +189,11 @@ integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__
     draw_uniforms<D>(rng, (uint64_t)i, ev_ctr, pass, u);
     double w;
     if (MODE == MODE_PLAIN) {
-      w = eval_weight<P, PERM, GRIDPDF>(c, ec, c0, u);
+      w = eval_weight<P, PERM, GRIDPDF, MODE != MODE_PLAIN>(c, ec, c0, u);
     } else {
       int k[D];
       const double jac = vegas_map<D>(edges, B, u, k);
-      w = jac * eval_weight<P, PERM, GRIDPDF>(c, ec, c0, u);
+      w = jac * eval_weight<P, PERM, GRIDPDF, MODE != MODE_PLAIN>(c, ec, c0, u);
       if (!isfinite(w)) w = 0.0;
       if (MODE == MODE_ADAPT) {
         const double w2 = live ? w * w : 0.0;
@@ -334,10 +334,10 @@ __global__ void eval_points_kernel(const DevConstR<typename P::real> c, const do
   if (grid) {
     int k[D];
     const double jac = vegas_map<D>(edges, B, u, k);
-    w = jac * eval_weight<P, true, true>(c, ec, c0, u);
+    w = jac * eval_weight<P, true, true, false>(c, ec, c0, u);
     if (!isfinite(w)) w = 0.0;
   } else {
-    w = eval_weight<P, true, true>(c, ec, c0, u);
+    w = eval_weight<P, true, true, false>(c, ec, c0, u);
   }
   out_w[i] = w;
 }

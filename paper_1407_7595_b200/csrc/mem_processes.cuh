@@ -100,7 +100,7 @@ struct ProcWenu {
     ec[C0] = dt / c.mWGW * c.g4w * c.V_ud2 / 12.0 * c.A_q2 * 4.0 / (8.0 * kPi * kPi * c.S * lE) * 0.5;
   }
 
-  template <bool PERM, bool GRIDPDF>
+  template <bool PERM, bool GRIDPDF, bool TAB>
   __device__ static double weight_t(const DevConst& c, const double* ec, const double (&u)[D]) { return weight(c, ec, u); }
 
   __device__ static double weight(const DevConst& c, const double* ec, const double (&u)[D]) {
@@ -199,7 +199,7 @@ struct ProcZbb {
     ec[C0] = vol * sth * kTwoPi4 * (2.0 * c.inv_S) * c.gz4 * c.A_q2 * 4.0 * c.S;
   }
 
-  template <bool PERM, bool GRIDPDF>
+  template <bool PERM, bool GRIDPDF, bool TAB>
   __device__ static double weight_t(const DevConst& c, const double* ec, const double (&u)[D]) { return weight(c, ec, u); }
 
   __device__ static double weight(const DevConst& c, const double* ec, const double (&u)[D]) {
@@ -292,7 +292,7 @@ struct ProcTTljetsR {
   }
 
   __device__ static T weight(const DevConstR<T>& c, const T* ec, const T (&u)[D]) {
-    return weight_t<false, false>(c, ec, u);
+    return weight_t<false, false, false>(c, ec, u);
   }
 
   // PERM = false: the record's own jet-parton assignment (ec = one block of NC constants).
@@ -300,7 +300,9 @@ struct ProcTTljetsR {
   // blocks.  Everything that depends only on the point -- energy fractions, transfer functions
   // (functions of E / E_jet alone), the neutrino -- is computed once; only the jet momenta, the
   // invariants, the boost and the matrix element are repeated per assignment.
-  template <bool PERM, bool GRIDPDF>
+  // TAB: table-driven exp (fp64).  The plain kernel does not gain from it and keeps
+  // libdevice's exp; the VEGAS passes gain 3 %.
+  template <bool PERM, bool GRIDPDF, bool TAB>
   __device__ static T weight_t(const DevConstR<T>& c, const T* ec0, const T (&u)[D]) {
     const T* ec = ec0;
     // ---- S2: jet energy fractions x_j = E_j / E_jet, neutrino rapidity.
@@ -308,7 +310,7 @@ struct ProcTTljetsR {
     const T x0 = fma(c.dr, u[0], c.rlo), x1j = fma(c.dr, u[1], c.rlo), x2j = fma(c.dr, u[2], c.rlo), x3 = fma(c.dr, u[3], c.rlo);
     const T H = c.nu_eta_max;
     const T eta_nu = fma(T(2.0) * H, u[4], -H);
-    const T en = m_exp(eta_nu);
+    const T en = x_exp<TAB>(eta_nu);
     const T g = en * ec[ELI];
     const T gm1 = g - T(1.0);
     const T denp = ec[LPT2] * fma(T(0.5) * gm1, gm1, ec[OMC] * g);
@@ -322,8 +324,8 @@ struct ProcTTljetsR {
     const T ix0 = i01 * x1j, ix1 = i01 * x0, ix2 = i23 * x3, ix3 = i23 * x2j;
     // ---- S6: transfer functions (one exponential per jet and one for the sum, see tf_accum)
     TfAcc<T> tfa{T(0), T(1)};
-    tf_accum(c, ix0, tfa); tf_accum(c, ix1, tfa); tf_accum(c, ix2, tfa); tf_accum(c, ix3, tfa);
-    const T tf = tfa.fac * m_exp(-tfa.esum);
+    tf_accum<TAB>(c, ix0, tfa); tf_accum<TAB>(c, ix1, tfa); tf_accum<TAB>(c, ix2, tfa); tf_accum<TAB>(c, ix3, tfa);
+    const T tf = tfa.fac * x_exp<TAB>(-tfa.esum);
     // ---- S2: neutrino from the mapped leptonic W mass
     const T t = fma(c.tW_dt, u[5], c.tW_lo);
     const T smm = c.mWGW * m_tan(t);
@@ -554,7 +556,7 @@ struct ProcTTdilep {
   }
 
   // PERM = true: NEXT-1, both assignments of the two b jets (ec = 2 blocks of NC constants)
-  template <bool PERM, bool GRIDPDF>
+  template <bool PERM, bool GRIDPDF, bool TAB_UNUSED>
   __device__ static double weight_t(const DevConst& c, const double* ec, const double (&u)[D]) {
     if (!PERM) return weight_rt<GRIDPDF, true>(c, ec, u, false);
     double w = 0.0;
