@@ -84,7 +84,7 @@ __device__ __forceinline__ void warp_hist_add(double* wh, int k, double v) {
 // sums go registers -> warp shuffle -> shared -> partials[event][chunk] in a fixed order.
 // MODE_GRID/ADAPT: grids = [n_events][D][B+1].  MODE_ADAPT also writes the block's histogram
 // of w^2 to hist[event][chunk][D][B].
-// Resident blocks per SM the register allocation aims at (measured on B200, profiles/r01_variants.md):
+// Resident blocks per SM the register allocation aims at (measured on B200):
 // the plain config-1/2/3 kernels (no register cap: 64/50/80 registers, no spills) are bound by FP64 issue and
 // gain nothing from more warps; the divergent config-4 kernel and the VEGAS passes (shuffle/match
 // latency) gain 43 % / 7 % from 3 blocks at 80 registers.
