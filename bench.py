@@ -73,6 +73,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--parton", action="store_true",
                     help="NEXT-2 parton-level mode: ME evaluations of --events configurations (default 10^5)")
+    ap.add_argument("--microbench", action="store_true",
+                    help="FP64 issue microbenchmarks behind the roofline discussion (mem_measure_fp64_rate)")
     ap.add_argument("--sweep", action="store_true",
                     help="config-5 sweep of BASELINE.json:configs[4]: events x final points, one JSON line")
     return ap.parse_args()
@@ -491,9 +493,25 @@ def run_parton(args):
     print(json.dumps(line), flush=True)
 
 
+def run_microbench(args):
+    import torch
+
+    import paper_1407_7595_b200 as mem
+    torch.cuda.set_device(0)
+    names = ["DFMA, two uniform operands (nominal peak)", "DFMA, three register operands",
+             "5 DFMA : 2 DMUL : 1 DADD, shuffled register operands", "8 DFMA (uniform) + 8 integer instructions",
+             "8 DFMA (uniform) + 16 integer instructions", "DMUL, two register operands", "DADD, two register operands"]
+    res = [{"kind": k, "what": n, "tera_fp64_inst_per_s": mem.mem_measure_fp64_rate(k, 5) / 2.0} for k, n in enumerate(names)]
+    for r in res:
+        r["frac_of_kind0"] = r["tera_fp64_inst_per_s"] / res[0]["tera_fp64_inst_per_s"]
+    print(json.dumps({"metric": "fp64_instruction_rate", "unit": "T inst/s", "n_gpus": 1, "microbench": res}), flush=True)
+
+
 def main():
     args = parse_args()
-    if args.parton:
+    if args.microbench:
+        run_microbench(args)
+    elif args.parton:
         run_parton(args)
     elif args.sweep:
         run_sweep(args)

@@ -179,6 +179,14 @@ mem_status mem_measure_fp64_peak(int32_t repeats, double* tflops, void* cuda_str
  * above on B200.  Reported beside the roofline as the ceiling of register-operand code. */
 mem_status mem_measure_fp64_peak_rrr(int32_t repeats, double* tflops, void* cuda_stream);
 
+/* The family of FP64 issue microbenchmarks behind the roofline discussion.  Every kind runs
+ * 8 independent FP64 instruction chains per thread; *tflops = 2 * FP64 instructions / second / 1e12 (i.e. an FMA
+ * counts 2 in every kind, so the figures compare instruction rates).  kind 0: DFMA with two uniform operands (=
+ * mem_measure_fp64_peak); 1: DFMA with three register operands (= ..._rrr); 2: 5 DFMA : 2 DMUL : 1 DADD with
+ * shuffled register operands; 3 / 4: kind 0 plus 8 / 16 independent integer instructions per 8 DFMAs; 5: DMUL and
+ * 6: DADD with two register operands. */
+mem_status mem_measure_fp64_rate(int32_t kind, int32_t repeats, double* tflops, void* cuda_stream);
+
 /* Thread-local description of the last error on this thread ("" if none). */
 const char* mem_last_error(void);
 

@@ -20,7 +20,7 @@ MEM_PROC_W_ENU, MEM_PROC_Z_BB, MEM_PROC_TT_LJETS, MEM_PROC_TT_DILEP = 1, 2, 3, 4
 EXPORTS = ("mem_params_default", "mem_event_fields", "mem_n_dims", "mem_create", "mem_destroy",
            "mem_set_event_offset", "mem_integrate", "mem_integrate_host", "mem_eval_points",
            "mem_eval_parton", "mem_set_pdf_grid", "mem_get_grid", "mem_launch_count", "mem_last_error", "mem_last_pass_ms", "mem_measure_fp64_peak",
-           "mem_measure_fp64_peak_rrr")
+           "mem_measure_fp64_peak_rrr", "mem_measure_fp64_rate")
 
 
 class mem_params(C.Structure):
@@ -73,6 +73,7 @@ def lib():
         L.mem_last_pass_ms.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
         L.mem_measure_fp64_peak.argtypes = [C.c_int32, C.POINTER(C.c_double), vp]
         L.mem_measure_fp64_peak_rrr.argtypes = [C.c_int32, C.POINTER(C.c_double), vp]
+        L.mem_measure_fp64_rate.argtypes = [C.c_int32, C.c_int32, C.POINTER(C.c_double), vp]
         L.mem_last_error.argtypes = []
         L.mem_last_error.restype = C.c_char_p
         _lib = L
@@ -138,6 +139,13 @@ def mem_measure_fp64_peak_rrr(repeats: int = 5, stream=None) -> float:
     """The same with three register operands per DFMA (what generic fused multiply-adds sustain), TFLOP/s."""
     t = C.c_double()
     _check(lib().mem_measure_fp64_peak_rrr(int(repeats), C.byref(t), _stream_ptr(stream)))
+    return t.value
+
+
+def mem_measure_fp64_rate(kind: int, repeats: int = 5, stream=None) -> float:
+    """FP64 issue microbenchmarks (include/mem.h): 2 x FP64 instructions/s/1e12 for instruction mix `kind`."""
+    t = C.c_double()
+    _check(lib().mem_measure_fp64_rate(int(kind), int(repeats), C.byref(t), _stream_ptr(stream)))
     return t.value
 
 

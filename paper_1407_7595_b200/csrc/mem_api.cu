@@ -430,8 +430,8 @@ mem_status mem_last_pass_ms(mem_handle* h, double* ms, int64_t* evals) {
   return MEM_OK;
 }
 
-static mem_status measure_fp64(bool rrr, int32_t repeats, double* tflops, void* cuda_stream) {
-  if (!tflops || repeats < 1) return fail(MEM_ERR_INVALID_ARG, "tflops is NULL or repeats < 1");
+static mem_status measure_fp64(int kind, int32_t repeats, double* tflops, void* cuda_stream) {
+  if (!tflops || repeats < 1 || kind < 0 || kind > 6) return fail(MEM_ERR_INVALID_ARG, "tflops is NULL, repeats < 1 or kind outside 0..6");
   cudaStream_t st = (cudaStream_t)cuda_stream;
   int dev = 0, sms = 0;
   CUDA_TRY(cudaGetDevice(&dev));
@@ -445,8 +445,15 @@ static mem_status measure_fp64(bool rrr, int32_t repeats, double* tflops, void* 
   double best = 0.0;
   for (int r = 0; r < repeats + 1; ++r) {                  // first launch is the warm-up
     cudaEventRecord(a, st);
-    if (rrr) fp64_peak_kernel<true><<<blocks, threads, 0, st>>>(sink, 0.999999, 1e-9);
-    else fp64_peak_kernel<false><<<blocks, threads, 0, st>>>(sink, 0.999999, 1e-9);
+    switch (kind) {
+      case 0: fp64_peak_kernel<0><<<blocks, threads, 0, st>>>(sink, 0.999999, 1e-9, 0x9e3779b9u); break;
+      case 1: fp64_peak_kernel<1><<<blocks, threads, 0, st>>>(sink, 0.999999, 1e-9, 0x9e3779b9u); break;
+      case 2: fp64_peak_kernel<2><<<blocks, threads, 0, st>>>(sink, 0.999999, 1e-9, 0x9e3779b9u); break;
+      case 3: fp64_peak_kernel<3><<<blocks, threads, 0, st>>>(sink, 0.999999, 1e-9, 0x9e3779b9u); break;
+      case 4: fp64_peak_kernel<4><<<blocks, threads, 0, st>>>(sink, 0.999999, 1e-9, 0x9e3779b9u); break;
+      case 5: fp64_peak_kernel<5><<<blocks, threads, 0, st>>>(sink, 0.999999, 1e-9, 0x9e3779b9u); break;
+      default: fp64_peak_kernel<6><<<blocks, threads, 0, st>>>(sink, 0.999999, 1e-9, 0x9e3779b9u); break;
+    }
     cudaEventRecord(b, st);
     cudaError_t e = cudaEventSynchronize(b);
     float ms = 0.f;
@@ -464,11 +471,15 @@ static mem_status measure_fp64(bool rrr, int32_t repeats, double* tflops, void* 
 }
 
 mem_status mem_measure_fp64_peak(int32_t repeats, double* tflops, void* cuda_stream) {
-  return measure_fp64(false, repeats, tflops, cuda_stream);
+  return measure_fp64(0, repeats, tflops, cuda_stream);
 }
 
 mem_status mem_measure_fp64_peak_rrr(int32_t repeats, double* tflops, void* cuda_stream) {
-  return measure_fp64(true, repeats, tflops, cuda_stream);
+  return measure_fp64(1, repeats, tflops, cuda_stream);
+}
+
+mem_status mem_measure_fp64_rate(int32_t kind, int32_t repeats, double* tflops, void* cuda_stream) {
+  return measure_fp64(kind, repeats, tflops, cuda_stream);
 }
 
 mem_status mem_integrate(mem_handle* h, const double* events, int64_t n_events, int64_t n_points, uint64_t seed,
