@@ -263,3 +263,14 @@ def test_full_size_vegas_sampled_output(mem):
     po, eo = oracle.vegas_integrate(proc, p, ev[:, e:e + 1], n_points, SEED, event_offset=e)
     assert abs(pg[e] - po[0]) <= TOL_EVENT * abs(po[0])
     assert abs(eg[e] - eo[0]) <= 1e-8 * abs(eo[0])
+
+
+def test_fp64_microbenchmarks(mem):
+    """the roofline denominators are measured, not assumed: plausible values, the documented ordering, argument checks"""
+    peak = mem.mem_measure_fp64_peak(2)
+    rrr = mem.mem_measure_fp64_peak_rrr(2)
+    assert 20.0 < peak < 45.0 and 10.0 < rrr < peak
+    assert abs(mem.mem_measure_fp64_rate(0, 2) - peak) < 0.1 * peak
+    assert mem.mem_measure_fp64_rate(4, 2) < mem.mem_measure_fp64_rate(3, 2) < peak * 1.02
+    with pytest.raises(mem.MemError):
+        mem.mem_measure_fp64_rate(7, 2)
