@@ -105,7 +105,9 @@ mem_status mem_set_event_offset(mem_handle* h, uint64_t first_event);
  * out_p, out_err : device, float64 [n_events]; overwritten
  * cuda_stream : a cudaStream_t (NULL = legacy default stream).  All work is
  *   enqueued on it and the call returns without synchronising.  The handle's
- *   workspace grows on demand (a growth step synchronises that stream).
+ *   workspace grows on demand (a growth step synchronises that stream); once a call
+ *   of the same size has run, further calls allocate nothing and may be captured
+ *   into a CUDA graph on a capturing stream and replayed.
  * n_events == 0 is MEM_OK with no launch; n_points < 2 is MEM_ERR_INVALID_ARG; so is a call made while
  * another CUDA device than the handle's is current.
  * Kinematically forbidden or non-finite points contribute w = 0 and still count in N. */

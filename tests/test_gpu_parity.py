@@ -274,3 +274,27 @@ def test_fp64_microbenchmarks(mem):
     assert mem.mem_measure_fp64_rate(4, 2) < mem.mem_measure_fp64_rate(3, 2) < peak * 1.02
     with pytest.raises(mem.MemError):
         mem.mem_measure_fp64_rate(7, 2)
+
+
+def test_cuda_graph_capture_and_replay(mem):
+    """mem_integrate only enqueues work on the caller's stream, so once a first call has sized the workspace the
+    whole pass sequence (here VEGAS: grid init, 2 x (adapt, refine), final, finalize) can be captured into a CUDA
+    graph and replayed; the replay reproduces the eager result bit for bit"""
+    import torch
+    proc = 3
+    ev = _dev(wl.make_events(proc, 48, seed=5))
+    out_p = torch.empty(48, dtype=torch.float64, device="cuda")
+    out_e = torch.empty_like(out_p)
+    with mem.Integrator(proc, vegas_iters=2, vegas_points=4096) as it:
+        s = torch.cuda.Stream()
+        with torch.cuda.stream(s):
+            it.integrate(ev, 8192, SEED, out_p=out_p, out_err=out_e)
+        s.synchronize()
+        ref_p, ref_e = out_p.clone(), out_e.clone()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            it.integrate(ev, 8192, SEED, out_p=out_p, out_err=out_e)
+        out_p.zero_(); out_e.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(out_p, ref_p) and torch.equal(out_e, ref_e)
