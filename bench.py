@@ -42,7 +42,7 @@ FP64_PER_CALL = {           # key = (config, jet-parton assignments per point)
     (5, 1): {"dfma": 166.0, "dmul": 115.1, "dadd": 55.7},
 }
 # fp32 variant of config 3 (reading A15): executed FFMA / FMUL / FADD per call (same ncu pass)
-FP32_PER_CALL = {3: {"ffma": 75.0, "fmul": 93.1, "fadd": 27.1}, 5: {"ffma": 75.0, "fmul": 93.1, "fadd": 27.1}}
+FP32_PER_CALL = {3: {"ffma": 81.0, "fmul": 93.3, "fadd": 27.4}, 5: {"ffma": 81.0, "fmul": 93.3, "fadd": 27.4}}
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant launch at full size, from an ncu metric pass
 # of the same command (profiles/r01_ncu_config3.md); key = (config, events, points/event, assignments, precision)
 TRAFFIC_BYTES = {(3, 4096, 1 << 20, 1, 64): 1821696}

@@ -102,6 +102,22 @@ __device__ __forceinline__ void draw_uniforms(const Philox& rng, uint64_t point,
   }
 }
 
+// fp32 variant (reading A15), plain Monte Carlo: single-precision uniforms straight from the same Philox words,
+// u = (k + 1/2) 2^-23 with k the 23 leading bits of the first word of the dimension's pair -- exact in fp32 and in
+// (0, 1); it is the fp64 uniform of the same counter truncated to 23 bits (they differ by less than 2^-23).
+// The VEGAS passes map the fp64 uniform through the grid first and round the mapped point instead.
+template <int D>
+__device__ __forceinline__ void draw_uniforms(const Philox& rng, uint64_t point, uint32_t event, uint32_t pass,
+                                              float (&u)[D]) {
+#pragma unroll
+  for (int j = 0; 2 * j < D; ++j) {
+    uint32_t r[4];
+    rng((uint32_t)point, (uint32_t)(point >> 32), event, pass * 256u + (uint32_t)j, r);
+    u[2 * j] = fmaf(__uint2float_rn(r[0] >> 9), 0x1p-23f, 0x1p-24f);
+    if (2 * j + 1 < D) u[2 * j + 1] = fmaf(__uint2float_rn(r[2] >> 9), 0x1p-23f, 0x1p-24f);
+  }
+}
+
 // ---------------------------------------------------------------------------------------
 // small fp64 helpers
 // ---------------------------------------------------------------------------------------

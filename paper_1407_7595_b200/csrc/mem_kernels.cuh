@@ -186,8 +186,14 @@ integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__
     const int64_t i = base + threadIdx.x;
     const bool live = i < hi;
     double u[D];
-    draw_uniforms<D>(rng, (uint64_t)i, ev_ctr, pass, u);
     double w;
+    if constexpr (MODE == MODE_PLAIN && !std::is_same<T, double>::value) {
+      T uf[D];                                          // fp32 core: uniforms drawn in fp32 (see draw_uniforms)
+      draw_uniforms<D>(rng, (uint64_t)i, ev_ctr, pass, uf);
+      w = (double)P::template weight_t<PERM, GRIDPDF, false>(c, ec, uf) * c0;
+      if (!isfinite(w)) w = 0.0;
+    } else {
+    draw_uniforms<D>(rng, (uint64_t)i, ev_ctr, pass, u);
     if (MODE == MODE_PLAIN) {
       w = eval_weight<P, PERM, GRIDPDF, MODE != MODE_PLAIN>(c, ec, c0, u);
     } else {
@@ -200,6 +206,7 @@ integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__
 #pragma unroll
         for (int d = 0; d < D; ++d) warp_hist_add(wh + d * B, live ? k[d] : -1 - (int)(threadIdx.x & 31), w2);
       }
+    }
     }
     if (live) { s1 += w; s2 = fma(w, w, s2); }
   }
@@ -329,8 +336,17 @@ __global__ void eval_points_kernel(const DevConstR<typename P::real> c, const do
   if (i >= n) return;
   const Philox rng{(uint32_t)seed, (uint32_t)(seed >> 32)};
   double u[D];
-  draw_uniforms<D>(rng, (uint64_t)(first + i), (uint32_t)(event_offset + (uint64_t)event), pass, u);
   double w;
+  if constexpr (!std::is_same<T, double>::value) {
+    if (!grid) {                                        // fp32 core, plain: the integrate kernel's own uniforms
+      T uf[D];
+      draw_uniforms<D>(rng, (uint64_t)(first + i), (uint32_t)(event_offset + (uint64_t)event), pass, uf);
+      w = (double)P::template weight_t<true, true, false>(c, ec, uf) * c0;
+      out_w[i] = isfinite(w) ? w : 0.0;
+      return;
+    }
+  }
+  draw_uniforms<D>(rng, (uint64_t)(first + i), (uint32_t)(event_offset + (uint64_t)event), pass, u);
   if (grid) {
     int k[D];
     const double jac = vegas_map<D>(edges, B, u, k);
