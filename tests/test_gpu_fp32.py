@@ -1,7 +1,8 @@
 """GPU parity of the fp32 variant of config 3 (BASELINE.json:configs[2] "fp64 and fp32 variants",
 reading A15) against the fp64 CPU oracle: per-event integral relative error <= 1e-4
-(BASELINE.json:north_star).  Sampling, per-event constants, the overall constant and the sums
-stay in fp64; only the integrand core runs in single precision."""
+(BASELINE.json:north_star).  Philox, per-event constants, the overall constant and the sums stay in
+fp64/integer; the integrand core runs in single precision on fp32 uniforms built from the same
+Philox words (within 2^-23 of the oracle's fp64 uniforms)."""
 import numpy as np
 import pytest
 
