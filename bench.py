@@ -302,8 +302,6 @@ def run_b200(args):
 
     if rank != 0:
         it.close()
-        if world > 1:
-            dist.destroy_process_group()
         return
 
     total_evals = evals_per_step * world * args.steps
@@ -380,8 +378,6 @@ def run_b200(args):
                                 "sample": "first %d events (%d per core) x %d points/event of the same workload"
                                           % (events, per_core, n_points)}
     print(json.dumps(line), flush=True)
-    if world > 1:
-        dist.destroy_process_group()
 
 
 def run_sweep(args):
