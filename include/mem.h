@@ -55,7 +55,9 @@ typedef struct mem_params {
   double sqrt_s;        /* pp centre-of-mass energy */
   double G_F, m_W, Gam_W, m_Z, Gam_Z, sin2_thw, m_t, Gam_t, alpha_s, V_ud, V_tb;
   double pdf_A_q, pdf_A_g, pdf_pow_x, pdf_pow_1mx; /* toy PDF f(x) = A x^pow_x (1-x)^pow_1mx */
-  double tf_w_tail, tf_mu1, tf_sig1, tf_mu2, tf_sig2; /* double-Gaussian jet TF, fractions of parton E */
+  double tf_w_tail, tf_mu1, tf_sig1, tf_mu2, tf_sig2; /* double-Gaussian jet TF, fractions of parton E; the core must not be
+                                                       * so much narrower than the tail that exp(z1^2 - z2^2) overflows inside
+                                                       * the energy window (sigma1 >~ 0.03 for the defaults): INVALID_ARG */
   double jetE_rlo, jetE_rhi; /* parton-energy window, fractions of the measured jet energy */
   double bw_nwidths;         /* Breit-Wigner windows m +- n Gamma */
   double nu_pz_max;          /* config 1: |nu_z| <= nu_pz_max */

@@ -190,6 +190,22 @@ mem_status check_params(int process, const mem_params& p) {
   if (!pos) return fail(MEM_ERR_INVALID_ARG, "mem_params: a constant that must be positive is not");
   if (!(p.tf_w_tail >= 0.0 && p.tf_w_tail <= 1.0)) return fail(MEM_ERR_INVALID_ARG, "tf_w_tail outside [0,1]");
   if (p.nu_eta_max > 50.0) return fail(MEM_ERR_INVALID_ARG, "nu_eta_max above 50");
+  if (process != MEM_PROC_W_ENU) {
+    // The kernels write E T = exp(-z1^2) (c1 + c2 exp(z1^2 - z2^2)) (mem_common.cuh: tf_accum); z1^2 - z2^2 must
+    // stay inside the range of exp over the parton-energy window, i.e. the core Gaussian must not be
+    // absurdly narrower than the tail one (sigma1 >~ 0.03 for the default window).
+    const double r2 = std::sqrt(2.0);
+    const double a1 = 1.0 / (p.tf_sig1 * r2), b1 = -(1.0 + p.tf_mu1) * a1, a2 = 1.0 / (p.tf_sig2 * r2), b2 = -(1.0 + p.tf_mu2) * a2;
+    auto g = [&](double v) { return (a1 * v + b1) * (a1 * v + b1) - (a2 * v + b2) * (a2 * v + b2); };
+    const double v_lo = 1.0 / p.jetE_rhi, v_hi = 1.0 / p.jetE_rlo;
+    double gmax = std::fmax(g(v_lo), g(v_hi));
+    if (a1 * a1 != a2 * a2) {
+      const double v = -(a1 * b1 - a2 * b2) / (a1 * a1 - a2 * a2);
+      if (v > v_lo && v < v_hi) gmax = std::fmax(gmax, g(v));
+    }
+    if (!(gmax < 600.0))
+      return fail(MEM_ERR_INVALID_ARG, "jet TF: core Gaussian too narrow for the parton-energy window (z1^2 - z2^2 reaches %.0f)", gmax);
+  }
   if (p.n_flav < 1 || p.n_flav > 5) return fail(MEM_ERR_INVALID_ARG, "n_flav outside 1..5");
   if (p.bw_nwidths * p.Gam_W >= p.m_W || p.bw_nwidths * p.Gam_t >= p.m_t)
     return fail(MEM_ERR_INVALID_ARG, "bw_nwidths * Gamma must stay below the mass");

@@ -210,6 +210,14 @@ def test_edge_cases_and_errors(mem):
     bad.tf_sig1 = -1.0
     with pytest.raises(mem.MemError):
         mem.mem_create(proc, bad)
+    bad = mem.mem_params_default(3)
+    bad.tf_sig1 = 0.02                                 # core so narrow that exp(z1^2 - z2^2) would overflow in the window
+    with pytest.raises(mem.MemError) as ei:
+        mem.mem_create(3, bad)
+    assert ei.value.status == mem.MEM_ERR_INVALID_ARG and "too narrow" in mem.mem_last_error()
+    ok = mem.mem_params_default(3)
+    ok.tf_sig1 = 0.05
+    mem.mem_destroy(mem.mem_create(3, ok))
     bad = mem.mem_params_default(proc)
     bad.struct_size = 8
     with pytest.raises(mem.MemError):
