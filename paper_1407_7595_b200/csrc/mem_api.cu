@@ -190,6 +190,8 @@ mem_status check_params(int process, const mem_params& p) {
   if (!pos) return fail(MEM_ERR_INVALID_ARG, "mem_params: a constant that must be positive is not");
   if (!(p.tf_w_tail >= 0.0 && p.tf_w_tail <= 1.0)) return fail(MEM_ERR_INVALID_ARG, "tf_w_tail outside [0,1]");
   if (p.nu_eta_max > 50.0) return fail(MEM_ERR_INVALID_ARG, "nu_eta_max above 50");
+  if (p.precision == 32 && p.nu_eta_max > 20.0)
+    return fail(MEM_ERR_INVALID_ARG, "nu_eta_max above 20 with precision 32 (e^(2 eta) leaves the fp32 range)");
   if (process != MEM_PROC_W_ENU) {
     // The kernels write E T = exp(-z1^2) (c1 + c2 exp(z1^2 - z2^2)) (mem_common.cuh: tf_accum); z1^2 - z2^2 must
     // stay inside the range of exp over the parton-energy window, i.e. the core Gaussian must not be
