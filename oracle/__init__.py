@@ -17,7 +17,7 @@ _SRC = os.path.join(_HERE, "mem_oracle.cpp")
 _HDR = os.path.join(_HERE, "mem_oracle.h")
 _LIB = os.path.join(_HERE, "libmem_oracle.so")
 
-W_ENU, Z_BB, TT_LJETS, TT_DILEP = 1, 2, 3, 4
+W_ENU, Z_BB, TT_LJETS, TT_DILEP, TTH_DILEP = 1, 2, 3, 4, 5
 
 
 def build(force: bool = False) -> str:
@@ -42,7 +42,9 @@ class Params(C.Structure):
                            ("vegas_bins", C.c_int32), ("n_flav", C.c_int32), ("n_perm", C.c_int32),
                            ("pdf_mode", C.c_int32), ("pdf_nx", C.c_int32), ("pdf_nq", C.c_int32), ("pdf_pad", C.c_int32),
                            ("pdf_lxmin", C.c_double), ("pdf_lxmax", C.c_double), ("pdf_lqmin", C.c_double),
-                           ("pdf_lqmax", C.c_double), ("pdf_Q", C.c_double), ("pdf_data", C.c_void_p)]
+                           ("pdf_lqmax", C.c_double), ("pdf_Q", C.c_double), ("pdf_data", C.c_void_p),
+                           ("m_H", C.c_double), ("Gam_H", C.c_double), ("yuk_t", C.c_double), ("yuk_b", C.c_double),
+                           ("tth_hyp", C.c_int32), ("tth_chart", C.c_int32)]
 
 
 _lib = None
@@ -85,6 +87,23 @@ def lib():
         L.orc_boost_transverse.restype = None
         L.orc_quartic_real_roots.argtypes = [_dp, _dp]
         L.orc_dilep_solve.argtypes = [_dp] * 4 + [C.c_double] * 6 + [_dp, _dp]
+        L.orc_eq9_roots.argtypes = [C.c_double] * 3 + [_dp, _dp, _dp]
+        L.orc_tth_radiator.argtypes = [C.POINTER(Params)] + [_dp] * 3
+        L.orc_tth_radiator.restype = C.c_double
+        L.orc_tth_decay.argtypes = [C.POINTER(Params), C.c_double]
+        L.orc_tth_decay.restype = C.c_double
+        L.orc_tth_tt_invariants.argtypes = [C.POINTER(Params)] + [_dp] * 4 + [C.POINTER(C.c_double)] * 3
+        for f in (L.orc_me_tt_gg_inv, L.orc_me_tt_qq_inv):
+            f.argtypes = [C.POINTER(Params)] + [C.c_double] * 3
+            f.restype = C.c_double
+        L.orc_tt_flavour_sum.argtypes = [C.POINTER(Params)] + [C.c_double] * 4
+        L.orc_tt_flavour_sum.restype = C.c_double
+        L.orc_me_top_decay_D.argtypes = [C.POINTER(Params), C.c_double] + [_dp] * 4 + [C.c_double]
+        L.orc_me_top_decay_D.restype = C.c_double
+        L.orc_normalisation.argtypes = [_dp, _dp, C.c_int64]
+        L.orc_normalisation.restype = C.c_double
+        L.orc_discriminant.argtypes = [_dp, _dp, C.c_int64, C.c_double, C.c_double, _dp]
+        L.orc_discriminant.restype = None
         L.orc_parton_weights.argtypes = [C.c_int, C.POINTER(Params), _dp, C.c_int64, C.c_int, _dp]
         L.orc_weight.argtypes = [C.c_int, C.POINTER(Params), _dp, _dp, _dp]
         L.orc_weight.restype = C.c_double
@@ -234,6 +253,61 @@ def dilep_solve(lp, b, lm, bb, sWp, st, sWm, stb, Sx, Sy):
     return sol[:8 * n].reshape(n, 2, 4).copy(), jac[:n].copy()
 
 
+def eq9_roots(K12, f, sH):
+    """NEXT-4, Eq. 9 inverted: returns (E1 [n], E2 [n], jac) with n = 0 or 2"""
+    e1, e2, j = np.empty(2), np.empty(2), C.c_double()
+    n = lib().orc_eq9_roots(K12, f, sH, _p(e1), _p(e2), C.byref(j))
+    return e1[:n].copy(), e2[:n].copy(), j.value
+
+
+def tth_radiator(p, pt, ptb, k):
+    a = _v4(pt, ptb, k)
+    return lib().orc_tth_radiator(C.byref(p), *[_p(x) for x in a])
+
+
+def tth_decay(p, sH):
+    return lib().orc_tth_decay(C.byref(p), float(sH))
+
+
+def tth_tt_invariants(p, q1, q2, pt, ptb):
+    """(ok, tau1, tau2, rho) of the t tbar subsystem (reading A20)"""
+    a = _v4(q1, q2, pt, ptb)
+    t1, t2, rho = C.c_double(), C.c_double(), C.c_double()
+    ok = lib().orc_tth_tt_invariants(C.byref(p), *[_p(x) for x in a], C.byref(t1), C.byref(t2), C.byref(rho))
+    return bool(ok), t1.value, t2.value, rho.value
+
+
+def me_tt_gg_inv(p, t1, t2, rho):
+    return lib().orc_me_tt_gg_inv(C.byref(p), t1, t2, rho)
+
+
+def me_tt_qq_inv(p, t1, t2, rho):
+    return lib().orc_me_tt_qq_inv(C.byref(p), t1, t2, rho)
+
+
+def tt_flavour_sum(p, x1, x2, me_gg, me_qq):
+    return lib().orc_tt_flavour_sum(C.byref(p), x1, x2, me_gg, me_qq)
+
+
+def me_top_decay_D(p, n_c, pt, pb, pf_down, pf_up, D_W):
+    a = _v4(pt, pb, pf_down, pf_up)
+    return lib().orc_me_top_decay_D(C.byref(p), float(n_c), *[_p(x) for x in a], float(D_W))
+
+
+def normalisation(p_evt, g_evt):
+    """reading A22: sigma = (1/n) sum_e p_e / g_e over events drawn from the density g"""
+    a, b = _f64(p_evt), _f64(g_evt)
+    return lib().orc_normalisation(_p(a), _p(b), a.shape[0])
+
+
+def discriminant(p_sig, p_bkg, sigma_sig, sigma_bkg):
+    """PAPER.md:143 Eq. 10 with the 1/sigma of Eq. 1"""
+    a, b = _f64(p_sig), _f64(p_bkg)
+    out = np.empty(a.shape[0])
+    lib().orc_discriminant(_p(a), _p(b), a.shape[0], sigma_sig, sigma_bkg, _p(out))
+    return out
+
+
 def parton_weights(process, p, mom, extended=False):
     """NEXT-2: parton-level weights; mom = [24, n_events] (l, nu, b_had, b_lep, q, qbar')"""
     m = _f64(mom)
@@ -246,7 +320,7 @@ def parton_weights(process, p, mom, extended=False):
 def weight(process, p, rec, u, debug=False):
     rec, u = _f64(rec), _f64(u)
     if debug:
-        dbg = np.zeros(1 + 4 * (2 + 4 * 6), dtype=np.float64)
+        dbg = np.zeros(1 + 8 * (2 + 4 * 8), dtype=np.float64)
         w = lib().orc_weight(process, C.byref(p), _p(rec), _p(u), _p(dbg))
         return w, dbg
     return lib().orc_weight(process, C.byref(p), _p(rec), _p(u), None)

@@ -203,18 +203,25 @@ template <typename R> void tt_invariants(const orc_params* p, const R q1[4], con
   *t2 = (dot(b, t) + dot(a, tb)) / shat;
   *rho = R(4) * R(p->m_t) * R(p->m_t) / shat;
 }
+// the two production matrix elements as functions of (tau1, tau2, rho)
+template <typename R> R me_tt_qq_inv(const orc_params* p, R t1, R t2, R rho) {
+  R g = gs2<R>(p);
+  return g * g * (R(4) / R(9)) * (t1 * t1 + t2 * t2 + rho / R(2));
+}
+template <typename R> R me_tt_gg_inv(const orc_params* p, R t1, R t2, R rho) {
+  R g = gs2<R>(p);
+  return g * g * (R(1) / (R(6) * t1 * t2) - R(3) / R(8)) *
+         (t1 * t1 + t2 * t2 + rho - rho * rho / (R(4) * t1 * t2));
+}
 template <typename R> R me_tt_qq(const orc_params* p, const R q1[4], const R q2[4], const R pt[4], const R ptb[4]) {
   R t1, t2, rho;
   tt_invariants<R>(p, q1, q2, pt, ptb, &t1, &t2, &rho);
-  R g = gs2<R>(p);
-  return g * g * (R(4) / R(9)) * (t1 * t1 + t2 * t2 + rho / R(2));
+  return me_tt_qq_inv<R>(p, t1, t2, rho);
 }
 template <typename R> R me_tt_gg(const orc_params* p, const R q1[4], const R q2[4], const R pt[4], const R ptb[4]) {
   R t1, t2, rho;
   tt_invariants<R>(p, q1, q2, pt, ptb, &t1, &t2, &rho);
-  R g = gs2<R>(p);
-  return g * g * (R(1) / (R(6) * t1 * t2) - R(3) / R(8)) *
-         (t1 * t1 + t2 * t2 + rho - rho * rho / (R(4) * t1 * t2));
+  return me_tt_gg_inv<R>(p, t1, t2, rho);
 }
 
 // sum over all spins of |M(t -> b W -> b fdown-bar... )|^2 with the pairing
@@ -722,6 +729,205 @@ template <typename R> R weight_tt_dilep(const orc_params* p, const double* rec, 
   return std::isfinite((double)w) ? w : R(0);
 }
 
+// ---------------- NEXT-4: t tbar H(-> b bbar), dilepton, four b jets, D = 8 ----------------
+// PAPER.md:101-109 Eq. 7 (the paper's own benchmark integral: four jet-energy TFs, the two neutrinos
+// fixed by the MET delta functions), :111-118 Eq. 8 (neutrino momenta -> q^2 of the W and top
+// propagators), :120-137 Eq. 9 (Higgs b-quark energies (E1, E2) -> (f = E1 + E2, m_H^2)), :178-180
+// Eq. 11 (the MET entering Eq. 8 is minus the visible transverse momentum of the point, so the total
+// transverse momentum vanishes and the O7 boost is the identity: it is not applied).
+// rec = [(pT,eta,phi) l+, (pT,eta,phi) l-, (E,eta,phi) x {b, bbar, b1, b2}]: b pairs with l+ (top),
+// bbar with l- (antitop), b1 b2 are the Higgs candidates.  No measured MET enters (Eq. 11).
+// DESIGN.md "NEXT-4" readings A18-A21.
+
+// Eq. 9 for massless b quarks ("E is set to |p|"): f = E1 + E2, m^2 = 2 E1 E2 K12 with
+// K12 = 1 - cos(Delta theta_12).  Inverse: E1 E2 = m^2/(2 K12), so E1, E2 = (f +- sqrt(f^2 - 2 m^2/K12))/2:
+// the map is two-to-one (E1 <-> E2) and BOTH orderings are returned (reading A19);
+// |d(E1,E2)/d(f,m^2)| = 1/(2 K12 |E1 - E2|).  Returns 0 or 2.
+template <typename R> int eq9_roots(R K12, R f, R sH, R E1[2], R E2[2], R* jac) {
+  const R disc = f * f - R(2) * sH / K12;
+  if (!(disc > R(0))) return 0;
+  const R rt = std::sqrt(disc);
+  E1[0] = (f + rt) / R(2); E2[0] = (f - rt) / R(2);
+  E1[1] = E2[0]; E2[1] = E1[0];
+  *jac = R(1) / (R(2) * K12 * rt);
+  return 2;
+}
+
+// Factorised matrix-element pieces of the two hypotheses (reading A20; SURVEY.md 8(f)-4 "factorised
+// t tbar H ME ... a second factorised hypothesis"): radiation of the b bbar system k = p_b1 + p_b2 off the
+// top pair, the propagator of what was radiated, and its decay into b bbar.
+//   hyp 0, t tbar H: soft-scalar (eikonal) emission off either top, y_t^2 4 m_t^2 (1/X_t + 1/X_tbar)^2 with
+//          X = 2 p.k + k^2; Higgs propagator D_H(k^2); sum |M(H -> b bbar)|^2 = 3 y_b^2 2 k^2 (massless b)
+//   hyp 1, non-resonant t tbar b bbar: eikonal vector emission g_s^2 (-J^2),
+//          J = p_t/(p_t.k) - p_tbar/(p_tbar.k) (>= 0 for timelike k); propagator 1/k^4; splitting g_s^2 k^2;
+//          colour factors set to 1.
+template <typename R> R tth_radiator(const orc_params* p, const V4<R>& pt, const V4<R>& ptb, const V4<R>& k) {
+  const R sH = dot(k, k);
+  if (p->tth_hyp == 0) {
+    const R Xt = R(2) * dot(pt, k) + sH, Xtb = R(2) * dot(ptb, k) + sH;
+    const R a = R(1) / Xt + R(1) / Xtb;
+    return R(p->yuk_t) * R(p->yuk_t) * R(4) * R(p->m_t) * R(p->m_t) * a * a;
+  }
+  const R tk = dot(pt, k), tbk = dot(ptb, k);
+  return gs2<R>(p) * (R(2) * dot(pt, ptb) / (tk * tbk) - dot(pt, pt) / (tk * tk) - dot(ptb, ptb) / (tbk * tbk));
+}
+template <typename R> R tth_decay(const orc_params* p, R sH) {
+  if (p->tth_hyp == 0) return R(3) * R(p->yuk_b) * R(p->yuk_b) * R(2) * sH;
+  return gs2<R>(p) * sH;
+}
+
+// t tbar production next to a third body (reading A20): tau1, tau2 of reading A9 normalised to
+// tau1 + tau2 = 1, rho = 4 m_t^2 / (p_t + p_tbar)^2; 0 unless rho < 1.
+template <typename R> bool tth_tt_invariants(const orc_params* p, const R q1[4], const R q2[4], const V4<R>& t,
+                                             const V4<R>& tb, R* t1, R* t2, R* rho) {
+  V4<R> a = from_arr(q1), b = from_arr(q2);
+  const R n1 = dot(a, t) + dot(b, tb), n2 = dot(b, t) + dot(a, tb);
+  const R stt = dot(t + tb, t + tb);
+  if (!(R(4) * R(p->m_t) * R(p->m_t) < stt)) return false;
+  *t1 = n1 / (n1 + n2); *t2 = n2 / (n1 + n2);
+  *rho = R(4) * R(p->m_t) * R(p->m_t) / stt;
+  return true;
+}
+
+// Everything that depends on the Higgs b-quark energies (E1, E2): jets b1, b2 with their TFs and measures,
+// Eq. 11, the neutrino solutions of Eq. 8, and per solution Jacobian x neutrino measure x PDFs x |M|^2 / flux.
+// propH = the propagator factor of the radiated system (D_H from the mapped variable, or 1/k^4).
+template <typename R> R tth_core(const orc_params* p, const double* rec, const V4<R>& lp, const V4<R>& lm,
+                                 const V4<R>& b, const V4<R>& bb, R E1, R E2, R sWp, R st, R sWm, R stb,
+                                 const R Dk[4], R propH, double* dbg, int* kept) {
+  const R S = R(p->sqrt_s) * R(p->sqrt_s), mt = p->m_t;
+  const R twopi3 = R(8) * pi_<R>() * pi_<R>() * pi_<R>();
+  const R Ej1 = rec[12], Ej2 = rec[15];
+  const V4<R> b1 = from_E_eta_phi<R>(E1, R(rec[13]), R(rec[14])), b2 = from_E_eta_phi<R>(E2, R(rec[16]), R(rec[17]));
+  const R tf12 = tf_jet<R>(p, Ej1, E1) * tf_jet<R>(p, Ej2, E2);
+  const R meas12 = E1 * (R(1) / std::cosh(R(rec[13]))) / (R(2) * twopi3) * E2 * (R(1) / std::cosh(R(rec[16]))) / (R(2) * twopi3);
+  // Eq. 11: the neutrino pair balances the visible system of THIS point
+  const V4<R> vis = lp + lm + b + bb + b1 + b2;
+  const R Sx = -vis.x, Sy = -vis.y;
+  R sol[4][8];
+  const int nsol = dilep_solve<R>(lp, b, lm, bb, sWp, st, sWm, stb, Sx, Sy, sol);
+  const V4<R> k = b1 + b2;
+  const R sH = dot(k, k);
+  R sum = R(0);
+  for (int i = 0; i < nsol; ++i) {
+    const R J = dilep_jacobian<R>(lp, b, lm, bb, sol[i]);
+    V4<R> nu = from_arr(sol[i]), nub = from_arr(sol[i] + 4);
+    const V4<R> P = vis + nu + nub;                         // P_T = 0 by construction
+    R x1, x2;
+    if (!beam_fractions<R>(p, P.E, P.z, &x1, &x2)) continue;
+    R q1[4], q2[4];
+    beams<R>(p, x1, x2, q1, q2);
+    const V4<R> pt = lp + nu + b, ptb = lm + nub + bb;
+    R t1, t2, rho;
+    if (!tth_tt_invariants<R>(p, q1, q2, pt, ptb, &t1, &t2, &rho)) continue;
+    const R prod = tt_flavour_sum<R>(p, x1, x2, me_tt_gg_inv<R>(p, t1, t2, rho), me_tt_qq_inv<R>(p, t1, t2, rho));   // includes the PDFs
+    R pta[4], ptba[4], la[4], na[4], ba[4], lma[4], nba[4], bba[4];
+    to_arr(pt, pta); to_arr(ptb, ptba); to_arr(lp, la); to_arr(nu, na); to_arr(b, ba);
+    to_arr(lm, lma); to_arr(nub, nba); to_arr(bb, bba);
+    const R dec1 = R(0.5) * me_top_decay_D<R>(p, R(1), pta, ba, la, na, Dk[0]);
+    const R dec2 = R(0.5) * me_top_decay_D<R>(p, R(1), ptba, bba, lma, nba, Dk[2]);
+    const R me = prod * tth_radiator<R>(p, pt, ptb, k) * propH * tth_decay<R>(p, sH) * Dk[1] * Dk[3] * dec1 * dec2;
+    const R flux = x1 * x2 * S / R(4);
+    const R ws = J / (twopi3 * twopi3 * R(4) * nu.E * nub.E) * me / flux;
+    if (!std::isfinite((double)ws)) continue;
+    sum += ws;
+    if (dbg && *kept < 8) {
+      R mom[32];
+      to_arr(lp, mom); to_arr(nu, mom + 4); to_arr(b, mom + 8); to_arr(lm, mom + 12); to_arr(nub, mom + 16);
+      to_arr(bb, mom + 20); to_arr(b1, mom + 24); to_arr(b2, mom + 28);
+      dbg_store<R>(dbg, *kept, 8, x1, x2, mom);
+    }
+    ++*kept;
+  }
+  (void)mt;
+  return tf12 * meas12 * sum;
+}
+
+template <typename R> R weight_tth_dilep(const orc_params* p, const double* rec, const double* u, double* dbg) {
+  const R S = R(p->sqrt_s) * R(p->sqrt_s), rlo = p->jetE_rlo, rhi = p->jetE_rhi, dr = rhi - rlo;
+  const R twopi3 = R(8) * pi_<R>() * pi_<R>() * pi_<R>();
+  if (dbg) dbg[0] = 0;
+  V4<R> lp = from_pt_eta_phi<R>(rec[0], rec[1], rec[2]), lm = from_pt_eta_phi<R>(rec[3], rec[4], rec[5]);
+  V4<R> jet[2];
+  R vol = R(1), tf = R(1), meas = R(1);
+  for (int j = 0; j < 2; ++j) {                              // b (top side), bbar (antitop side): O5
+    R Ej = rec[6 + 3 * j], eta = rec[7 + 3 * j], phi = rec[8 + 3 * j];
+    R E = Ej * (rlo + dr * R(u[j]));
+    vol *= Ej * dr;
+    tf *= tf_jet<R>(p, Ej, E);
+    meas *= E * (R(1) / std::cosh(eta)) / (R(2) * twopi3);
+    jet[j] = from_E_eta_phi<R>(E, eta, phi);
+  }
+  const V4<R> &b = jet[0], &bb = jet[1];
+  // four Breit-Wigner mapped masses: u2 -> s_W+, u3 -> s_t, u4 -> s_W-, u5 -> s_tbar (O6), as in config 4
+  const R mW = p->m_W, GW = p->Gam_W, mt = p->m_t, Gt = p->Gam_t, n = p->bw_nwidths;
+  R tWlo, tWhi, tTlo, tThi;
+  bw_window<R>(mW, GW, (mW - n * GW) * (mW - n * GW), (mW + n * GW) * (mW + n * GW), &tWlo, &tWhi);
+  bw_window<R>(mt, Gt, (mt - n * Gt) * (mt - n * Gt), (mt + n * Gt) * (mt + n * Gt), &tTlo, &tThi);
+  R smm[4], dsdt[4], Dk[4];
+  for (int k = 0; k < 4; ++k) {
+    const bool isW = (k == 0 || k == 2);
+    const R lo = isW ? tWlo : tTlo, hi = isW ? tWhi : tThi;
+    const R t = lo + (hi - lo) * R(u[2 + k]);
+    vol *= (hi - lo);
+    bw_point<R>(isW ? mW : mt, isW ? GW : Gt, t, &smm[k], &dsdt[k], &Dk[k]);
+  }
+  const R sWp = mW * mW + smm[0], st = mt * mt + smm[1], sWm = mW * mW + smm[2], stb = mt * mt + smm[3];
+  meas *= R(1) / (R(2) * lp.E * twopi3) * R(1) / (R(2) * lm.E * twopi3);   // leptons: delta TF
+  // Higgs candidates b1, b2
+  const R Ej1 = rec[12], Ej2 = rec[15];
+  const V4<R> n1 = from_E_eta_phi<R>(R(1), R(rec[13]), R(rec[14])), n2 = from_E_eta_phi<R>(R(1), R(rec[16]), R(rec[17]));
+  const R K12 = dot(n1, n2);                                 // 1 - cos(Delta theta_12)
+  const R mH = p->m_H, GH = p->Gam_H;
+  // window of k^2 = (p_b1 + p_b2)^2.  hyp 0: Breit-Wigner window of the Higgs, mapped by O6;
+  // hyp 1: everything the two energy windows allow, s in 2 K12 Ej1 Ej2 [rlo^2, rhi^2], mapped with
+  // s = s_lo (s_hi/s_lo)^u (flat in ln s, ds/du = s ln(s_hi/s_lo))
+  R tHlo = 0, tHhi = 0;
+  if (p->tth_hyp == 0) bw_window<R>(mH, GH, (mH - n * GH) * (mH - n * GH), (mH + n * GH) * (mH + n * GH), &tHlo, &tHhi);
+  const R s_lo = R(2) * K12 * Ej1 * Ej2 * rlo * rlo, lnr = R(2) * std::log(rhi / rlo);
+  int kept = 0;
+  R sum = R(0);
+  if (p->tth_chart == 0) {
+    // Eq. 9 chart: u6 -> k^2, u7 -> f = E1 + E2 flat over the sum of the two energy windows
+    R sH, propH, jac_map;
+    if (p->tth_hyp == 0) {
+      const R t = tHlo + (tHhi - tHlo) * R(u[6]);
+      R smH, dsdtH, DH;
+      bw_point<R>(mH, GH, t, &smH, &dsdtH, &DH);
+      sH = mH * mH + smH; propH = DH; jac_map = (tHhi - tHlo) * dsdtH;
+    } else {
+      sH = s_lo * std::exp(lnr * R(u[6]));
+      propH = R(1) / (sH * sH); jac_map = lnr * sH;
+    }
+    const R f = (Ej1 + Ej2) * (rlo + dr * R(u[7]));
+    const R volf = (Ej1 + Ej2) * dr;
+    R E1[2], E2[2], jac9;
+    const int nroot = eq9_roots<R>(K12, f, sH, E1, E2, &jac9);
+    for (int r = 0; r < nroot; ++r) {
+      // a root counts only inside both parton-energy windows, so that the chart covers exactly the box of O5
+      if (!(E1[r] >= rlo * Ej1 && E1[r] <= rhi * Ej1 && E2[r] >= rlo * Ej2 && E2[r] <= rhi * Ej2)) continue;
+      sum += jac_map * volf * jac9 * tth_core<R>(p, rec, lp, lm, b, bb, E1[r], E2[r], sWp, st, sWm, stb, Dk, propH, dbg, &kept);
+    }
+  } else {
+    // pin chart (tests only): (E1, E2) flat in their windows, k^2 from the momenta
+    const R E1 = Ej1 * (rlo + dr * R(u[6])), E2 = Ej2 * (rlo + dr * R(u[7]));
+    const R sH = R(2) * E1 * E2 * K12;
+    R propH;
+    bool inside = true;
+    if (p->tth_hyp == 0) {
+      inside = (sH >= (mH - n * GH) * (mH - n * GH)) && (sH <= (mH + n * GH) * (mH + n * GH));
+      propH = bw_D<R>(sH - mH * mH, mH, GH);
+    } else {
+      propH = R(1) / (sH * sH);
+    }
+    if (inside) sum = Ej1 * dr * Ej2 * dr * tth_core<R>(p, rec, lp, lm, b, bb, E1, E2, sWp, st, sWm, stb, Dk, propH, dbg, &kept);
+  }
+  if (dbg) dbg[0] = kept < 8 ? kept : 8;
+  R w = vol * dsdt[0] * dsdt[1] * dsdt[2] * dsdt[3] * tf * meas *
+        (R(16) * pi_<R>() * pi_<R>() * pi_<R>() * pi_<R>()) * (R(2) / S) * sum;
+  return std::isfinite((double)w) ? w : R(0);
+}
+
 // NEXT-1 (Eq. 7: "The outer sum is over all permutations of assigning measured
 // jets to partons in the matrix element").  The sum over
 // assignments sits outside the integral, i.e. every sample point is evaluated for each assignment:
@@ -738,6 +944,16 @@ inline int jet_perms(int process, int n_perm, int perm[24][4]) {
     push(0, 1, 2, 3); push(0, 1, 3, 2); push(1, 0, 2, 3); push(1, 0, 3, 2);
   } else if (process == ORC_TT_DILEP && n_perm == 2) {
     push(0, 1, 2, 3); push(1, 0, 2, 3);
+  } else if (process == ORC_TTH_DILEP && n_perm == 12) {
+    // roles (b, bbar, b1, b2); the integrand is symmetric in b1 <-> b2 (both Eq. 9 orderings are summed),
+    // so the 4!/2 = 12 distinct assignments are the ordered choices of (b, bbar), the remaining two jets
+    // in ascending order
+    for (int a = 0; a < 4; ++a) for (int b = 0; b < 4; ++b) {
+      if (a == b) continue;
+      int rest[2], m = 0;
+      for (int c = 0; c < 4; ++c) if (c != a && c != b) rest[m++] = c;
+      push(a, b, rest[0], rest[1]);
+    }
   } else {
     push(id[0], id[1], id[2], id[3]);
   }
@@ -749,16 +965,17 @@ template <typename R> R weight_permuted(int process, const orc_params* p, const 
   int perm[24][4];
   const int n = jet_perms(process, p->n_perm, perm);
   const int first_jet = (process == ORC_TT_LJETS) ? 3 : 6;   // record offset of the first (E, eta, phi) triple
-  const int n_jets = (process == ORC_TT_LJETS) ? 4 : 2;
-  const int nf = (process == ORC_TT_LJETS) ? 17 : 14;
+  const int n_jets = (process == ORC_TT_DILEP) ? 2 : 4;
+  const int nf = orc_n_fields(process);
   R sum = R(0);
   for (int k = 0; k < n; ++k) {
     double r2[32];
     for (int f = 0; f < nf; ++f) r2[f] = rec[f];
     for (int role = 0; role < n_jets; ++role)
       for (int c = 0; c < 3; ++c) r2[first_jet + 3 * role + c] = rec[first_jet + 3 * perm[k][role] + c];
-    sum += (process == ORC_TT_LJETS) ? weight_tt_ljets<R>(p, r2, u, k == 0 ? dbg : nullptr)
-                                     : weight_tt_dilep<R>(p, r2, u, k == 0 ? dbg : nullptr);
+    sum += (process == ORC_TT_LJETS)   ? weight_tt_ljets<R>(p, r2, u, k == 0 ? dbg : nullptr)
+           : (process == ORC_TT_DILEP) ? weight_tt_dilep<R>(p, r2, u, k == 0 ? dbg : nullptr)
+                                       : weight_tth_dilep<R>(p, r2, u, k == 0 ? dbg : nullptr);
   }
   return sum;
 }
@@ -818,6 +1035,7 @@ template <typename R> double weight_any(int process, const orc_params* p, const 
     case ORC_Z_BB: w = weight_z_bb<R>(p, rec, u, dbg); break;
     case ORC_TT_LJETS: w = weight_permuted<R>(process, p, rec, u, dbg); break;
     case ORC_TT_DILEP: w = weight_permuted<R>(process, p, rec, u, dbg); break;
+    case ORC_TTH_DILEP: w = weight_permuted<R>(process, p, rec, u, dbg); break;
     default: return std::nan("");
   }
   double wd = (double)w;
@@ -853,12 +1071,12 @@ extern "C" {
 // --------------------------------------------------------------------------
 int orc_n_fields(int process) {
   switch (process) { case ORC_W_ENU: return 5; case ORC_Z_BB: return 6;
-                     case ORC_TT_LJETS: return 17; case ORC_TT_DILEP: return 14; }
+                     case ORC_TT_LJETS: return 17; case ORC_TT_DILEP: return 14; case ORC_TTH_DILEP: return 18; }
   return -1;
 }
 int orc_n_dims(int process) {
   switch (process) { case ORC_W_ENU: return 1; case ORC_Z_BB: return 2;
-                     case ORC_TT_LJETS: return 6; case ORC_TT_DILEP: return 8; }
+                     case ORC_TT_LJETS: return 6; case ORC_TT_DILEP: return 8; case ORC_TTH_DILEP: return 8; }
   return -1;
 }
 
@@ -878,6 +1096,12 @@ int orc_params_default(int process, orc_params* p) {
   p->nu_eta_max = 5.0; p->met_sigma = 10.0; p->met_nsigma = 4.0;
   p->vegas_alpha = 0.5; p->vegas_points = 1 << 17; p->vegas_iters = 0; p->vegas_bins = 50;  // configs[4]
   p->n_flav = (process == ORC_Z_BB) ? 3 : 5; // configs[1] "u,d,s"; PAPER.md:141 (d,u,s,c,b)
+  // NEXT-4 (reading A21; the paper gives none): m_H = 125, Gamma_H = 4.07 MeV ("very narrow"),
+  // Yukawa couplings y_f = m_f sqrt(2 sqrt2 G_F) with m_b = 4.18 in the coupling only (kinematics massless)
+  p->m_H = 125.0; p->Gam_H = 0.00407;
+  p->yuk_t = p->m_t * std::sqrt(2.0 * std::sqrt(2.0) * p->G_F);
+  p->yuk_b = 4.18 * std::sqrt(2.0 * std::sqrt(2.0) * p->G_F);
+  p->tth_hyp = 0; p->tth_chart = 0;
   return 0;
 }
 
@@ -978,6 +1202,42 @@ int orc_parton_weights(int process, const orc_params* p, const double* mom, int6
 }
 
 double orc_pdf_grid(const orc_params* p, int species, double x, double Q) { return pdf_grid<double>(p, species, x, Q); }
+
+// NEXT-4 building blocks (pinned by tests/test_oracle_tth.py)
+int orc_eq9_roots(double K12, double f, double sH, double E1[2], double E2[2], double* jac) {
+  return eq9_roots<double>(K12, f, sH, E1, E2, jac);
+}
+double orc_tth_radiator(const orc_params* p, const double pt[4], const double ptb[4], const double k[4]) {
+  return tth_radiator<double>(p, from_arr(pt), from_arr(ptb), from_arr(k));
+}
+double orc_tth_decay(const orc_params* p, double sH) { return tth_decay<double>(p, sH); }
+int orc_tth_tt_invariants(const orc_params* p, const double q1[4], const double q2[4], const double pt[4],
+                          const double ptb[4], double* t1, double* t2, double* rho) {
+  return tth_tt_invariants<double>(p, q1, q2, from_arr(pt), from_arr(ptb), t1, t2, rho) ? 1 : 0;
+}
+double orc_me_tt_gg_inv(const orc_params* p, double t1, double t2, double rho) { return me_tt_gg_inv<double>(p, t1, t2, rho); }
+double orc_me_tt_qq_inv(const orc_params* p, double t1, double t2, double rho) { return me_tt_qq_inv<double>(p, t1, t2, rho); }
+double orc_tt_flavour_sum(const orc_params* p, double x1, double x2, double me_gg, double me_qq) {
+  return tt_flavour_sum<double>(p, x1, x2, me_gg, me_qq);
+}
+// sum over all spins of |M(t -> b f fbar')|^2 with the W propagator passed in (mapped resonance, O6)
+double orc_me_top_decay_D(const orc_params* p, double n_c, const double pt[4], const double pb[4],
+                          const double pf_down[4], const double pf_up[4], double D_W) {
+  return me_top_decay_D<double>(p, n_c, pt, pb, pf_down, pf_up, D_W);
+}
+
+// post-processing of PAPER.md:45 (1/sigma) and :143 Eq. 10 (reading A22): sigma as the importance-sampled
+// acceptance integral (1/n) sum_e p_e / g_e over events drawn from the density g; D = log10 of the ratio of
+// the two normalised likelihoods.
+double orc_normalisation(const double* p, const double* g, int64_t n) {
+  NSum s;
+  for (int64_t e = 0; e < n; ++e) s.add(p[e] / g[e]);
+  return s.value() / (double)n;
+}
+void orc_discriminant(const double* p_sig, const double* p_bkg, int64_t n, double sigma_sig, double sigma_bkg,
+                      double* out_D) {
+  for (int64_t e = 0; e < n; ++e) out_D[e] = std::log10((p_sig[e] / sigma_sig) / (p_bkg[e] / sigma_bkg));
+}
 
 double orc_weight(int process, const orc_params* p, const double* rec, const double* u, double* dbg) {
   return weight_any<double>(process, p, rec, u, dbg);

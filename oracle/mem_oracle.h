@@ -18,7 +18,7 @@
 extern "C" {
 #endif
 
-enum { ORC_W_ENU = 1, ORC_Z_BB = 2, ORC_TT_LJETS = 3, ORC_TT_DILEP = 4 };
+enum { ORC_W_ENU = 1, ORC_Z_BB = 2, ORC_TT_LJETS = 3, ORC_TT_DILEP = 4, ORC_TTH_DILEP = 5 };
 
 /* DESIGN.md "Readings" O8/A13: the paper gives no constants; BASELINE.json
  * configs give sqrt_s, m_W, Gam_W, m_t, Gam_t, the toy PDF and the TF numbers. */
@@ -48,11 +48,18 @@ typedef struct orc_params {
   int32_t pdf_mode, pdf_nx, pdf_nq, pdf_pad;
   double pdf_lxmin, pdf_lxmax, pdf_lqmin, pdf_lqmax, pdf_Q;
   const double* pdf_data;
+  /* NEXT-4, t tbar H(-> b bbar) dilepton (PAPER.md:101-137 Eq. 7-9, :178-180 Eq. 11; readings A18-A21):
+   * Higgs mass and width (Breit-Wigner map of Eq. 9's m_H^2), Yukawa couplings of the factorised matrix element,
+   * tth_hyp 0 = t tbar H signal, 1 = non-resonant t tbar b bbar stand-in (the second hypothesis of Eq. 10);
+   * tth_chart (oracle only) 0 = Eq. 9 chart (f, m_H^2), 1 = flat (E1, E2) chart for the chart-independence pin.
+   * ORC_TTH_DILEP: n_perm 12 = all 4!/2 distinct assignments of four b jets to (b, bbar, {b1, b2}). */
+  double m_H, Gam_H, yuk_t, yuk_b;
+  int32_t tth_hyp, tth_chart;
 } orc_params;
 
 int  orc_params_default(int process, orc_params* p);
-int  orc_n_fields(int process);   /* 5 / 6 / 17 / 14 */
-int  orc_n_dims(int process);     /* 1 / 2 / 6 / 8  */
+int  orc_n_fields(int process);   /* 5 / 6 / 17 / 14 / 18 */
+int  orc_n_dims(int process);     /* 1 / 2 / 6 / 8 / 8 */
 
 /* --- random numbers (O2) --- */
 void   orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
@@ -89,8 +96,30 @@ int    orc_dilep_solve(const double lp[4], const double b[4], const double lm[4]
                        double sWp, double st, double sWm, double stb, double Sx, double Sy,
                        double* sol, double* jac);
 
+/* NEXT-4 building blocks.  Eq. 9 inverted for massless b quarks: both orderings
+ * (E1[r], E2[r]) with E1 + E2 = f, 2 E1 E2 K12 = sH, *jac = |d(E1,E2)/d(f,sH)|; returns 0 or 2.
+ * Factorised matrix-element pieces (reading A20): radiation factor of k = p_b1 + p_b2 off the top pair and
+ * the decay factor of the radiated system, both for p->tth_hyp; normalised (tau1, tau2, rho) of the t tbar
+ * subsystem (returns 0 when rho >= 1); the production MEs as functions of (tau1, tau2, rho); the flavour sum
+ * incl. the PDFs. */
+int    orc_eq9_roots(double K12, double f, double sH, double E1[2], double E2[2], double* jac);
+double orc_tth_radiator(const orc_params* p, const double pt[4], const double ptb[4], const double k[4]);
+double orc_tth_decay(const orc_params* p, double sH);
+int    orc_tth_tt_invariants(const orc_params* p, const double q1[4], const double q2[4], const double pt[4],
+                             const double ptb[4], double* t1, double* t2, double* rho);
+double orc_me_tt_gg_inv(const orc_params* p, double t1, double t2, double rho);
+double orc_me_tt_qq_inv(const orc_params* p, double t1, double t2, double rho);
+double orc_tt_flavour_sum(const orc_params* p, double x1, double x2, double me_gg, double me_qq);
+double orc_me_top_decay_D(const orc_params* p, double n_c, const double pt[4], const double pb[4],
+                          const double pf_down[4], const double pf_up[4], double D_W);
+/* 1/sigma and the discriminant (Eq. 10; reading A22) */
+double orc_normalisation(const double* p, const double* g, int64_t n);
+void   orc_discriminant(const double* p_sig, const double* p_bkg, int64_t n, double sigma_sig, double sigma_bkg,
+                        double* out_D);
+
 /* --- the integrand: one event record (n_fields doubles), one unit-cube point --- */
-/* dbg (may be NULL): [0]=n_sol, [1..]= per solution: x1, x2, then the boosted final momenta. */
+/* dbg (may be NULL): [0]=n_sol, [1..]= per solution: x1, x2, then the boosted final momenta
+ * (2 / 6 / 8 four-vectors; room for 8 solutions of 8 particles: 273 doubles). */
 double orc_weight(int process, const orc_params* p, const double* rec, const double* u, double* dbg);
 /* Extended-precision referee: the same templates instantiated in long double (x87, 64-bit
  * mantissa), result rounded to double.  Used by the tests to adjudicate ill-conditioned points. */

@@ -17,9 +17,9 @@ import numpy as np
 
 DEFAULT_SEED = 20140729
 
-W_ENU, Z_BB, TT_LJETS, TT_DILEP = 1, 2, 3, 4
-N_FIELDS = {W_ENU: 5, Z_BB: 6, TT_LJETS: 17, TT_DILEP: 14}
-N_DIMS = {W_ENU: 1, Z_BB: 2, TT_LJETS: 6, TT_DILEP: 8}
+W_ENU, Z_BB, TT_LJETS, TT_DILEP, TTH_DILEP = 1, 2, 3, 4, 5
+N_FIELDS = {W_ENU: 5, Z_BB: 6, TT_LJETS: 17, TT_DILEP: 14, TTH_DILEP: 18}
+N_DIMS = {W_ENU: 1, Z_BB: 2, TT_LJETS: 6, TT_DILEP: 8, TTH_DILEP: 8}
 
 # BASELINE.json:configs[0..3]: (process, n_events, n_points)
 CONFIGS = {
@@ -27,6 +27,8 @@ CONFIGS = {
     2: (Z_BB, 1024, 1 << 18),
     3: (TT_LJETS, 4096, 1 << 20),
     4: (TT_DILEP, 16384, 1 << 18),
+    # NEXT-4 (not a BASELINE config; sizes follow config 4): the paper's own benchmark shape
+    6: (TTH_DILEP, 16384, 1 << 18),
 }
 
 
@@ -74,11 +76,30 @@ def make_events(process: int, n_events: int, seed: int = DEFAULT_SEED) -> np.nda
         rad = np.sqrt(-2.0 * np.log1p(-u1))      # Box-Muller
         rows = [*lp, *lm, *b, *bb, -vx + 10.0 * rad * np.cos(2 * np.pi * u2),
                 -vy + 10.0 * rad * np.sin(2 * np.pi * u2)]
+    elif process == TTH_DILEP:
+        # two leptons and four b jets (b, bbar, b1, b2), i.i.d. like configs 3-4; no MET field (Eq. 11)
+        rows = [*_lepton(r, n), *_lepton(r, n)]
+        for _ in range(4):
+            rows += [*_jet(r, n)]
     else:
         raise ValueError("unknown process %r" % (process,))
     ev = np.ascontiguousarray(np.stack(rows, axis=0), dtype=np.float64)
     assert ev.shape == (N_FIELDS[process], n)
     return ev
+
+
+def event_density(process: int, ev: np.ndarray) -> np.ndarray:
+    """Probability density g(X) of make_events' records with respect to the record's own coordinates
+    (pT or E, eta, phi per object), for the importance-sampled normalisation sigma = <p/g> (DESIGN.md
+    reading A22).  Implemented for the processes whose records are products of independent objects."""
+    if process != TTH_DILEP:
+        raise ValueError("event_density: process %r has correlated fields" % (process,))
+    g = np.ones(ev.shape[1])
+    for k in range(2):                                       # leptons: pT = 20 + Exp(40)
+        g *= np.exp(-(ev[3 * k] - 20.0) / 40.0) / 40.0 / 5.0 / (2.0 * np.pi)
+    for k in range(4):                                       # jets: E = 30 + Exp(60)
+        g *= np.exp(-(ev[6 + 3 * k] - 30.0) / 60.0) / 60.0 / 5.0 / (2.0 * np.pi)
+    return g
 
 
 def shard_range(n_events: int, rank: int, world: int):
@@ -143,6 +164,59 @@ def make_parton_events(n_events: int, seed: int = DEFAULT_SEED, sqrt_s: float = 
     q, qb = _two_body(r, W2, np.zeros(n), np.zeros(n))
     ev = np.concatenate([lep, nu, b_had, b_lep, q, qb], axis=0)
     return np.ascontiguousarray(ev, dtype=np.float64)
+
+
+def _smear_jet(r, E, w_tail=0.3, mu1=0.0, sig1=0.15, mu2=-0.1, sig2=0.35):
+    """measured jet energy for parton energy E: a draw from the double-Gaussian shape BASELINE.json:configs[1]
+    states (mixture of two normals in (E_jet - E)/E); pure sampling, the TF itself lives in the kernels"""
+    n = E.shape[0]
+    tail = r.random(n) < w_tail
+    u1, u2 = r.random(n), r.random(n)
+    g = np.sqrt(-2.0 * np.log1p(-u1)) * np.cos(2.0 * np.pi * u2)
+    return E * (1.0 + np.where(tail, mu2 + sig2 * g, mu1 + sig1 * g))
+
+
+def _eta_phi(p):
+    pt = np.hypot(p[1], p[2])
+    return np.arcsinh(p[3] / pt), np.mod(np.arctan2(p[2], p[1]), 2.0 * np.pi)
+
+
+def make_tth_events(n_events: int, seed: int = DEFAULT_SEED, resonant: bool = True, smear: bool = True,
+                    m_H: float = 125.0, m_t: float = 173.0, Gam_t: float = 1.4, m_W: float = 80.4,
+                    Gam_W: float = 2.09, sqrt_s: float = 14000.0, return_truth: bool = False):
+    """NEXT-4 closure sample, [18, n_events] records of MEM_PROC_TTH_DILEP built from physical
+    t tbar (b bbar) kinematics: s-hat -> (t tbar)(bb) -> t, tbar, b1 b2 by isotropic two-body steps,
+    Breit-Wigner top and W masses, dileptonic decays, jets smeared with the double Gaussian.
+    resonant: m_bb = m_H (signal-like); otherwise m_bb log-uniform in [20, 300] GeV (background-like).
+    Stands in for the paper's MadGraph+Pythia t tbar H / t tbar b bbar samples."""
+    r = np.random.Generator(np.random.PCG64([int(seed), 1407, 9 if resonant else 10]))
+    n = int(n_events)
+    mt1, mt2 = _breit_wigner(r, n, m_t, Gam_t, 15.0), _breit_wigner(r, n, m_t, Gam_t, 15.0)
+    mw1, mw2 = _breit_wigner(r, n, m_W, Gam_W, 15.0), _breit_wigner(r, n, m_W, Gam_W, 15.0)
+    mbb = np.full(n, m_H) if resonant else 20.0 * np.exp(np.log(15.0) * r.random(n))
+    mtt = mt1 + mt2 + 20.0 + _exp(r.random(n), 120.0)
+    rs = mtt + mbb + 20.0 + _exp(r.random(n), 150.0)
+    y = -1.5 + 3.0 * r.random(n)
+    rs = np.minimum(rs, 0.9 * sqrt_s * np.exp(-np.abs(y)))
+    P = np.stack([rs * np.cosh(y), np.zeros(n), np.zeros(n), rs * np.sinh(y)])
+    TT, H = _two_body(r, P, mtt, mbb)
+    t, tb = _two_body(r, TT, mt1, mt2)
+    W1, b = _two_body(r, t, mw1, np.zeros(n))
+    lp, nu = _two_body(r, W1, np.zeros(n), np.zeros(n))
+    W2, bb = _two_body(r, tb, mw2, np.zeros(n))
+    lm, nub = _two_body(r, W2, np.zeros(n), np.zeros(n))
+    b1, b2 = _two_body(r, H, np.zeros(n), np.zeros(n))
+    rows = []
+    for l in (lp, lm):
+        eta, phi = _eta_phi(l)
+        rows += [np.hypot(l[1], l[2]), eta, phi]
+    for j in (b, bb, b1, b2):
+        eta, phi = _eta_phi(j)
+        rows += [_smear_jet(r, j[0]) if smear else j[0].copy(), eta, phi]
+    ev = np.ascontiguousarray(np.stack(rows, axis=0), dtype=np.float64)
+    if return_truth:
+        return ev, dict(lp=lp, nu=nu, b=b, lm=lm, nub=nub, bb=bb, b1=b1, b2=b2)
+    return ev
 
 
 # ------------------------------------------------------------------------------------------
