@@ -43,7 +43,14 @@ typedef enum {
   MEM_PROC_W_ENU = 1,    /* u dbar -> W+ -> e+ nu,            D = 1,  5 record fields */
   MEM_PROC_Z_BB = 2,     /* q qbar -> Z -> b bbar,            D = 2,  6 record fields */
   MEM_PROC_TT_LJETS = 3, /* t tbar -> b l nu bbar q qbar',    D = 6, 17 record fields */
-  MEM_PROC_TT_DILEP = 4  /* t tbar -> b l+ nu bbar l- nubar,  D = 8, 14 record fields */
+  MEM_PROC_TT_DILEP = 4, /* t tbar -> b l+ nu bbar l- nubar,  D = 8, 14 record fields */
+  /* NEXT-4, the paper's own benchmark integral (PAPER.md:101-109 Eq. 7, :111-118 Eq. 8, :120-137 Eq. 9, :178-180
+   * Eq. 11): t tbar H(-> b bbar), both tops leptonic, four b jets.  Record = (pT, eta, phi) of l+ and l-, then
+   * (E, eta, phi) of the jets taken as b (pairs with l+), bbar (pairs with l-), b1, b2 (Higgs candidates); no MET
+   * field: Eq. 11 defines the neutrinos' total transverse momentum from the partons of each point.  Dimensions:
+   * E_b, E_bbar, the Breit-Wigner mapped s_W+, s_t, s_W-, s_tbar, and Eq. 9's (m_H^2, f = E1 + E2) with both
+   * orderings of its inverse summed.  mem_params.tth_hyp selects the hypothesis of Eq. 10. */
+  MEM_PROC_TTH_DILEP = 5 /* t tbar H -> b l+ nu bbar l- nubar b bbar, D = 8, 18 record fields */
 } mem_process;
 
 /* All physics constants, integration windows and VEGAS options (DESIGN.md
@@ -71,13 +78,20 @@ typedef struct mem_params {
   int32_t n_perm;            /* jet-parton assignments summed per point (Eq. 7 "sum over all
                               * permutations of assigning measured jets to partons"): 0 or 1 = record order only;
                               * MEM_PROC_TT_LJETS: 4 = b-tags known (b jets swapped x light jets swapped), 24 = all;
-                              * MEM_PROC_TT_DILEP: 2 = both b assignments.  Anything else: MEM_ERR_INVALID_ARG. */
+                              * MEM_PROC_TT_DILEP: 2 = both b assignments; MEM_PROC_TTH_DILEP: 12 = the 4!/2
+                              * distinct assignments of four b jets to (b, bbar, {b1, b2}).
+                              * Anything else: MEM_ERR_INVALID_ARG. */
+  /* NEXT-4 (MEM_PROC_TTH_DILEP only; readings A20, A21) */
+  double m_H, Gam_H;         /* Higgs mass and width: Breit-Wigner map of Eq. 9's m_H^2, window m +- n Gamma */
+  double yuk_t, yuk_b;       /* Yukawa couplings of the factorised t tbar H matrix element */
+  int32_t tth_hyp;           /* hypothesis of Eq. 10: 0 = t tbar H(-> b bbar), 1 = non-resonant t tbar b bbar stand-in */
+  int32_t reserved0;         /* must be 0 */
 } mem_params;
 
 /* Fill *params with the defaults of `process` (precision 64, plain MC). */
 mem_status mem_params_default(mem_process process, mem_params* params /* host, out */);
 
-/* Record fields per event (5 / 6 / 17 / 14) and integration dimensions (1 / 2 / 6 / 8);
+/* Record fields per event (5 / 6 / 17 / 14 / 18) and integration dimensions (1 / 2 / 6 / 8 / 8);
  * -1 for an unknown process. */
 int32_t mem_event_fields(mem_process process);
 int32_t mem_n_dims(mem_process process);
@@ -159,6 +173,19 @@ mem_status mem_set_pdf_grid(mem_handle* h, const double* table, int32_t nx, int3
  * MEM_PROC_TT_LJETS handles with precision 64 only (MEM_ERR_UNSUPPORTED otherwise). */
 mem_status mem_eval_parton(mem_handle* h, const double* momenta, int64_t n_events, double* out_w,
                            void* cuda_stream);
+
+/* Post-processing of the likelihoods (PAPER.md:45 Eq. 1 "sigma is the overall normalization", :143 Eq. 10
+ * "D = log10(p_ttH / p_ttbb)"; reading A22).
+ * mem_normalisation: sigma = (1/n) sum_e p[e] / g[e], the importance-sampled acceptance integral of the
+ *   likelihood over events drawn from the density g (one fixed-order reduction, result reproducible).
+ *   p, g : device, float64 [n], read-only;  out_sigma : device, float64 [1].
+ * mem_discriminant: out_D[e] = log10((p_sig[e] / sigma_sig[0]) / (p_bkg[e] / sigma_bkg[0])).
+ *   p_sig, p_bkg : device, float64 [n];  sigma_sig, sigma_bkg : device, float64 [1];  out_D : device [n].
+ * Both are asynchronous on cuda_stream, need no handle and never synchronise.  n < 1 (normalisation) or
+ * n < 0 (discriminant), NULL or misaligned pointers: MEM_ERR_INVALID_ARG. */
+mem_status mem_normalisation(const double* p, const double* g, int64_t n, double* out_sigma, void* cuda_stream);
+mem_status mem_discriminant(const double* p_sig, const double* p_bkg, int64_t n, const double* sigma_sig,
+                            const double* sigma_bkg, double* out_D, void* cuda_stream);
 
 /* Diagnostic: copy the VEGAS grids left by the last mem_integrate with
  * vegas_iters > 0 into out_grid (device, float64 [n_events][D][vegas_bins+1]). */

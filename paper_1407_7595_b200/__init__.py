@@ -15,12 +15,12 @@ from . import build as _build
 from . import workloads  # noqa: F401  (seeded input generators; no arithmetic of the method)
 
 MEM_OK, MEM_ERR_INVALID_ARG, MEM_ERR_UNSUPPORTED, MEM_ERR_CUDA, MEM_ERR_NOMEM = 0, 1, 2, 3, 4
-MEM_PROC_W_ENU, MEM_PROC_Z_BB, MEM_PROC_TT_LJETS, MEM_PROC_TT_DILEP = 1, 2, 3, 4
+MEM_PROC_W_ENU, MEM_PROC_Z_BB, MEM_PROC_TT_LJETS, MEM_PROC_TT_DILEP, MEM_PROC_TTH_DILEP = 1, 2, 3, 4, 5
 
 EXPORTS = ("mem_params_default", "mem_event_fields", "mem_n_dims", "mem_create", "mem_destroy",
            "mem_set_event_offset", "mem_integrate", "mem_integrate_host", "mem_eval_points",
            "mem_eval_parton", "mem_set_pdf_grid", "mem_get_grid", "mem_launch_count", "mem_last_error", "mem_last_pass_ms", "mem_measure_fp64_peak",
-           "mem_measure_fp64_peak_rrr", "mem_measure_fp64_rate")
+           "mem_measure_fp64_peak_rrr", "mem_measure_fp64_rate", "mem_normalisation", "mem_discriminant")
 
 
 class mem_params(C.Structure):
@@ -32,7 +32,9 @@ class mem_params(C.Structure):
                     "tf_w_tail", "tf_mu1", "tf_sig1", "tf_mu2", "tf_sig2", "jetE_rlo", "jetE_rhi",
                     "bw_nwidths", "nu_pz_max", "nu_eta_max", "met_sigma", "met_nsigma", "vegas_alpha")] +
                 [("vegas_points", C.c_int64), ("vegas_iters", C.c_int32), ("vegas_bins", C.c_int32),
-                 ("n_flav", C.c_int32), ("n_perm", C.c_int32)])
+                 ("n_flav", C.c_int32), ("n_perm", C.c_int32),
+                 ("m_H", C.c_double), ("Gam_H", C.c_double), ("yuk_t", C.c_double), ("yuk_b", C.c_double),
+                 ("tth_hyp", C.c_int32), ("reserved0", C.c_int32)])
 
 
 class MemError(RuntimeError):
@@ -74,6 +76,8 @@ def lib():
         L.mem_measure_fp64_peak.argtypes = [C.c_int32, C.POINTER(C.c_double), vp]
         L.mem_measure_fp64_peak_rrr.argtypes = [C.c_int32, C.POINTER(C.c_double), vp]
         L.mem_measure_fp64_rate.argtypes = [C.c_int32, C.c_int32, C.POINTER(C.c_double), vp]
+        L.mem_normalisation.argtypes = [dp, dp, i64, dp, vp]
+        L.mem_discriminant.argtypes = [dp, dp, i64, dp, dp, dp, vp]
         L.mem_last_error.argtypes = []
         L.mem_last_error.restype = C.c_char_p
         _lib = L
@@ -234,6 +238,29 @@ def mem_eval_parton(handle, momenta, out_w=None, stream=None):
     _check(lib().mem_eval_parton(handle, _dev_f64(momenta, "momenta"), n_events,
                                  _dev_f64(out_w, "out_w", (n_events,)), _stream_ptr(stream)))
     return out_w
+
+
+def mem_normalisation(p, g, out_sigma=None, stream=None):
+    """sigma = mean(p / g) over events drawn from the density g (reading A22): CUDA tensor [1]."""
+    import torch
+    n = int(p.shape[0])
+    if out_sigma is None:
+        out_sigma = torch.empty(1, dtype=torch.float64, device=p.device)
+    _check(lib().mem_normalisation(_dev_f64(p, "p", (n,)), _dev_f64(g, "g", (n,)), n, _dev_f64(out_sigma, "out_sigma", (1,)),
+                                   _stream_ptr(stream)))
+    return out_sigma
+
+
+def mem_discriminant(p_sig, p_bkg, sigma_sig, sigma_bkg, out_D=None, stream=None):
+    """D = log10((p_sig / sigma_sig) / (p_bkg / sigma_bkg)) per event (Eq. 10): CUDA tensor [n]."""
+    import torch
+    n = int(p_sig.shape[0])
+    if out_D is None:
+        out_D = torch.empty(n, dtype=torch.float64, device=p_sig.device)
+    _check(lib().mem_discriminant(_dev_f64(p_sig, "p_sig", (n,)), _dev_f64(p_bkg, "p_bkg", (n,)), n,
+                                  _dev_f64(sigma_sig, "sigma_sig", (1,)), _dev_f64(sigma_bkg, "sigma_bkg", (1,)),
+                                  _dev_f64(out_D, "out_D", (n,)), _stream_ptr(stream)))
+    return out_D
 
 
 def mem_get_grid(handle, n_events: int, n_dims: int, bins: int, device=None, stream=None):

@@ -40,6 +40,7 @@ int n_fields_of(int process) {
     case MEM_PROC_Z_BB: return 6;
     case MEM_PROC_TT_LJETS: return 17;
     case MEM_PROC_TT_DILEP: return 14;
+    case MEM_PROC_TTH_DILEP: return 18;
   }
   return -1;
 }
@@ -49,6 +50,7 @@ int n_dims_of(int process) {
     case MEM_PROC_Z_BB: return 2;
     case MEM_PROC_TT_LJETS: return 6;
     case MEM_PROC_TT_DILEP: return 8;
+    case MEM_PROC_TTH_DILEP: return 8;
   }
   return -1;
 }
@@ -58,6 +60,7 @@ int n_consts_of(int process) {
     case MEM_PROC_Z_BB: return ProcZbb::NC;
     case MEM_PROC_TT_LJETS: return ProcTTljets::NC;
     case MEM_PROC_TT_DILEP: return ProcTTdilep::NC;
+    case MEM_PROC_TTH_DILEP: return ProcTTHdilep::NC;
   }
   return -1;
 }
@@ -155,6 +158,15 @@ DevConst make_dev_const(const mem_params& p) {
   c.met_sigma = p.met_sigma; c.met_nsigma = p.met_nsigma;
   c.vegas_bins = p.vegas_bins; c.vegas_alpha = p.vegas_alpha;
   c.n_perm = p.n_perm > 1 ? p.n_perm : 1;
+  // NEXT-4 (mem_tth.cuh; readings A20, A21)
+  c.rhi = p.jetE_rhi; c.lnr = 2.0 * std::log(p.jetE_rhi / p.jetE_rlo);
+  c.mH2 = p.m_H * p.m_H; c.mHGH = p.m_H * p.Gam_H;
+  bw_window(p.m_H, p.Gam_H, p.bw_nwidths, &c.tH_lo, &c.tH_dt);
+  c.tth_hyp = p.tth_hyp;
+  // hypothesis 0: dt_H (ds/dt D_H = 1/(m_H Gam_H)) y_t^2 4 m_t^2 (eikonal scalar emission) 3 y_b^2 2 (H -> b bbar; k^2 stays);
+  // hypothesis 1: ln(s_hi/s_lo) (ds/du = s ln) g_s^2 (eikonal vector emission) (1/k^4) g_s^2 k^2 (splitting) -> constant
+  c.tth_c = p.tth_hyp ? c.lnr * gs2 * gs2
+                      : c.tH_dt / c.mHGH * (p.yuk_t * p.yuk_t * 4.0 * p.m_t * p.m_t) * (3.0 * p.yuk_b * p.yuk_b * 2.0);
   c.pdf_tab = nullptr; c.pdf_nx = 0; c.pdf_lxmin = c.pdf_dx = c.pdf_inv_dx = 0.0;
   return c;
 }
@@ -166,8 +178,9 @@ DevConstF to_float(const DevConst& d) {
   CP(tf_a1); CP(tf_b1); CP(tf_c1); CP(tf_a2); CP(tf_b2); CP(tf_c2); CP(mW); CP(GW); CP(mW2); CP(mWGW); CP(mWGW2);
   CP(tW_lo); CP(tW_dt); CP(mt2); CP(mtGt); CP(mtGt2); CP(tT_lo); CP(tT_dt); CP(mZ2); CP(mZGZ2); CP(g4w); CP(gz4);
   CP(gs4); CP(V_ud2); CP(V_tb2); CP(z_cu); CP(z_ct); CP(nu_pz_max); CP(nu_eta_max); CP(met_sigma); CP(met_nsigma);
-  CP(vegas_alpha);
+  CP(vegas_alpha); CP(rhi); CP(mH2); CP(mHGH); CP(tH_lo); CP(tH_dt); CP(lnr); CP(tth_c);
 #undef CP
+  f.tth_hyp = d.tth_hyp;
   f.pdf_fast = d.pdf_fast; f.n_flav = d.n_flav; f.vegas_bins = d.vegas_bins; f.n_perm = d.n_perm;
   f.pdf_tab = nullptr; f.pdf_nx = 0; f.pdf_lxmin = f.pdf_dx = f.pdf_inv_dx = 0.0;      // grid PDFs are fp64 only
   return f;
@@ -211,6 +224,11 @@ mem_status check_params(int process, const mem_params& p) {
   if (p.n_flav < 1 || p.n_flav > 5) return fail(MEM_ERR_INVALID_ARG, "n_flav outside 1..5");
   if (p.bw_nwidths * p.Gam_W >= p.m_W || p.bw_nwidths * p.Gam_t >= p.m_t)
     return fail(MEM_ERR_INVALID_ARG, "bw_nwidths * Gamma must stay below the mass");
+  if (process == MEM_PROC_TTH_DILEP) {
+    if (!(p.m_H > 0 && p.Gam_H > 0 && p.yuk_t > 0 && p.yuk_b > 0)) return fail(MEM_ERR_INVALID_ARG, "m_H, Gam_H, yuk_t, yuk_b must be positive");
+    if (p.bw_nwidths * p.Gam_H >= p.m_H) return fail(MEM_ERR_INVALID_ARG, "bw_nwidths * Gam_H must stay below m_H");
+    if (p.tth_hyp != 0 && p.tth_hyp != 1) return fail(MEM_ERR_INVALID_ARG, "tth_hyp must be 0 or 1");
+  }
   if (p.vegas_iters < 0 || p.vegas_iters > 255) return fail(MEM_ERR_INVALID_ARG, "vegas_iters outside 0..255");
   if (p.vegas_iters > 0) {
     if (p.vegas_bins < 1 || p.vegas_bins > kMaxBins) return fail(MEM_ERR_INVALID_ARG, "vegas_bins outside 1..%d", kMaxBins);
@@ -219,7 +237,8 @@ mem_status check_params(int process, const mem_params& p) {
   }
   const bool perm_ok = p.n_perm == 0 || p.n_perm == 1 ||
                        (process == MEM_PROC_TT_LJETS && (p.n_perm == 4 || p.n_perm == 24)) ||
-                       (process == MEM_PROC_TT_DILEP && p.n_perm == 2);
+                       (process == MEM_PROC_TT_DILEP && p.n_perm == 2) ||
+                       (process == MEM_PROC_TTH_DILEP && p.n_perm == 12);
   if (!perm_ok) return fail(MEM_ERR_INVALID_ARG, "n_perm = %d is not defined for process %d", p.n_perm, process);
   return MEM_OK;
 }
@@ -383,6 +402,11 @@ mem_status mem_params_default(mem_process process, mem_params* p) {
   p->nu_eta_max = 5.0; p->met_sigma = 10.0; p->met_nsigma = 4.0;
   p->vegas_alpha = 0.5; p->vegas_points = 1 << 17; p->vegas_iters = 0; p->vegas_bins = 50;      // configs[4]
   p->n_flav = (process == MEM_PROC_Z_BB) ? 3 : 5;            // configs[1]
+  // NEXT-4 (reading A21; the paper gives none): m_H = 125, Gamma_H = 4.07 MeV, y_f = m_f sqrt(2 sqrt2 G_F), m_b = 4.18
+  p->m_H = 125.0; p->Gam_H = 0.00407;
+  p->yuk_t = p->m_t * std::sqrt(2.0 * std::sqrt(2.0) * p->G_F);
+  p->yuk_b = 4.18 * std::sqrt(2.0 * std::sqrt(2.0) * p->G_F);
+  p->tth_hyp = 0;
   return MEM_OK;
 }
 
@@ -526,6 +550,7 @@ mem_status mem_integrate(mem_handle* h, const double* events, int64_t n_events, 
         return integrate_impl<ProcTTljetsF>(h, events, n_events, n_points, seed, out_p, out_err, st);
       return integrate_impl<ProcTTljets>(h, events, n_events, n_points, seed, out_p, out_err, st);
     case MEM_PROC_TT_DILEP: return integrate_impl<ProcTTdilep>(h, events, n_events, n_points, seed, out_p, out_err, st);
+    case MEM_PROC_TTH_DILEP: return integrate_impl<ProcTTHdilep>(h, events, n_events, n_points, seed, out_p, out_err, st);
   }
   return fail(MEM_ERR_UNSUPPORTED, "process %d is not implemented", h->process);
 }
@@ -576,6 +601,7 @@ mem_status mem_eval_points(mem_handle* h, const double* events, int64_t n_events
         return eval_impl<ProcTTljetsF>(h, events, n_events, event, first_point, n, seed, iteration, grid, out_w, st);
       return eval_impl<ProcTTljets>(h, events, n_events, event, first_point, n, seed, iteration, grid, out_w, st);
     case MEM_PROC_TT_DILEP: return eval_impl<ProcTTdilep>(h, events, n_events, event, first_point, n, seed, iteration, grid, out_w, st);
+    case MEM_PROC_TTH_DILEP: return eval_impl<ProcTTHdilep>(h, events, n_events, event, first_point, n, seed, iteration, grid, out_w, st);
   }
   return fail(MEM_ERR_UNSUPPORTED, "process %d is not implemented", h->process);
 }
@@ -587,7 +613,8 @@ mem_status mem_set_pdf_grid(mem_handle* h, const double* table, int32_t nx, int3
     h->dc.pdf_tab = nullptr;
     return MEM_OK;
   }
-  if ((h->process != MEM_PROC_TT_LJETS && h->process != MEM_PROC_TT_DILEP) || h->params.precision != 64)
+  if ((h->process != MEM_PROC_TT_LJETS && h->process != MEM_PROC_TT_DILEP && h->process != MEM_PROC_TTH_DILEP) ||
+      h->params.precision != 64)
     return fail(MEM_ERR_UNSUPPORTED, "grid PDFs are implemented for the t tbar processes in fp64");
   if (nx < 2 || nq < 2 || nx > 65536 || nq > 65536) return fail(MEM_ERR_INVALID_ARG, "nx, nq outside 2..65536");
   if (!(lxmax > lxmin) || !(lqmax > lqmin) || !(Q > 0.0)) return fail(MEM_ERR_INVALID_ARG, "empty grid range or Q <= 0");
@@ -634,6 +661,29 @@ mem_status mem_eval_parton(mem_handle* h, const double* momenta, int64_t n_event
   if (blocks > 0x7fffffffLL) return fail(MEM_ERR_INVALID_ARG, "n_events exceeds the grid limit");
   parton_ttljets_kernel<<<(unsigned)blocks, threads, 0, (cudaStream_t)cuda_stream>>>(h->dc, momenta, n_events, out_w);
   ++h->launches;
+  CUDA_TRY(cudaGetLastError());
+  return MEM_OK;
+}
+
+mem_status mem_normalisation(const double* p, const double* g, int64_t n, double* out_sigma, void* cuda_stream) {
+  if (n < 1) return fail(MEM_ERR_INVALID_ARG, "n < 1");
+  if (!p || !g || !out_sigma) return fail(MEM_ERR_INVALID_ARG, "p / g / out_sigma is NULL");
+  if (!aligned8(p) || !aligned8(g) || !aligned8(out_sigma)) return fail(MEM_ERR_INVALID_ARG, "device pointers must be 8-byte aligned");
+  normalisation_kernel<<<1, kThreads, 0, (cudaStream_t)cuda_stream>>>(p, g, n, out_sigma);
+  CUDA_TRY(cudaGetLastError());
+  return MEM_OK;
+}
+
+mem_status mem_discriminant(const double* p_sig, const double* p_bkg, int64_t n, const double* sigma_sig,
+                            const double* sigma_bkg, double* out_D, void* cuda_stream) {
+  if (n < 0) return fail(MEM_ERR_INVALID_ARG, "n < 0");
+  if (n == 0) return MEM_OK;
+  if (!p_sig || !p_bkg || !sigma_sig || !sigma_bkg || !out_D) return fail(MEM_ERR_INVALID_ARG, "a pointer is NULL");
+  if (!aligned8(p_sig) || !aligned8(p_bkg) || !aligned8(sigma_sig) || !aligned8(sigma_bkg) || !aligned8(out_D))
+    return fail(MEM_ERR_INVALID_ARG, "device pointers must be 8-byte aligned");
+  const int64_t blocks = (n + 255) / 256;
+  if (blocks > 0x7fffffffLL) return fail(MEM_ERR_INVALID_ARG, "n exceeds the grid limit");
+  discriminant_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>(p_sig, p_bkg, n, sigma_sig, sigma_bkg, out_D);
   CUDA_TRY(cudaGetLastError());
   return MEM_OK;
 }

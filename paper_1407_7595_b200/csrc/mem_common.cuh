@@ -52,6 +52,10 @@ struct DevConstR {
   int vegas_bins;
   T vegas_alpha;
   int n_perm;                      // jet-parton assignments summed per point (>= 1)
+  // NEXT-4 (mem_tth.cuh): upper edge of the parton-energy window, Higgs Breit-Wigner data, 2 ln(rhi/rlo),
+  // hypothesis (0 = t tbar H, 1 = non-resonant t tbar b bbar) and every constant factor of the radiated system
+  T rhi, mH2, mHGH, tH_lo, tH_dt, lnr, tth_c;
+  int tth_hyp;
   // NEXT-3 grid PDFs: tables already interpolated in ln Q at the handle's fixed scale, [6][pdf_nx]
   // (species 0 = g, 1..5 = d,u,s,c,b), sample i at pdf_lxmin + i pdf_dx; nullptr = toy PDF
   const double* pdf_tab;

@@ -7,6 +7,7 @@
 //   eval_points_kernel  diagnostic: one thread per point, writes w
 #pragma once
 #include "mem_processes.cuh"
+#include "mem_tth.cuh"
 
 namespace memb200 {
 

@@ -27,7 +27,7 @@ def test_library_builds_and_exports_every_declared_symbol():
 
 
 def test_params_struct_matches_header_and_defaults():
-    for proc, nf, nd in ((1, 5, 1), (2, 6, 2), (3, 17, 6), (4, 14, 8)):
+    for proc, nf, nd in ((1, 5, 1), (2, 6, 2), (3, 17, 6), (4, 14, 8), (5, 18, 8)):
         p = mem.mem_params_default(proc)
         assert p.struct_size == C.sizeof(mem.mem_params)
         assert p.precision == 64 and p.vegas_iters == 0 and p.vegas_bins == 50
@@ -35,6 +35,7 @@ def test_params_struct_matches_header_and_defaults():
         assert (p.tf_w_tail, p.tf_sig1, p.tf_mu2, p.tf_sig2) == (0.3, 0.15, -0.1, 0.35)
         assert p.n_flav == (3 if proc == 2 else 5)
         assert mem.mem_event_fields(proc) == nf and mem.mem_n_dims(proc) == nd
+        assert (p.m_H, p.Gam_H, p.tth_hyp, p.reserved0) == (125.0, 0.00407, 0, 0) and 0.99 < p.yuk_t < 1.0    # reading A21
     assert mem.mem_event_fields(7) == -1
     with pytest.raises(mem.MemError):
         mem.mem_params_default(0)
