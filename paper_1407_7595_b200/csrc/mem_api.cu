@@ -220,6 +220,11 @@ mem_status check_params(int process, const mem_params& p) {
     }
     if (!(gmax < 600.0))
       return fail(MEM_ERR_INVALID_ARG, "jet TF: core Gaussian too narrow for the parton-energy window (z1^2 - z2^2 reaches %.0f)", gmax);
+    // the kernels' inner exponentials (exp_tab<false>, no range check) see z1^2 - z2^2: bounded above by gmax and
+    // below by -max z2^2; the outer exponential exp(-sum z1^2 ...) is range checked (it may legitimately underflow)
+    const double z2max = std::fmax(std::fabs(a2 * v_lo + b2), std::fabs(a2 * v_hi + b2));
+    if (!(z2max * z2max < 600.0))
+      return fail(MEM_ERR_INVALID_ARG, "jet TF: tail Gaussian too narrow for the parton-energy window (z2^2 reaches %.0f)", z2max * z2max);
   }
   if (p.n_flav < 1 || p.n_flav > 5) return fail(MEM_ERR_INVALID_ARG, "n_flav outside 1..5");
   if (p.bw_nwidths * p.Gam_W >= p.m_W || p.bw_nwidths * p.Gam_t >= p.m_t)
@@ -276,7 +281,7 @@ mem_status launch_pass(mem_handle* h, int64_t n_events, int64_t n_points, int64_
   auto launch = [&](auto perm, auto grid) {
     integrate_kernel<P, MODE, decltype(perm)::value, decltype(grid)::value><<<(unsigned)blocks, kThreads, smem, st>>>(
         dc_of<typename P::real>(h), (const double*)h->ecs.p, (const double*)h->grids.p, (double*)h->partials.p,
-        (double*)h->hist.p, n_points, chunk, n_chunks, seed, h->event_offset, pass);
+        (double*)h->hist.p, n_points, chunk, n_chunks, make_philox(seed), h->event_offset, pass);
   };
   const bool perm = h->dc.n_perm > 1, grid = h->dc.pdf_tab != nullptr;
   if (perm && grid) launch(std::true_type{}, std::true_type{});
@@ -369,7 +374,7 @@ mem_status eval_impl(mem_handle* h, const double* events, int64_t n_events, int6
   const int threads = 128;
   const size_t smem = ((size_t)P::NC * h->dc.n_perm + (size_t)P::D * (kMaxBins + 1)) * sizeof(double);
   eval_points_kernel<P><<<(unsigned)((n + threads - 1) / threads), threads, smem, st>>>(
-      dc_of<typename P::real>(h), (const double*)h->ecs.p, event, grid, first, n, seed, h->event_offset, (uint32_t)iteration, out_w);
+      dc_of<typename P::real>(h), (const double*)h->ecs.p, event, grid, first, n, make_philox(seed), h->event_offset, (uint32_t)iteration, out_w);
   ++h->launches;
   CUDA_TRY(cudaGetLastError());
   return MEM_OK;

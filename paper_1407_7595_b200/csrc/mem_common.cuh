@@ -68,28 +68,36 @@ using DevConstF = DevConstR<float>;   // fp32 integrand core of config 3 (readin
 // ---------------------------------------------------------------------------------------
 // S1. Philox4x32-10 (Salmon et al. 2011; multipliers and Weyl constants are the published ones)
 // ---------------------------------------------------------------------------------------
+// The ten round keys (key + r * Weyl constant) are formed once on the host (make_philox in mem_api.cu) and reach the
+// kernels as a by-value argument, i.e. as constant-bank operands of the round's XOR: no key arithmetic in the point loop.
+// Each round's two 32 x 32 -> 64 products are written as 64-bit multiplies (one IMAD.WIDE each, high and low word at once).
 struct Philox {
-  uint32_t k0, k1;                      // key = (seed low, seed high)
+  uint32_t ka[10], kb[10];              // round keys of key word 0 and key word 1
   __device__ __forceinline__ void operator()(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
                                              uint32_t (&out)[4]) const {
-    uint32_t a = k0, b = k1;
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
-      const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
-      const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
-      c0 = hi1 ^ c1 ^ a; c1 = lo1; c2 = hi0 ^ c3 ^ b; c3 = lo0;
-      a += 0x9E3779B9u; b += 0xBB67AE85u;
+      const uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
+      const uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0, hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+      c0 = hi1 ^ c1 ^ ka[r]; c1 = lo1; c2 = hi0 ^ c3 ^ kb[r]; c3 = lo0;
     }
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
   }
 };
+inline Philox make_philox(uint64_t seed) {
+  Philox p;
+  uint32_t a = (uint32_t)seed, b = (uint32_t)(seed >> 32);
+  for (int r = 0; r < 10; ++r) { p.ka[r] = a; p.kb[r] = b; a += 0x9E3779B9u; b += 0xBB67AE85u; }
+  return p;
+}
 
 // 52-bit uniform in (0,1): u = (k + 1/2) 2^-52, k = (a >> 6) 2^26 + (b >> 6).  Built without an
 // integer->double conversion: 1.k (binary) = 1 + k 2^-52 is assembled in the mantissa, and
 // adding -(1 - 2^-53) is exact because (2k + 1) 2^-53 is representable.
 __device__ __forceinline__ double u52(uint32_t a, uint32_t b) {
-  const uint32_t hi = 0x3FF00000u | (a >> 12);
-  const uint32_t lo = ((a >> 6) << 26) | (b >> 6);
+  const uint32_t A = a >> 6;
+  const uint32_t hi = 0x3FF00000u | (A >> 6);
+  const uint32_t lo = __funnelshift_r(b, A, 6);        // low word of ((A : b) >> 6) = (A << 26) | (b >> 6)
   return __hiloint2double((int)hi, (int)lo) + (-0x1.fffffffffffffp-1);
 }
 
@@ -137,6 +145,28 @@ __device__ __forceinline__ double rcp_fast(double x) {
   return fma(y, e, y);
 }
 
+// 1/sqrt(x) for normal, finite, positive x: MUFU seed (relative error ~2^-20) -> one cubic step
+// y (1 + e/2 + 3 e^2/8), e = 1 - x y^2 (error ~e^3) -> one linear step; about 1 ulp, no special-case branch.
+__device__ __forceinline__ double rsqrt_fast(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double e = fma(-x * y, y, 1.0);
+  y = fma(y * e, fma(0.375, e, 0.5), y);
+  e = fma(-x * y, y, 1.0);
+  return fma(0.5 * y, e, y);
+}
+
+// Polynomial coefficients live in the constant bank (c[3][..] operands of DFMA): as 64-bit literals each costs two
+// UMOVs per use inside the point loop (there are more of them than uniform registers to hoist them into), and a
+// DFMA with a constant-bank operand issues at the full FP64 rate (profiles/r01_microbench.md).
+__constant__ double kTanS[6] = {-0x1.5555555555554p-3, 0x1.1111111110a86p-7, -0x1.a01a019e3e0afp-13,
+                                0x1.71de373e0fee6p-19, -0x1.ae5fb0a5df712p-26, 0x1.5deb31d167e93p-33};
+__constant__ double kTanC[6] = {0x1.5555555555555p-5, -0x1.6c16c16c168d0p-10, 0x1.a01a019f2bd7bp-16,
+                                -0x1.27e4f9eb9238ep-22, 0x1.1eeb3bafbb15dp-29, -0x1.905db35e3086ap-37};
+// exp_tab: 256/ln2, the rounding constant 1.5 2^52, -ln2/256 in two parts, 1/24, 1/6, 1/2
+__constant__ double kExpC[7] = {0x1.71547652b82fep+8, 6755399441055744.0, -0x1.62e42fee00000p-9, -0x1.a39ef35793c76p-41,
+                                1.0 / 24.0, 1.0 / 6.0, 0.5};
+
 // tan(t) for the Breit-Wigner maps (O6): t = atan(..) lies strictly inside (-pi/2, pi/2), so no
 // general range reduction (and none of libdevice's large-argument path) is needed.  |t| <= pi/4:
 // tan = S(t)/C(t); otherwise with r = pi/2 - |t| (pi/2 in two parts): tan = C(r)/S(r).  S, C are
@@ -145,10 +175,8 @@ __device__ __forceinline__ double rcp_fast(double x) {
 // the Horner steps interleaved so that each coefficient is fetched once for all of them.
 template <int N>
 __device__ __forceinline__ void tan_bw_n(const double (&t)[N], double (&out)[N]) {
-  constexpr double kS[6] = {-0x1.5555555555554p-3, 0x1.1111111110a86p-7, -0x1.a01a019e3e0afp-13,
-                            0x1.71de373e0fee6p-19, -0x1.ae5fb0a5df712p-26, 0x1.5deb31d167e93p-33};
-  constexpr double kC[6] = {0x1.5555555555555p-5, -0x1.6c16c16c168d0p-10, 0x1.a01a019f2bd7bp-16,
-                            -0x1.27e4f9eb9238ep-22, 0x1.1eeb3bafbb15dp-29, -0x1.905db35e3086ap-37};
+  const double* kS = kTanS;
+  const double* kC = kTanC;
   double r[N], z[N], ps[N], pc[N];
   bool big[N];
 #pragma unroll
@@ -175,8 +203,7 @@ __device__ __forceinline__ void tan_bw_n(const double (&t)[N], double (&out)[N])
 // cos(x) for 0 <= x <= pi/3 (the trigonometric form of the resolvent cubic): 1 - 2 sin^2(x/2) with the
 // sine polynomial of tan_bw_n on |x/2| <= pi/6; no range reduction, no large-argument path.
 __device__ __forceinline__ double cos_third(double x) {
-  constexpr double kS[6] = {-0x1.5555555555554p-3, 0x1.1111111110a86p-7, -0x1.a01a019e3e0afp-13,
-                            0x1.71de373e0fee6p-19, -0x1.ae5fb0a5df712p-26, 0x1.5deb31d167e93p-33};
+  const double* kS = kTanS;
   const double h = 0.5 * x, z = h * h;
   double ps = kS[5];
 #pragma unroll
@@ -192,43 +219,96 @@ __device__ __forceinline__ double tan_bw(double t) {
   return o[0];
 }
 
-// exp(x) for the hot loops: x = k ln2/64 + r with |r| <= ln2/128, exp(x) = 2^(k >> 6) * T[k & 63] * (1 + p(r)),
-// T[j] = 2^(j/64) (correctly rounded, own table), p = r + r^2 (1/2 + r (1/6 + r (1/24 + r/120))) (remainder
-// r^6/720 < 3.4e-17), 2^(k >> 6) through the exponent field.  10 FP64 instructions against libdevice's 17 per
-// call; about 1 ulp.  |x| >= 700 (or NaN) returns 0 or +inf without touching the exponent arithmetic.
-__device__ const double kExpTab[64] = {
-    0x1.0000000000000p+0, 0x1.02c9a3e778061p+0, 0x1.059b0d3158574p+0, 0x1.0874518759bc8p+0,
-    0x1.0b5586cf9890fp+0, 0x1.0e3ec32d3d1a2p+0, 0x1.11301d0125b51p+0, 0x1.1429aaea92de0p+0,
-    0x1.172b83c7d517bp+0, 0x1.1a35beb6fcb75p+0, 0x1.1d4873168b9aap+0, 0x1.2063b88628cd6p+0,
-    0x1.2387a6e756238p+0, 0x1.26b4565e27cddp+0, 0x1.29e9df51fdee1p+0, 0x1.2d285a6e4030bp+0,
-    0x1.306fe0a31b715p+0, 0x1.33c08b26416ffp+0, 0x1.371a7373aa9cbp+0, 0x1.3a7db34e59ff7p+0,
-    0x1.3dea64c123422p+0, 0x1.4160a21f72e2ap+0, 0x1.44e086061892dp+0, 0x1.486a2b5c13cd0p+0,
-    0x1.4bfdad5362a27p+0, 0x1.4f9b2769d2ca7p+0, 0x1.5342b569d4f82p+0, 0x1.56f4736b527dap+0,
-    0x1.5ab07dd485429p+0, 0x1.5e76f15ad2148p+0, 0x1.6247eb03a5585p+0, 0x1.6623882552225p+0,
-    0x1.6a09e667f3bcdp+0, 0x1.6dfb23c651a2fp+0, 0x1.71f75e8ec5f74p+0, 0x1.75feb564267c9p+0,
-    0x1.7a11473eb0187p+0, 0x1.7e2f336cf4e62p+0, 0x1.82589994cce13p+0, 0x1.868d99b4492edp+0,
-    0x1.8ace5422aa0dbp+0, 0x1.8f1ae99157736p+0, 0x1.93737b0cdc5e5p+0, 0x1.97d829fde4e50p+0,
-    0x1.9c49182a3f090p+0, 0x1.a0c667b5de565p+0, 0x1.a5503b23e255dp+0, 0x1.a9e6b5579fdbfp+0,
-    0x1.ae89f995ad3adp+0, 0x1.b33a2b84f15fbp+0, 0x1.b7f76f2fb5e47p+0, 0x1.bcc1e904bc1d2p+0,
-    0x1.c199bdd85529cp+0, 0x1.c67f12e57d14bp+0, 0x1.cb720dcef9069p+0, 0x1.d072d4a07897cp+0,
-    0x1.d5818dcfba487p+0, 0x1.da9e603db3285p+0, 0x1.dfc97337b9b5fp+0, 0x1.e502ee78b3ff6p+0,
-    0x1.ea4afa2a490dap+0, 0x1.efa1bee615a27p+0, 0x1.f50765b6e4540p+0, 0x1.fa7c1819e90d8p+0};
+// exp(x) for the hot loops: x = k ln2/256 + r with |r| <= ln2/512, exp(x) = 2^(k >> 8) * T[k & 255] * (1 + p(r)),
+// T[j] = 2^(j/256) (correctly rounded, own table), p = r + r^2 (1/2 + r (1/6 + r/24)) (remainder r^5/120 < 3.8e-17),
+// 2^(k >> 8) through the exponent field.  9 FP64 instructions against libdevice's 17 per call; about 1 ulp.
+// CHECK = false (the integrands): the caller guarantees |x| < 700 -- mem_create validates the transfer-function and
+// window parameters that bound every argument (mem_api.cu: check_params).  CHECK = true: |x| >= 700 (or NaN)
+// returns 0 or +inf without touching the exponent arithmetic.
+__device__ const double kExpTab[256] = {
+    0x1.0000000000000p+0, 0x1.00b1afa5abcbfp+0, 0x1.0163da9fb3335p+0, 0x1.02168143b0281p+0,
+    0x1.02c9a3e778061p+0, 0x1.037d42e11bbccp+0, 0x1.04315e86e7f85p+0, 0x1.04e5f72f654b1p+0,
+    0x1.059b0d3158574p+0, 0x1.0650a0e3c1f89p+0, 0x1.0706b29ddf6dep+0, 0x1.07bd42b72a836p+0,
+    0x1.0874518759bc8p+0, 0x1.092bdf66607e0p+0, 0x1.09e3ecac6f383p+0, 0x1.0a9c79b1f3919p+0,
+    0x1.0b5586cf9890fp+0, 0x1.0c0f145e46c85p+0, 0x1.0cc922b7247f7p+0, 0x1.0d83b23395decp+0,
+    0x1.0e3ec32d3d1a2p+0, 0x1.0efa55fdfa9c5p+0, 0x1.0fb66affed31bp+0, 0x1.1073028d7233ep+0,
+    0x1.11301d0125b51p+0, 0x1.11edbab5e2ab6p+0, 0x1.12abdc06c31ccp+0, 0x1.136a814f204abp+0,
+    0x1.1429aaea92de0p+0, 0x1.14e95934f312ep+0, 0x1.15a98c8a58e51p+0, 0x1.166a45471c3c2p+0,
+    0x1.172b83c7d517bp+0, 0x1.17ed48695bbc0p+0, 0x1.18af9388c8deap+0, 0x1.1972658375d2fp+0,
+    0x1.1a35beb6fcb75p+0, 0x1.1af99f8138a1cp+0, 0x1.1bbe084045cd4p+0, 0x1.1c82f95281c6bp+0,
+    0x1.1d4873168b9aap+0, 0x1.1e0e75eb44027p+0, 0x1.1ed5022fcd91dp+0, 0x1.1f9c18438ce4dp+0,
+    0x1.2063b88628cd6p+0, 0x1.212be3578a819p+0, 0x1.21f49917ddc96p+0, 0x1.22bdda27912d1p+0,
+    0x1.2387a6e756238p+0, 0x1.2451ffb82140ap+0, 0x1.251ce4fb2a63fp+0, 0x1.25e85711ece75p+0,
+    0x1.26b4565e27cddp+0, 0x1.2780e341ddf29p+0, 0x1.284dfe1f56381p+0, 0x1.291ba7591bb70p+0,
+    0x1.29e9df51fdee1p+0, 0x1.2ab8a66d10f13p+0, 0x1.2b87fd0dad990p+0, 0x1.2c57e39771b2fp+0,
+    0x1.2d285a6e4030bp+0, 0x1.2df961f641589p+0, 0x1.2ecafa93e2f56p+0, 0x1.2f9d24abd886bp+0,
+    0x1.306fe0a31b715p+0, 0x1.31432edeeb2fdp+0, 0x1.32170fc4cd831p+0, 0x1.32eb83ba8ea32p+0,
+    0x1.33c08b26416ffp+0, 0x1.3496266e3fa2dp+0, 0x1.356c55f929ff1p+0, 0x1.36431a2de883bp+0,
+    0x1.371a7373aa9cbp+0, 0x1.37f26231e754ap+0, 0x1.38cae6d05d866p+0, 0x1.39a401b7140efp+0,
+    0x1.3a7db34e59ff7p+0, 0x1.3b57fbfec6cf4p+0, 0x1.3c32dc313a8e5p+0, 0x1.3d0e544ede173p+0,
+    0x1.3dea64c123422p+0, 0x1.3ec70df1c5175p+0, 0x1.3fa4504ac801cp+0, 0x1.40822c367a024p+0,
+    0x1.4160a21f72e2ap+0, 0x1.423fb2709468ap+0, 0x1.431f5d950a897p+0, 0x1.43ffa3f84b9d4p+0,
+    0x1.44e086061892dp+0, 0x1.45c2042a7d232p+0, 0x1.46a41ed1d0057p+0, 0x1.4786d668b3237p+0,
+    0x1.486a2b5c13cd0p+0, 0x1.494e1e192aed2p+0, 0x1.4a32af0d7d3dep+0, 0x1.4b17dea6db7d7p+0,
+    0x1.4bfdad5362a27p+0, 0x1.4ce41b817c114p+0, 0x1.4dcb299fddd0dp+0, 0x1.4eb2d81d8abffp+0,
+    0x1.4f9b2769d2ca7p+0, 0x1.508417f4531eep+0, 0x1.516daa2cf6642p+0, 0x1.5257de83f4eefp+0,
+    0x1.5342b569d4f82p+0, 0x1.542e2f4f6ad27p+0, 0x1.551a4ca5d920fp+0, 0x1.56070dde910d2p+0,
+    0x1.56f4736b527dap+0, 0x1.57e27dbe2c4cfp+0, 0x1.58d12d497c7fdp+0, 0x1.59c0827ff07ccp+0,
+    0x1.5ab07dd485429p+0, 0x1.5ba11fba87a03p+0, 0x1.5c9268a5946b7p+0, 0x1.5d84590998b93p+0,
+    0x1.5e76f15ad2148p+0, 0x1.5f6a320dceb71p+0, 0x1.605e1b976dc09p+0, 0x1.6152ae6cdf6f4p+0,
+    0x1.6247eb03a5585p+0, 0x1.633dd1d1929fdp+0, 0x1.6434634ccc320p+0, 0x1.652b9febc8fb7p+0,
+    0x1.6623882552225p+0, 0x1.671c1c70833f6p+0, 0x1.68155d44ca973p+0, 0x1.690f4b19e9538p+0,
+    0x1.6a09e667f3bcdp+0, 0x1.6b052fa75173ep+0, 0x1.6c012750bdabfp+0, 0x1.6cfdcddd47645p+0,
+    0x1.6dfb23c651a2fp+0, 0x1.6ef9298593ae5p+0, 0x1.6ff7df9519484p+0, 0x1.70f7466f42e87p+0,
+    0x1.71f75e8ec5f74p+0, 0x1.72f8286ead08ap+0, 0x1.73f9a48a58174p+0, 0x1.74fbd35d7cbfdp+0,
+    0x1.75feb564267c9p+0, 0x1.77024b1ab6e09p+0, 0x1.780694fde5d3fp+0, 0x1.790b938ac1cf6p+0,
+    0x1.7a11473eb0187p+0, 0x1.7b17b0976cfdbp+0, 0x1.7c1ed0130c132p+0, 0x1.7d26a62ff86f0p+0,
+    0x1.7e2f336cf4e62p+0, 0x1.7f3878491c491p+0, 0x1.80427543e1a12p+0, 0x1.814d2add106d9p+0,
+    0x1.82589994cce13p+0, 0x1.8364c1eb941f7p+0, 0x1.8471a4623c7adp+0, 0x1.857f4179f5b21p+0,
+    0x1.868d99b4492edp+0, 0x1.879cad931a436p+0, 0x1.88ac7d98a6699p+0, 0x1.89bd0a478580fp+0,
+    0x1.8ace5422aa0dbp+0, 0x1.8be05bad61778p+0, 0x1.8cf3216b5448cp+0, 0x1.8e06a5e0866d9p+0,
+    0x1.8f1ae99157736p+0, 0x1.902fed0282c8ap+0, 0x1.9145b0b91ffc6p+0, 0x1.925c353aa2fe2p+0,
+    0x1.93737b0cdc5e5p+0, 0x1.948b82b5f98e5p+0, 0x1.95a44cbc8520fp+0, 0x1.96bdd9a7670b3p+0,
+    0x1.97d829fde4e50p+0, 0x1.98f33e47a22a2p+0, 0x1.9a0f170ca07bap+0, 0x1.9b2bb4d53fe0dp+0,
+    0x1.9c49182a3f090p+0, 0x1.9d674194bb8d5p+0, 0x1.9e86319e32323p+0, 0x1.9fa5e8d07f29ep+0,
+    0x1.a0c667b5de565p+0, 0x1.a1e7aed8eb8bbp+0, 0x1.a309bec4a2d33p+0, 0x1.a42c980460ad8p+0,
+    0x1.a5503b23e255dp+0, 0x1.a674a8af46052p+0, 0x1.a799e1330b358p+0, 0x1.a8bfe53c12e59p+0,
+    0x1.a9e6b5579fdbfp+0, 0x1.ab0e521356ebap+0, 0x1.ac36bbfd3f37ap+0, 0x1.ad5ff3a3c2774p+0,
+    0x1.ae89f995ad3adp+0, 0x1.afb4ce622f2ffp+0, 0x1.b0e07298db666p+0, 0x1.b20ce6c9a8952p+0,
+    0x1.b33a2b84f15fbp+0, 0x1.b468415b749b1p+0, 0x1.b59728de5593ap+0, 0x1.b6c6e29f1c52ap+0,
+    0x1.b7f76f2fb5e47p+0, 0x1.b928cf22749e4p+0, 0x1.ba5b030a1064ap+0, 0x1.bb8e0b79a6f1fp+0,
+    0x1.bcc1e904bc1d2p+0, 0x1.bdf69c3f3a207p+0, 0x1.bf2c25bd71e09p+0, 0x1.c06286141b33dp+0,
+    0x1.c199bdd85529cp+0, 0x1.c2d1cd9fa652cp+0, 0x1.c40ab5fffd07ap+0, 0x1.c544778fafb22p+0,
+    0x1.c67f12e57d14bp+0, 0x1.c7ba88988c933p+0, 0x1.c8f6d9406e7b5p+0, 0x1.ca3405751c4dbp+0,
+    0x1.cb720dcef9069p+0, 0x1.ccb0f2e6d1675p+0, 0x1.cdf0b555dc3fap+0, 0x1.cf3155b5bab74p+0,
+    0x1.d072d4a07897cp+0, 0x1.d1b532b08c968p+0, 0x1.d2f87080d89f2p+0, 0x1.d43c8eacaa1d6p+0,
+    0x1.d5818dcfba487p+0, 0x1.d6c76e862e6d3p+0, 0x1.d80e316c98398p+0, 0x1.d955d71ff6075p+0,
+    0x1.da9e603db3285p+0, 0x1.dbe7cd63a8315p+0, 0x1.dd321f301b460p+0, 0x1.de7d5641c0658p+0,
+    0x1.dfc97337b9b5fp+0, 0x1.e11676b197d17p+0, 0x1.e264614f5a129p+0, 0x1.e3b333b16ee12p+0,
+    0x1.e502ee78b3ff6p+0, 0x1.e653924676d76p+0, 0x1.e7a51fbc74c83p+0, 0x1.e8f7977cdb740p+0,
+    0x1.ea4afa2a490dap+0, 0x1.eb9f4867cca6ep+0, 0x1.ecf482d8e67f1p+0, 0x1.ee4aaa2188510p+0,
+    0x1.efa1bee615a27p+0, 0x1.f0f9c1cb6412ap+0, 0x1.f252b376bba97p+0, 0x1.f3ac948dd7274p+0,
+    0x1.f50765b6e4540p+0, 0x1.f6632798844f8p+0, 0x1.f7bfdad9cbe14p+0, 0x1.f91d802243c89p+0,
+    0x1.fa7c1819e90d8p+0, 0x1.fbdba3692d514p+0, 0x1.fd3c22b8f71f1p+0, 0x1.fe9d96b2a23d9p+0
+};
+template <bool CHECK = false>
 __device__ __forceinline__ double exp_tab(double x) {
-  const int hx = __double2hiint(x);
-  const double kf = fma(x, 0x1.71547652b82fep+6, 6755399441055744.0);   // 64/ln2; 1.5 * 2^52 rounds to the nearest integer
+  const double kf = fma(x, kExpC[0], kExpC[1]);                           // 256/ln2; 1.5 * 2^52 rounds to the nearest integer
   const int k = __double2loint(kf);
-  const double kd = kf - 6755399441055744.0;
-  double r = fma(kd, -0x1.62e42fee00000p-7, x);                           // ln2/64, 32 leading bits (exact product)
-  r = fma(kd, -0x1.a39ef35793c76p-39, r);                                 // ... and the rest
+  const double kd = kf - kExpC[1];
+  double r = fma(kd, kExpC[2], x);                                        // ln2/256, 32 leading bits (exact product)
+  r = fma(kd, kExpC[3], r);                                               // ... and the rest
   const double r2 = r * r;
-  double q = fma(r, 1.0 / 120.0, 1.0 / 24.0);
-  q = fma(q, r, 1.0 / 6.0);
-  q = fma(q, r, 0.5);
+  double q = fma(r, kExpC[4], kExpC[5]);
+  q = fma(q, r, kExpC[6]);
   const double pm1 = fma(q, r2, r);                                       // exp(r) - 1
-  const double t = __ldg(kExpTab + (k & 63));
+  const double t = __ldg(kExpTab + (k & 255));
   const double y = fma(t, pm1, t);
-  double res = __hiloint2double(__double2hiint(y) + ((k >> 6) << 20), __double2loint(y));
-  if ((hx & 0x7fffffff) >= 0x4085e000) res = (hx < 0) ? 0.0 : __longlong_as_double(0x7ff0000000000000LL);
+  double res = __hiloint2double(__double2hiint(y) + ((k >> 8) << 20), __double2loint(y));
+  if (CHECK) {
+    const int hx = __double2hiint(x);
+    if ((hx & 0x7fffffff) >= 0x4085e000) res = (hx < 0) ? 0.0 : __longlong_as_double(0x7ff0000000000000LL);
+  }
   return res;
 }
 
@@ -275,7 +355,7 @@ __device__ __forceinline__ double m_exp(double x) { return exp(x); }
 __device__ __forceinline__ float m_exp(float x) { return __expf(x); }
 __device__ __forceinline__ double m_tan(double x) { return tan_bw(x); }
 __device__ __forceinline__ float m_tan(float x) { return tan_bw(x); }
-__device__ __forceinline__ double m_rsqrt(double x) { return rsqrt(x); }
+__device__ __forceinline__ double m_rsqrt(double x) { return rsqrt_fast(x); }
 __device__ __forceinline__ float m_rsqrt(float x) { return rsqrtf(x); }
 
 // NEXT-3 (listing :274-306, reading A17): one species of the grid PDF at ln x = L.
@@ -296,10 +376,13 @@ __device__ __forceinline__ double pdf_grid_1d(const double* __restrict__ tab, in
 // GRIDPDF = false compiles the toy branch only (the hot kernels are instantiated both ways and the
 // launch picks one: carrying the table code costs 1-4 % even when it is not taken).
 template <typename T> struct TtLumi { T gg, qq; };
+// rsxx = (x1 x2)^(-1/2) when the caller has it already (toy PDF with the default exponents), else < 0
 template <bool GRIDPDF, typename T>
-__device__ __forceinline__ TtLumi<T> tt_lumi(const DevConstR<T>& c, T x1, T x2) {
+__device__ __forceinline__ TtLumi<T> tt_lumi(const DevConstR<T>& c, T x1, T x2, T rsxx = T(-1)) {
   if (!GRIDPDF || c.pdf_tab == nullptr) {
-    const T ff = pdf_pair(c, x1, x2);
+    T ff;
+    if (c.pdf_fast && rsxx > T(0)) { const T yy = (T(1) - x1) * (T(1) - x2); ff = rsxx * (yy * yy * yy); }
+    else ff = pdf_pair(c, x1, x2);
     return {ff * c.A_g2, ff * ((T(2.0) * c.n_flav * (T(4.0) / T(9.0))) * c.A_q2)};
   }
   const double L1 = log((double)x1), L2 = log((double)x2);
@@ -313,8 +396,12 @@ __device__ __forceinline__ TtLumi<T> tt_lumi(const DevConstR<T>& c, T x1, T x2) 
   return {(T)gg, (T)(qq * (2.0 * 4.0 / 9.0))};
 }
 
-template <bool TAB> __device__ __forceinline__ double x_exp(double x) { return TAB ? exp_tab(x) : exp(x); }
+// the outer exponential of a product of Gaussians: its argument may run below the range of exp (the result is then 0)
+template <bool TAB> __device__ __forceinline__ double x_exp(double x) { return TAB ? exp_tab<true>(x) : exp(x); }
 template <bool TAB> __device__ __forceinline__ float x_exp(float x) { return m_exp(x); }
+// an exponential whose argument is bounded by construction (|eta_nu| <= nu_eta_max <= 50)
+template <bool TAB> __device__ __forceinline__ double b_exp(double x) { return TAB ? exp_tab<false>(x) : exp(x); }
+template <bool TAB> __device__ __forceinline__ float b_exp(float x) { return m_exp(x); }
 
 // TAB: exp_tab instead of libdevice's exp (fp64 only).  Measured: configs 2 and 4 gain 5.7 % and 5.8 %;
 // config 3's time does not move (its plain kernel sits on the mixed-operand FP64 ceiling either way) while

@@ -98,7 +98,7 @@ template <class P, int MODE, bool PERM, bool GRIDPDF>
 __global__ void __launch_bounds__(kThreads, min_blocks<P, MODE>())
 integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__ ecs, const double* __restrict__ grids,
                  double* __restrict__ partials, double* __restrict__ hist, int64_t n_points,
-                 int64_t chunk, int n_chunks, uint64_t seed, uint64_t event_offset, uint32_t pass) {
+                 int64_t chunk, int n_chunks, const Philox rng, uint64_t event_offset, uint32_t pass) {
   constexpr int D = P::D;
   using T = typename P::real;                         // fp64, or fp32 for the A15 variant
   extern __shared__ double smem[];
@@ -119,7 +119,6 @@ integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__
     for (int k = threadIdx.x; k < kWarps * D * B; k += kThreads) whist[k] = 0.0;
   __syncthreads();
 
-  const Philox rng{(uint32_t)seed, (uint32_t)(seed >> 32)};
   const uint32_t ev_ctr = (uint32_t)(event_offset + (uint64_t)e);
   const int64_t lo = (int64_t)ch * chunk;
   const int64_t hi = (lo + chunk < n_points) ? lo + chunk : n_points;
@@ -196,11 +195,11 @@ integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__
     } else {
     draw_uniforms<D>(rng, (uint64_t)i, ev_ctr, pass, u);
     if (MODE == MODE_PLAIN) {
-      w = eval_weight<P, PERM, GRIDPDF, MODE != MODE_PLAIN>(c, ec, c0, u);
+      w = eval_weight<P, PERM, GRIDPDF, true>(c, ec, c0, u);
     } else {
       int k[D];
       const double jac = vegas_map<D>(edges, B, u, k);
-      w = jac * eval_weight<P, PERM, GRIDPDF, MODE != MODE_PLAIN>(c, ec, c0, u);
+      w = jac * eval_weight<P, PERM, GRIDPDF, true>(c, ec, c0, u);
       if (!isfinite(w)) w = 0.0;
       if (MODE == MODE_ADAPT) {
         const double w2 = live ? w * w : 0.0;
@@ -319,7 +318,7 @@ __global__ void refine_kernel(const DevConst c, const double* __restrict__ hist,
 template <class P>
 __global__ void eval_points_kernel(const DevConstR<typename P::real> c, const double* __restrict__ ecs, int64_t event,
                                    const double* __restrict__ grid, int64_t first, int64_t n,
-                                   uint64_t seed, uint64_t event_offset, uint32_t pass,
+                                   const Philox rng, uint64_t event_offset, uint32_t pass,
                                    double* __restrict__ out_w) {
   constexpr int D = P::D;
   using T = typename P::real;
@@ -335,7 +334,6 @@ __global__ void eval_points_kernel(const DevConstR<typename P::real> c, const do
   __syncthreads();
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
-  const Philox rng{(uint32_t)seed, (uint32_t)(seed >> 32)};
   double u[D];
   double w;
   if constexpr (!std::is_same<T, double>::value) {
@@ -351,10 +349,10 @@ __global__ void eval_points_kernel(const DevConstR<typename P::real> c, const do
   if (grid) {
     int k[D];
     const double jac = vegas_map<D>(edges, B, u, k);
-    w = jac * eval_weight<P, true, true, false>(c, ec, c0, u);
+    w = jac * eval_weight<P, true, true, true>(c, ec, c0, u);
     if (!isfinite(w)) w = 0.0;
   } else {
-    w = eval_weight<P, true, true, false>(c, ec, c0, u);
+    w = eval_weight<P, true, true, true>(c, ec, c0, u);
   }
   out_w[i] = w;
 }

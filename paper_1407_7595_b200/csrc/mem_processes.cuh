@@ -205,7 +205,7 @@ struct ProcZbb {
   __device__ static double weight(const DevConst& c, const double* ec, const double (&u)[D]) {
     TfAcc<double> tfa{0.0, 1.0};
     const Jet p1 = jet_point(c, ec + J0, u[0], tfa), p2 = jet_point(c, ec + J1, u[1], tfa);
-    const double tf = tfa.fac * exp_tab(-tfa.esum);
+    const double tf = tfa.fac * exp_tab<true>(-tfa.esum);
     // O7 without the cancellation in 1 - beta^2 (nearly collinear jets): with P = p1 + p2,
     //   P_E'^2 = P_E^2 - P_T^2 = p1z^2 + p2z^2 + 2 E1 E2 (1 - n1T.n2T)
     //   E_i'   = gamma (E_i - beta.p_iT) = (p_iz^2 + E1 E2 (1 - n1T.n2T)) / P_E'
@@ -310,7 +310,7 @@ struct ProcTTljetsR {
     const T x0 = fma(c.dr, u[0], c.rlo), x1j = fma(c.dr, u[1], c.rlo), x2j = fma(c.dr, u[2], c.rlo), x3 = fma(c.dr, u[3], c.rlo);
     const T H = c.nu_eta_max;
     const T eta_nu = fma(T(2.0) * H, u[4], -H);
-    const T en = x_exp<TAB>(eta_nu);
+    const T en = b_exp<TAB>(eta_nu);
     const T g = en * ec[ELI];
     const T gm1 = g - T(1.0);
     const T denp = ec[LPT2] * fma(T(0.5) * gm1, gm1, ec[OMC] * g);
@@ -332,8 +332,8 @@ struct ProcTTljetsR {
     const T sW = c.mW2 + smm;
     const T iden = g * idenp;                                                    // 1 / (2 pT_l (cosh - cos))
     const T nuT = sW * iden;
-    const T chn = T(0.5) * (en + eni), shn = T(0.5) * (en - eni);
-    const T nE = nuT * chn, nx = nuT * ec[CPN], ny = nuT * ec[SPN], nz = nuT * shn;
+    const T hnuT = T(0.5) * nuT;
+    const T nE = hnuT * (en + eni), nx = nuT * ec[CPN], ny = nuT * ec[SPN], nz = hnuT * (en - eni);
     T sum = T(0);
     const int n_perm = PERM ? c.n_perm : 1;
     for (int k = 0; k < n_perm; ++k, ec += NC) {
@@ -361,29 +361,35 @@ struct ProcTTljetsR {
     const T xx = x1 * x2, shat = xx * c.S;
     ok = ok && T(4.0) * c.mt2 < shat;                                             // reading A9
     // ---- S5: production.  tau1 = (q1.pt + q2.ptb)/s-hat, tau2 = (q2.pt + q1.ptb)/s-hat
-    const T ish = rcp_fast(shat);
+    // one reciprocal square root serves 1/s-hat and the toy PDF's (x1 x2)^(-1/2) = sqrt(S) / sqrt(s-hat)
+    const T rs = m_rsqrt(shat);
+    const T ish = rs * rs;
     const T hs = T(0.5) * c.sqrt_s * ish;
     const T tau1 = hs * fma(x1, tEb - tz, x2 * (aEb + az));
     const T tau2 = hs * fma(x2, tEb + tz, x1 * (aEb - az));
     const T rho = T(4.0) * c.mt2 * ish;
-    const T iT = rcp_fast(tau1 * tau2);
-    const T tt = fma(tau1, tau1, tau2 * tau2);
-    const T Mgg = fma(iT, T(1.0) / T(6.0), -T(0.375)) * (tt + rho - T(0.25) * rho * rho * iT);
-    const T Mqq = tt + T(0.5) * rho;
-    const TtLumi<T> lum = tt_lumi<GRIDPDF>(c, x1, x2);
-    const T prod = fma(lum.gg, Mgg, lum.qq * Mqq);                             // flavour sum incl. the PDFs
+    const T t12 = tau1 * tau2;
     // ---- S5: propagators and decays
     const T t_l = fma(T(0.5), sW, bl_l);                                       // p_t . l
     const T a_q = bh_q + q_qb;                                                 // p_tbar . q
-    T decprop;                                                                 // decays x propagators
+    T decprop, iT;                                                             // decays x propagators, 1/(tau1 tau2)
     if constexpr (kSplitC0) {
       // fp32: keep every intermediate inside the single-precision range
+      iT = rcp_fast(t12);
       decprop = (t_l * bl_nu * rcp_fast(fma(st_m, st_m, c.mtGt2))) * (a_q * rcp_fast(fma(stb_m, stb_m, c.mtGt2))) *
                 (bh_qb * rcp_fast(fma(swh_m, swh_m, c.mWGW2)));
     } else {
+      // one reciprocal for 1/(tau1 tau2) and the three propagator denominators
       const T dens = fma(st_m, st_m, c.mtGt2) * fma(stb_m, stb_m, c.mtGt2) * fma(swh_m, swh_m, c.mWGW2);
-      decprop = t_l * bl_nu * a_q * bh_qb * rcp_fast(dens);
+      const T inv = rcp_fast(t12 * dens);
+      iT = inv * dens;
+      decprop = t_l * bl_nu * a_q * bh_qb * (inv * t12);
     }
+    const T tt = fma(tau1, tau1, tau2 * tau2);
+    const T Mgg = fma(iT, T(1.0) / T(6.0), -T(0.375)) * (tt + rho - T(0.25) * rho * rho * iT);
+    const T Mqq = tt + T(0.5) * rho;
+    const TtLumi<T> lum = tt_lumi<GRIDPDF>(c, x1, x2, rs * c.sqrt_s);
+    const T prod = fma(lum.gg, Mgg, lum.qq * Mqq);                             // flavour sum incl. the PDFs
     // ---- S4, S7
     const T core = ish * prod * decprop;
     if (ok && isfinite(core)) sum += core;
@@ -712,7 +718,7 @@ struct ProcTTdilep {
     const double dec = fma(Eb0, ec[S0 + ELK], 0.5 * sW0) * (Eb0 * hD0) * fma(Eb1, ec[S1 + ELK], 0.5 * sW1) * (Eb1 * hD1);
     // jets' Gaussians and the MET Gaussian share one exponential
     const double targ = fma(ec[MEXP], fma(g6, g6, g7 * g7), -tfa.esum);
-    const double tf_tmet = tfa.fac * (TAB ? exp_tab(targ) : exp(targ));
+    const double tf_tmet = tfa.fac * (TAB ? exp_tab<true>(targ) : exp(targ));
     const double w = ec[C0] * tf_tmet * dec * (iEb0 * iEb1) * sum;
     return isfinite(w) ? w : 0.0;
   }

@@ -307,7 +307,7 @@ struct ProcTTHdilep {
         TfAcc<double> th{0.0, 1.0};
         tf_accum<TAB>(c, rcp_fast(E1 * ec[IEJ2]), th);
         tf_accum<TAB>(c, rcp_fast(E2 * ec[IEJ3]), th);
-        total = fma(th.fac * (TAB ? exp_tab(-th.esum) : exp(-th.esum)), sum, total);
+        total = fma(th.fac * (TAB ? exp_tab<true>(-th.esum) : exp(-th.esum)), sum, total);
       }
     }
     if (which == -2) return counts;
@@ -316,7 +316,7 @@ struct ProcTTHdilep {
     TfAcc<double> tfa{0.0, 1.0};
     tf_accum<TAB>(c, ixb0, tfa);
     tf_accum<TAB>(c, ixb1, tfa);
-    const double tf = tfa.fac * (TAB ? exp_tab(-tfa.esum) : exp(-tfa.esum));
+    const double tf = tfa.fac * (TAB ? exp_tab<true>(-tfa.esum) : exp(-tfa.esum));
     const double dec = fma(Eb0, ec[S0 + ELK], 0.5 * sW0) * (Eb0 * hD0) * fma(Eb1, ec[S1 + ELK], 0.5 * sW1) * (Eb1 * hD1);
     // hypothesis 0: sum |M(H -> b bbar)|^2 carries k^2; hypothesis 1: (1/k^4)(k^2)(dk^2/du ~ k^2) is constant
     const double hfac = c.tth_hyp ? 1.0 : sH;
