@@ -144,6 +144,8 @@ DevConst make_dev_const(const mem_params& p) {
   c.tf_a1 = 1.0 / (p.tf_sig1 * r2); c.tf_b1 = -(1.0 + p.tf_mu1) / (p.tf_sig1 * r2);
   c.tf_a2 = 1.0 / (p.tf_sig2 * r2); c.tf_b2 = -(1.0 + p.tf_mu2) / (p.tf_sig2 * r2);
   c.tf_c1 = (1.0 - p.tf_w_tail) / (p.tf_sig1 * r2pi); c.tf_c2 = p.tf_w_tail / (p.tf_sig2 * r2pi);
+  c.tf_q2 = (c.tf_a1 - c.tf_a2) * (c.tf_a1 + c.tf_a2); c.tf_q1 = 2.0 * (c.tf_a1 * c.tf_b1 - c.tf_a2 * c.tf_b2);
+  c.tf_q0 = (c.tf_b1 - c.tf_b2) * (c.tf_b1 + c.tf_b2);
   c.mW = p.m_W; c.GW = p.Gam_W; c.mW2 = p.m_W * p.m_W; c.mWGW = p.m_W * p.Gam_W; c.mWGW2 = c.mWGW * c.mWGW;
   bw_window(p.m_W, p.Gam_W, p.bw_nwidths, &c.tW_lo, &c.tW_dt);
   c.mt2 = p.m_t * p.m_t; c.mtGt = p.m_t * p.Gam_t; c.mtGt2 = c.mtGt * c.mtGt;
@@ -175,7 +177,7 @@ DevConstF to_float(const DevConst& d) {
   DevConstF f;
 #define CP(x) f.x = (float)d.x
   CP(sqrt_s); CP(inv_sqrt_s); CP(S); CP(inv_S); CP(pdf_pow_x); CP(pdf_pow_1mx); CP(A_q2); CP(A_g2); CP(rlo); CP(dr);
-  CP(tf_a1); CP(tf_b1); CP(tf_c1); CP(tf_a2); CP(tf_b2); CP(tf_c2); CP(mW); CP(GW); CP(mW2); CP(mWGW); CP(mWGW2);
+  CP(tf_a1); CP(tf_b1); CP(tf_c1); CP(tf_a2); CP(tf_b2); CP(tf_c2); CP(tf_q2); CP(tf_q1); CP(tf_q0); CP(mW); CP(GW); CP(mW2); CP(mWGW); CP(mWGW2);
   CP(tW_lo); CP(tW_dt); CP(mt2); CP(mtGt); CP(mtGt2); CP(tT_lo); CP(tT_dt); CP(mZ2); CP(mZGZ2); CP(g4w); CP(gz4);
   CP(gs4); CP(V_ud2); CP(V_tb2); CP(z_cu); CP(z_ct); CP(nu_pz_max); CP(nu_eta_max); CP(met_sigma); CP(met_nsigma);
   CP(vegas_alpha); CP(rhi); CP(mH2); CP(mHGH); CP(tH_lo); CP(tH_dt); CP(lnr); CP(tth_c);

@@ -85,12 +85,12 @@ __device__ __forceinline__ void warp_hist_add(double* wh, int k, double v) {
 // sums go registers -> warp shuffle -> shared -> partials[event][chunk] in a fixed order.
 // MODE_GRID/ADAPT: grids = [n_events][D][B+1].  MODE_ADAPT also writes the block's histogram
 // of w^2 to hist[event][chunk][D][B].
-// Resident blocks per SM the register allocation aims at (measured on B200):
-// the plain config-1/2/3 kernels (no register cap: 64/50/80 registers, no spills) are bound by FP64 issue and
-// gain nothing from more warps; the divergent config-4 kernel and the VEGAS passes (shuffle/match
-// latency) gain 43 % / 7 % from 3 blocks at 80 registers.
+// Resident blocks per SM the register allocation aims at (measured on B200): 3 blocks of 256
+// threads = 80 registers for every integrate kernel.  The plain config-1/2/3 kernels fit without spills (uncapped
+// the config-3 kernel takes 100 registers, 2 blocks/SM, and is 1.6 % slower; 4 blocks at 64 registers change nothing);
+// the divergent conic-solver kernels and the VEGAS passes (shuffle/match latency) gain 43 % / 7 % from 3 blocks.
 template <class P, int MODE>
-constexpr int min_blocks() { return (P::kHeavy || MODE != MODE_PLAIN) ? 3 : 0; }   // 0 = no cap
+constexpr int min_blocks() { return 3; }
 
 // PERM: sum over c.n_perm jet-parton assignments per point (NEXT-1); the per-event constants are
 // then n_perm blocks of NC.  GRIDPDF: the flavour sum may use interpolated tables (NEXT-3).
