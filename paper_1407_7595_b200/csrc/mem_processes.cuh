@@ -354,8 +354,9 @@ struct ProcTTljetsR {
     const T M2 = fma(PE, PE, -fma(Px, Px, Py * Py));
     bool ok = M2 > T(0);                     // cuts are predicates: the select at the end discards the point
     const T rM = m_rsqrt(M2);
-    const T tEb = rM * fma(tE, PE, -fma(Px, tx, Py * ty)), aEb = rM * fma(aE, PE, -fma(Px, ax, Py * ay));
-    const T PEb = tEb + aEb;
+    // the boosted total energy is sqrt(P_E^2 - P_T^2) itself; the antitop's is the rest
+    const T tEb = rM * fma(tE, PE, -fma(Px, tx, Py * ty));
+    const T PEb = M2 * rM, aEb = PEb - tEb;
     const T x1 = (PEb + Pz) * c.inv_sqrt_s, x2 = (PEb - Pz) * c.inv_sqrt_s;
     ok = ok && x1 > T(0) && x1 < T(1.0) && x2 > T(0) && x2 < T(1.0);
     const T xx = x1 * x2, shat = xx * c.S;
@@ -392,7 +393,8 @@ struct ProcTTljetsR {
     const T prod = fma(lum.gg, Mgg, lum.qq * Mqq);                             // flavour sum incl. the PDFs
     // ---- S4, S7
     const T core = ish * prod * decprop;
-    if (ok && isfinite(core)) sum += core;
+    if constexpr (PERM) { if (ok && isfinite(core)) sum += core; }
+    else sum = ok ? core : T(0);                            // a non-finite value is caught by the final test
     }
     const T pt = tf * (nuT * iden) * sum;
     // fp64: the per-event constant (identical for every assignment) is applied here; fp32: by the
