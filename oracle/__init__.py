@@ -112,7 +112,7 @@ def lib():
         L.orc_weight_x.argtypes = [C.c_int, C.POINTER(Params), _dp, _dp]
         L.orc_weight_x.restype = C.c_double
         L.orc_eval_points_x.argtypes = [C.c_int, C.POINTER(Params), _dp, C.c_int64, C.c_int64, C.c_uint64,
-                                        C.c_int64, C.c_int64, C.c_uint64, C.c_int32, _dp]
+                                        C.c_int64, C.c_int64, C.c_uint64, C.c_int32, _dp, _dp]
         L.orc_integrate.argtypes = [C.c_int, C.POINTER(Params), _dp, C.c_int64, C.c_uint64, C.c_int64,
                                     C.c_uint64, _dp, _dp]
         L.orc_vegas_map.argtypes = [_dp, C.c_int, C.c_int, _dp, _dp, C.POINTER(C.c_int), _dp]
@@ -343,11 +343,12 @@ def weight_x(process, p, rec, u):
     return lib().orc_weight_x(process, C.byref(p), _p(rec), _p(u))
 
 
-def eval_points_x(process, p, events, event, first_point, n, seed, iteration=0, event_offset=0):
+def eval_points_x(process, p, events, event, first_point, n, seed, iteration=0, event_offset=0, grid=None):
     ev = _f64(events)
     out = np.empty(n, dtype=np.float64)
+    g = None if grid is None else _f64(grid)
     rc = lib().orc_eval_points_x(process, C.byref(p), _p(ev), ev.shape[1], event, event_offset, first_point, n,
-                                 seed, iteration, _p(out))
+                                 seed, iteration, None if g is None else _p(g), _p(out))
     if rc != 0:
         raise ValueError("orc_eval_points_x failed")
     return out

@@ -1316,18 +1316,26 @@ int orc_eval_points(int process, const orc_params* p, const double* events, int6
   return 0;
 }
 
-// referee version of orc_eval_points (no grid: the warped point z is itself a rounded fp64
-// quantity on both sides, so grid parity is tested through orc_eval_points)
+// referee version of orc_eval_points.  With a grid the warp u -> z and its Jacobian are the fp64 ones of
+// orc_vegas_map (the warped point is itself a rounded fp64 quantity on both sides); the integrand at z is
+// evaluated in long double.
 int orc_eval_points_x(int process, const orc_params* p, const double* events, int64_t n_events,
                       int64_t event, uint64_t event_offset, int64_t first_point, int64_t n,
-                      uint64_t seed, int32_t iteration, double* out_w) {
+                      uint64_t seed, int32_t iteration, const double* grid, double* out_w) {
   int nf = orc_n_fields(process), D = orc_n_dims(process);
   if (nf < 0 || !p || !events || !out_w || event < 0 || event >= n_events) return 1;
-  double rec[32], u[16];
+  double rec[32], u[16], z[16];
   load_record(events, n_events, event, nf, rec);
+  const int B = p->vegas_bins;
   for (int64_t i = 0; i < n; ++i) {
     orc_uniforms(seed, event_offset + (uint64_t)event, (uint64_t)(first_point + i), (uint32_t)iteration, D, u);
-    out_w[i] = orc_weight_x(process, p, rec, u);
+    if (grid) {
+      double jac;
+      orc_vegas_map(grid + (size_t)event * D * (B + 1), B, D, u, z, nullptr, &jac);
+      out_w[i] = (double)((long double)jac * (long double)orc_weight_x(process, p, rec, z));
+    } else {
+      out_w[i] = orc_weight_x(process, p, rec, u);
+    }
   }
   return 0;
 }

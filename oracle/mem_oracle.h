@@ -132,7 +132,7 @@ int orc_eval_points(int process, const orc_params* p, const double* events, int6
                     uint64_t seed, int32_t iteration, const double* grid, double* out_w);
 int orc_eval_points_x(int process, const orc_params* p, const double* events, int64_t n_events,
                       int64_t event, uint64_t event_offset, int64_t first_point, int64_t n,
-                      uint64_t seed, int32_t iteration, double* out_w);
+                      uint64_t seed, int32_t iteration, const double* grid, double* out_w);
 int orc_integrate(int process, const orc_params* p, const double* events, int64_t n_events,
                   uint64_t event_offset, int64_t n_points, uint64_t seed,
                   double* out_p, double* out_err);

@@ -45,4 +45,4 @@ def test_cuda_path_reproduces_the_stored_values(case):
         p, err = it.integrate(ev, n_points, mg.SEED)
     ref = _stored()[label]
     assert np.all(np.abs(p.cpu().numpy() - ref[:, 0]) <= 1e-9 * np.abs(ref[:, 0]))
-    assert np.all(np.abs(err.cpu().numpy() - ref[:, 1]) <= 1e-8 * np.abs(ref[:, 1]) + 1e-300)
+    assert np.all(np.abs(err.cpu().numpy() - ref[:, 1]) <= 1e-9 * np.abs(ref[:, 1]) + 1e-300)

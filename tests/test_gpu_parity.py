@@ -158,15 +158,14 @@ def test_vegas_parity(mem):
         assert np.max(np.abs(gg - go)) <= 1e-11
         assert np.all(np.diff(gg, axis=2) > 0) and np.all(gg[:, :, 0] == 0) and np.all(gg[:, :, -1] == 1)
         assert np.all(np.abs(pg - po) <= TOL_EVENT * np.abs(po))
-        assert np.all(np.abs(eg - eo) <= 1e-8 * np.abs(eo))
+        assert np.all(np.abs(eg - eo) <= TOL_EVENT * np.abs(eo))
         # S1v per point through the oracle's grid
         import torch
         for e in range(ne):
             wg = it.eval_points(dev, e, 0, 3000, SEED, iteration=3, grid=torch.from_numpy(go[e]).cuda()).cpu().numpy()
             wo = oracle.eval_points(proc, p, ev, e, 0, 3000, SEED, iteration=3, grid=go)
-            assert np.array_equal(wg == 0, wo == 0)
-            nz = wo != 0
-            assert np.max(np.abs(wg[nz] - wo[nz]) / np.abs(wo[nz])) <= 2e-11
+            wx = oracle.eval_points_x(proc, p, ev, e, 0, 3000, SEED, iteration=3, grid=go)
+            _check_points(wg, wo, wx, "vegas event %d" % e)
         # the adapted estimate is more precise than plain MC of the same size
     with mem.Integrator(proc) as plain:
         _, e_plain = plain.integrate(_dev(ev), n_points, SEED)
@@ -270,7 +269,7 @@ def test_full_size_vegas_sampled_output(mem):
     e = 137
     po, eo = oracle.vegas_integrate(proc, p, ev[:, e:e + 1], n_points, SEED, event_offset=e)
     assert abs(pg[e] - po[0]) <= TOL_EVENT * abs(po[0])
-    assert abs(eg[e] - eo[0]) <= 1e-8 * abs(eo[0])
+    assert abs(eg[e] - eo[0]) <= TOL_EVENT * abs(eo[0])
 
 
 def test_fp64_microbenchmarks(mem):
