@@ -18,7 +18,14 @@
  * or retains caller buffers.  All functions return a mem_status and never
  * throw or abort; mem_last_error() gives a thread-local message for the last
  * failure on the calling thread.  A handle must not be used from two threads
- * at once; distinct handles are independent.
+ * at once; distinct handles are independent.  One handle may be used from
+ * several CUDA streams in turn: its workspace is shared by consecutive calls,
+ * so every call first makes its stream wait (on the device, without blocking
+ * the host) for the previous call on that handle, and a workspace growth step
+ * waits for it on the host before freeing anything.  The exception is a call
+ * made while its stream is being captured into a CUDA graph: no cross-stream
+ * ordering is recorded then, and the caller owns the handle exclusively for
+ * as long as the graph is replayed.
  */
 #ifndef MEM_B200_H
 #define MEM_B200_H
@@ -100,7 +107,7 @@ int32_t mem_n_dims(mem_process process);
  * params (host) is copied; NULL = defaults.  *out receives the handle. */
 mem_status mem_create(mem_process process, const mem_params* params, mem_handle** out);
 
-/* Free the handle and its workspace (synchronises the device). NULL is a no-op. */
+/* Free the handle and its workspace (synchronises the handle's device, whichever device is current). NULL is a no-op. */
 mem_status mem_destroy(mem_handle* h);
 
 /* Multi-GPU sharding: the event index that enters the
@@ -121,9 +128,10 @@ mem_status mem_set_event_offset(mem_handle* h, uint64_t first_event);
  * out_p, out_err : device, float64 [n_events]; overwritten
  * cuda_stream : a cudaStream_t (NULL = legacy default stream).  All work is
  *   enqueued on it and the call returns without synchronising.  The handle's
- *   workspace grows on demand (a growth step synchronises that stream); once a call
- *   of the same size has run, further calls allocate nothing and may be captured
- *   into a CUDA graph on a capturing stream and replayed.
+ *   workspace grows on demand (a growth step synchronises that stream and waits for
+ *   the handle's previous call); once a call of the same size has run, further calls
+ *   allocate nothing and may be captured into a CUDA graph on a capturing stream and
+ *   replayed (mem_last_pass_ms does not see captured calls).
  * n_events == 0 is MEM_OK with no launch; n_points < 2 is MEM_ERR_INVALID_ARG; so is a call made while
  * another CUDA device than the handle's is current.
  * Kinematically forbidden or non-finite points contribute w = 0 and still count in N. */
@@ -132,11 +140,13 @@ mem_status mem_integrate(mem_handle* h, const double* events, int64_t n_events,
                          double* out_p, double* out_err, void* cuda_stream);
 
 /* Same computation through host buffers: copies `events` host->device, runs
- * mem_integrate, copies the two result arrays device->host and synchronises.
+ * mem_integrate, copies the two result arrays device->host, all on cuda_stream,
+ * and synchronises that stream before returning (other streams keep running).
+ * Pinned host buffers make the copies asynchronous with respect to other streams.
  * This is the end-to-end entry the benchmark's "e2e" figure times. */
 mem_status mem_integrate_host(mem_handle* h, const double* events_host, int64_t n_events,
                               int64_t n_points, uint64_t seed,
-                              double* out_p_host, double* out_err_host);
+                              double* out_p_host, double* out_err_host, void* cuda_stream);
 
 /* Diagnostic for the parity tests: the individual weights w_i of one event,
  * i in [first_point, first_point + n), for Philox pass `iteration`.
@@ -157,7 +167,8 @@ mem_status mem_eval_points(mem_handle* h, const double* events, int64_t n_events
  *         [0, n - 2] as in the listing, so points outside the grid extrapolate the edge cell.
  * The flavour sum of t tbar production becomes f_g f_g |M_gg|^2 + sum over the first n_flav quark species of
  * 2 f_q f_q |M_qq|^2.  MEM_PROC_TT_LJETS / MEM_PROC_TT_DILEP with precision 64 only (MEM_ERR_UNSUPPORTED
- * otherwise).  Synchronises the device copy; call it between, not during, integrations. */
+ * otherwise).  Synchronises the whole device first (work in flight on any stream may still read the
+ * table being replaced), then copies synchronously. */
 mem_status mem_set_pdf_grid(mem_handle* h, const double* table, int32_t nx, int32_t nq, double lxmin, double lxmax,
                             double lqmin, double lqmax, double Q);
 
@@ -197,7 +208,8 @@ int64_t mem_launch_count(const mem_handle* h);
 /* Measurement support.  Every mem_integrate records CUDA events on
  * its stream around the dominant kernel, i.e. the integrate pass that produces the outputs.
  * mem_last_pass_ms waits for that pass and returns its duration in *ms (host, out) and the
- * number of integrand evaluations it made in *evals (host, out; may be NULL). */
+ * number of integrand evaluations it made in *evals (host, out; may be NULL).  A call captured into a CUDA
+ * graph records no events: after it mem_last_pass_ms returns MEM_ERR_INVALID_ARG until an eager call has run. */
 mem_status mem_last_pass_ms(mem_handle* h, double* ms, int64_t* evals);
 
 /* FP64 FMA peak of the current device, measured with independent DFMA chains on all SMs:

@@ -65,7 +65,7 @@ def lib():
         L.mem_destroy.argtypes = [vp]
         L.mem_set_event_offset.argtypes = [vp, u64]
         L.mem_integrate.argtypes = [vp, dp, i64, i64, u64, dp, dp, vp]
-        L.mem_integrate_host.argtypes = [vp, dp, i64, i64, u64, dp, dp]
+        L.mem_integrate_host.argtypes = [vp, dp, i64, i64, u64, dp, dp, vp]
         L.mem_eval_points.argtypes = [vp, dp, i64, i64, i64, i64, u64, C.c_int32, dp, dp, vp]
         L.mem_eval_parton.argtypes = [vp, dp, i64, dp, vp]
         L.mem_set_pdf_grid.argtypes = [vp, dp, C.c_int32, C.c_int32] + [C.c_double] * 5
@@ -107,10 +107,31 @@ def mem_n_dims(process: int) -> int:
     return lib().mem_n_dims(int(process))
 
 
-def mem_create(process: int, params: mem_params | None = None):
-    h = C.c_void_p()
+class Handle(C.c_void_p):
+    """The opaque mem_handle* plus what the binding needs to validate arguments: the process and the device
+    the handle was created on (the C ABI cannot see tensor shapes or devices)."""
+    process = 0
+    device = -1
+    bins = 50
+
+
+def mem_create(process: int, params: mem_params | None = None) -> Handle:
+    h = Handle()
     _check(lib().mem_create(int(process), None if params is None else C.byref(params), C.byref(h)))
+    import torch
+    h.process, h.device = int(process), torch.cuda.current_device()
+    h.bins = int(params.vegas_bins) if params is not None else 50
     return h
+
+
+def _check_tensor(handle, t, name, rows=None):
+    """shape[0] == rows and the tensor lives on the handle's device (a transposed record array or a record of
+    another process would make the kernels read beyond the allocation)"""
+    if rows is not None and (t.dim() != 2 or int(t.shape[0]) != rows):
+        raise ValueError("%s must have shape [%d, n_events], got %s" % (name, rows, tuple(t.shape)))
+    dev = getattr(handle, "device", -1)
+    if dev >= 0 and t.is_cuda and t.device.index != dev:
+        raise ValueError("%s is on cuda:%d, the handle was created on cuda:%d" % (name, t.device.index, dev))
 
 
 def mem_destroy(handle) -> None:
@@ -174,31 +195,35 @@ def mem_integrate(handle, events, n_points: int, seed: int, out_p=None, out_err=
     import torch
     if events.dim() != 2:
         raise ValueError("events must be [n_fields, n_events]")
+    _check_tensor(handle, events, "events", mem_event_fields(handle.process) if getattr(handle, "process", 0) else None)
     n_events = int(events.shape[1])
     if out_p is None:
         out_p = torch.empty(n_events, dtype=torch.float64, device=events.device)
     if out_err is None:
         out_err = torch.empty(n_events, dtype=torch.float64, device=events.device)
+    _check_tensor(handle, out_p, "out_p")
+    _check_tensor(handle, out_err, "out_err")
     _check(lib().mem_integrate(handle, _dev_f64(events, "events"), n_events, int(n_points), int(seed),
                                _dev_f64(out_p, "out_p", (n_events,)), _dev_f64(out_err, "out_err", (n_events,)),
                                _stream_ptr(stream)))
     return out_p, out_err
 
 
-def mem_integrate_host(handle, events, n_points: int, seed: int, out_p=None, out_err=None):
+def mem_integrate_host(handle, events, n_points: int, seed: int, out_p=None, out_err=None, stream=None):
     """events: float64 CPU tensor or numpy array [n_fields, n_events].  Copies in, integrates, copies the
-    results back into float64 CPU tensors and synchronises."""
+    results back into float64 CPU tensors, all on `stream` (default: torch's current stream), and synchronises it."""
     import torch
     ev = torch.as_tensor(events)
     if not (ev.dtype == torch.float64 and ev.is_contiguous() and not ev.is_cuda and ev.dim() == 2):
         raise TypeError("events must be a contiguous float64 host array [n_fields, n_events]")
+    _check_tensor(handle, ev, "events", mem_event_fields(handle.process) if getattr(handle, "process", 0) else None)
     n_events = int(ev.shape[1])
     if out_p is None:
         out_p = torch.empty(n_events, dtype=torch.float64)
     if out_err is None:
         out_err = torch.empty(n_events, dtype=torch.float64)
     _check(lib().mem_integrate_host(handle, C.c_void_p(ev.data_ptr()), n_events, int(n_points), int(seed),
-                                    C.c_void_p(out_p.data_ptr()), C.c_void_p(out_err.data_ptr())))
+                                    C.c_void_p(out_p.data_ptr()), C.c_void_p(out_err.data_ptr()), _stream_ptr(stream)))
     return out_p, out_err
 
 
@@ -206,9 +231,15 @@ def mem_eval_points(handle, events, event: int, first_point: int, n: int, seed: 
                     grid=None, out_w=None, stream=None):
     """Diagnostic: weights of points [first_point, first_point + n) of one event (CUDA tensor [n])."""
     import torch
+    _check_tensor(handle, events, "events", mem_event_fields(handle.process) if getattr(handle, "process", 0) else None)
     n_events = int(events.shape[1])
     if out_w is None:
         out_w = torch.empty(int(n), dtype=torch.float64, device=events.device)
+    if grid is not None:
+        _check_tensor(handle, grid, "grid")
+        if grid.dim() != 2 or int(grid.shape[0]) != mem_n_dims(handle.process) or int(grid.shape[1]) != handle.bins + 1:
+            raise ValueError("grid must have shape [D, vegas_bins + 1] = [%d, %d], got %s"
+                             % (mem_n_dims(handle.process), handle.bins + 1, tuple(grid.shape)))
     g = None if grid is None else _dev_f64(grid, "grid")
     _check(lib().mem_eval_points(handle, _dev_f64(events, "events"), n_events, int(event), int(first_point), int(n),
                                  int(seed), int(iteration), g, _dev_f64(out_w, "out_w", (int(n),)),
@@ -232,6 +263,7 @@ def mem_set_pdf_grid(handle, table, lxmin, lxmax, lqmin, lqmax, Q):
 def mem_eval_parton(handle, momenta, out_w=None, stream=None):
     """Parton-level mode (NEXT-2): momenta = CUDA float64 tensor [24, n_events]; returns out_w [n_events]."""
     import torch
+    _check_tensor(handle, momenta, "momenta", 24)
     n_events = int(momenta.shape[1])
     if out_w is None:
         out_w = torch.empty(n_events, dtype=torch.float64, device=momenta.device)

@@ -83,14 +83,19 @@ struct mem_handle {
   int64_t grid_events;      // events covered by the grids of the last VEGAS call
   Buffer ecs, partials, grids, hist, stage_in, stage_out, pdf_tab;
   cudaEvent_t ev_begin, ev_end;  // around the dominant kernel of the last mem_integrate
+  cudaEvent_t ev_done;           // recorded after the last launch of every call that uses the workspace
+  bool has_done;                 // ev_done has been recorded at least once
   int64_t last_evals;            // integrand evaluations of that kernel; 0 = none yet
 };
 
 namespace {
 
-mem_status ensure(Buffer& b, size_t bytes, cudaStream_t st) {
+// Grow-only workspace.  A growth step frees the old allocation, so it first waits for every kernel that may still
+// read it: the last call on this handle (whatever stream it ran on) and the current stream.
+mem_status ensure(mem_handle* h, Buffer& b, size_t bytes, cudaStream_t st) {
   if (bytes <= b.cap) return MEM_OK;
   if (b.p) {
+    if (h->has_done) CUDA_TRY(cudaEventSynchronize(h->ev_done));
     CUDA_TRY(cudaStreamSynchronize(st));
     CUDA_TRY(cudaFree(b.p));
     b.p = nullptr; b.cap = 0;
@@ -108,6 +113,40 @@ mem_status ensure(Buffer& b, size_t bytes, cudaStream_t st) {
     return fail(MEM_ERR_NOMEM, "cudaMalloc(%zu bytes): %s", want, cudaGetErrorString(e));
   }
   b.cap = want;
+  return MEM_OK;
+}
+
+// Every entry point that launches on a handle: the current device must be the handle's.
+mem_status check_device(const mem_handle* h) {
+  int dev = -1;
+  CUDA_TRY(cudaGetDevice(&dev));
+  if (dev != h->device)
+    return fail(MEM_ERR_INVALID_ARG, "handle was created on device %d, the current device is %d", h->device, dev);
+  return MEM_OK;
+}
+// ... and the event index must fit the 32-bit Philox counter word
+mem_status check_counter(const mem_handle* h, int64_t n_events) {
+  if (h->event_offset + (uint64_t)n_events > 0x100000000ULL)
+    return fail(MEM_ERR_INVALID_ARG, "event index exceeds the 32-bit Philox counter word");
+  return MEM_OK;
+}
+
+// One handle, several streams: the workspace (per-event constants, partial sums, grids, histograms) is shared by
+// consecutive calls, so a call first makes its stream wait for the previous call on this handle (a no-op when that
+// ran on the same stream) and leaves an event behind for the next one.  While the stream is being captured into a
+// CUDA graph neither is done (events recorded outside a capture cannot be waited on inside it): the caller then owns
+// the handle exclusively for the lifetime of the graph.
+mem_status begin_call(mem_handle* h, cudaStream_t st, bool* capturing) {
+  cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+  CUDA_TRY(cudaStreamIsCapturing(st, &cs));
+  *capturing = cs != cudaStreamCaptureStatusNone;
+  if (!*capturing && h->has_done) CUDA_TRY(cudaStreamWaitEvent(st, h->ev_done, 0));
+  return MEM_OK;
+}
+mem_status end_call(mem_handle* h, cudaStream_t st, bool capturing) {
+  if (capturing) return MEM_OK;
+  CUDA_TRY(cudaEventRecord(h->ev_done, st));
+  h->has_done = true;
   return MEM_OK;
 }
 
@@ -262,7 +301,7 @@ size_t integrate_smem(int NC, int D, int B, int mode) {   // NC = constants per 
 template <class P>
 mem_status launch_prepare(mem_handle* h, const double* events, int64_t n_events, cudaStream_t st) {
   const int64_t n_rec = n_events * h->dc.n_perm;            // one block of NC constants per (event, assignment)
-  mem_status s = ensure(h->ecs, (size_t)n_rec * P::NC * sizeof(double), st);
+  mem_status s = ensure(h, h->ecs, (size_t)n_rec * P::NC * sizeof(double), st);
   if (s != MEM_OK) return s;
   const int threads = 128;
   prepare_kernel<P><<<(unsigned)((n_rec + threads - 1) / threads), threads, 0, st>>>(
@@ -308,23 +347,27 @@ int64_t chunk_for(int64_t n_points) {
 // the pass that produces the outputs, bracketed by the handle's events
 template <class P, int MODE>
 mem_status launch_timed_pass(mem_handle* h, int64_t n_events, int64_t n_points, int n_chunks, uint64_t seed,
-                             uint32_t pass, cudaStream_t st) {
-  CUDA_TRY(cudaEventRecord(h->ev_begin, st));
+                             uint32_t pass, cudaStream_t st, bool capturing) {
+  // no event records inside a stream capture: they would belong to the graph and mem_last_pass_ms could not read them
+  if (!capturing) CUDA_TRY(cudaEventRecord(h->ev_begin, st));
   mem_status s = launch_pass<P, MODE>(h, n_events, n_points, chunk_for(n_points), n_chunks, seed, pass, st);
   if (s != MEM_OK) return s;
-  CUDA_TRY(cudaEventRecord(h->ev_end, st));
-  h->last_evals = n_events * n_points;
+  if (!capturing) CUDA_TRY(cudaEventRecord(h->ev_end, st));
+  h->last_evals = capturing ? 0 : n_events * n_points;
   return MEM_OK;
 }
 
 template <class P>
 mem_status integrate_impl(mem_handle* h, const double* events, int64_t n_events, int64_t n_points, uint64_t seed,
                           double* out_p, double* out_err, cudaStream_t st) {
-  mem_status s = launch_prepare<P>(h, events, n_events, st);
+  bool capturing = false;
+  mem_status s = begin_call(h, st, &capturing);
+  if (s != MEM_OK) return s;
+  s = launch_prepare<P>(h, events, n_events, st);
   if (s != MEM_OK) return s;
   const int64_t chunk = chunk_for(n_points);
   const int n_chunks = (int)((n_points + chunk - 1) / chunk);
-  s = ensure(h->partials, (size_t)n_events * n_chunks * 2 * sizeof(double), st);
+  s = ensure(h, h->partials, (size_t)n_events * n_chunks * 2 * sizeof(double), st);
   if (s != MEM_OK) return s;
   const mem_params& p = h->params;
   if (p.vegas_iters > 0) {
@@ -334,12 +377,12 @@ mem_status integrate_impl(mem_handle* h, const double* events, int64_t n_events,
     if (a_chunk < chunk_for(p.vegas_points)) a_chunk = chunk_for(p.vegas_points);
     a_chunk = (a_chunk + kThreads - 1) / kThreads * kThreads;
     const int a_chunks = (int)((p.vegas_points + a_chunk - 1) / a_chunk);
-    s = ensure(h->grids, (size_t)n_events * D * (B + 1) * sizeof(double), st);
+    s = ensure(h, h->grids, (size_t)n_events * D * (B + 1) * sizeof(double), st);
     if (s != MEM_OK) return s;
-    s = ensure(h->hist, (size_t)n_events * a_chunks * D * B * sizeof(double), st);
+    s = ensure(h, h->hist, (size_t)n_events * a_chunks * D * B * sizeof(double), st);
     if (s != MEM_OK) return s;
     if (a_chunks > n_chunks) {
-      s = ensure(h->partials, (size_t)n_events * a_chunks * 2 * sizeof(double), st);
+      s = ensure(h, h->partials, (size_t)n_events * a_chunks * 2 * sizeof(double), st);
       if (s != MEM_OK) return s;
     }
     const int64_t ng = n_events * D * (B + 1);
@@ -355,23 +398,26 @@ mem_status integrate_impl(mem_handle* h, const double* events, int64_t n_events,
       CUDA_TRY(cudaGetLastError());
     }
     h->grid_events = n_events;
-    s = launch_timed_pass<P, MODE_GRID>(h, n_events, n_points, n_chunks, seed, (uint32_t)p.vegas_iters, st);
+    s = launch_timed_pass<P, MODE_GRID>(h, n_events, n_points, n_chunks, seed, (uint32_t)p.vegas_iters, st, capturing);
   } else {
-    s = launch_timed_pass<P, MODE_PLAIN>(h, n_events, n_points, n_chunks, seed, 0u, st);
+    s = launch_timed_pass<P, MODE_PLAIN>(h, n_events, n_points, n_chunks, seed, 0u, st, capturing);
   }
   if (s != MEM_OK) return s;
   finalize_kernel<<<(unsigned)((n_events + 127) / 128), 128, 0, st>>>((const double*)h->partials.p, n_chunks,
                                                                       n_events, n_points, out_p, out_err);
   ++h->launches;
   CUDA_TRY(cudaGetLastError());
-  return MEM_OK;
+  return end_call(h, st, capturing);
 }
 
 template <class P>
 mem_status eval_impl(mem_handle* h, const double* events, int64_t n_events, int64_t event, int64_t first,
                      int64_t n, uint64_t seed, int32_t iteration, const double* grid, double* out_w,
                      cudaStream_t st) {
-  mem_status s = launch_prepare<P>(h, events, n_events, st);
+  bool capturing = false;
+  mem_status s = begin_call(h, st, &capturing);
+  if (s != MEM_OK) return s;
+  s = launch_prepare<P>(h, events, n_events, st);
   if (s != MEM_OK) return s;
   const int threads = 128;
   const size_t smem = ((size_t)P::NC * h->dc.n_perm + (size_t)P::D * (kMaxBins + 1)) * sizeof(double);
@@ -379,7 +425,7 @@ mem_status eval_impl(mem_handle* h, const double* events, int64_t n_events, int6
       dc_of<typename P::real>(h), (const double*)h->ecs.p, event, grid, first, n, make_philox(seed), h->event_offset, (uint32_t)iteration, out_w);
   ++h->launches;
   CUDA_TRY(cudaGetLastError());
-  return MEM_OK;
+  return end_call(h, st, capturing);
 }
 
 }  // namespace
@@ -437,9 +483,10 @@ mem_status mem_create(mem_process process, const mem_params* params, mem_handle*
   mem_handle* h = new (std::nothrow) mem_handle();
   if (!h) return fail(MEM_ERR_NOMEM, "out of host memory");
   h->process = (int)process; h->device = dev; h->params = p; h->dc = make_dev_const(p); h->dcf = to_float(h->dc);
-  h->event_offset = 0; h->launches = 0; h->grid_events = 0; h->last_evals = 0;
+  h->event_offset = 0; h->launches = 0; h->grid_events = 0; h->last_evals = 0; h->has_done = false;
   cudaError_t ce = cudaEventCreate(&h->ev_begin);
   if (ce == cudaSuccess) ce = cudaEventCreate(&h->ev_end);
+  if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&h->ev_done, cudaEventDisableTiming);
   if (ce != cudaSuccess) {
     delete h;
     return fail(MEM_ERR_CUDA, "cudaEventCreate: %s", cudaGetErrorString(ce));
@@ -450,12 +497,18 @@ mem_status mem_create(mem_process process, const mem_params* params, mem_handle*
 
 mem_status mem_destroy(mem_handle* h) {
   if (!h) return MEM_OK;
+  // synchronise and free on the handle's own device, whatever device is current, and restore the caller's
+  int cur = -1;
+  const bool have_cur = cudaGetDevice(&cur) == cudaSuccess;
+  if (have_cur && cur != h->device) cudaSetDevice(h->device);
   cudaDeviceSynchronize();
   Buffer* bs[] = {&h->ecs, &h->partials, &h->grids, &h->hist, &h->stage_in, &h->stage_out, &h->pdf_tab};
   for (Buffer* b : bs)
     if (b->p) cudaFree(b->p);
   cudaEventDestroy(h->ev_begin);
   cudaEventDestroy(h->ev_end);
+  cudaEventDestroy(h->ev_done);
+  if (have_cur && cur != h->device) cudaSetDevice(cur);
   delete h;
   return MEM_OK;
 }
@@ -487,9 +540,14 @@ static mem_status measure_fp64(int kind, int32_t repeats, double* tflops, void* 
   CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
   double* sink = nullptr;
   CUDA_TRY(cudaMalloc(&sink, sizeof(double)));
-  cudaEvent_t a, b;
-  CUDA_TRY(cudaEventCreate(&a));
-  CUDA_TRY(cudaEventCreate(&b));
+  cudaEvent_t a = nullptr, b = nullptr;
+  cudaError_t ce = cudaEventCreate(&a);
+  if (ce == cudaSuccess) ce = cudaEventCreate(&b);
+  if (ce != cudaSuccess) {
+    cudaFree(sink);
+    if (a) cudaEventDestroy(a);
+    return fail(MEM_ERR_CUDA, "cudaEventCreate: %s", cudaGetErrorString(ce));
+  }
   const int blocks = sms * 8 * 4, threads = 256;           // 4 waves of 8 resident blocks per SM
   double best = 0.0;
   for (int r = 0; r < repeats + 1; ++r) {                  // first launch is the warm-up
@@ -540,14 +598,9 @@ mem_status mem_integrate(mem_handle* h, const double* events, int64_t n_events, 
   if (!events || !out_p || !out_err) return fail(MEM_ERR_INVALID_ARG, "events / out_p / out_err is NULL");
   if (!aligned8(events) || !aligned8(out_p) || !aligned8(out_err))
     return fail(MEM_ERR_INVALID_ARG, "device pointers must be 8-byte aligned");
-  {
-    int dev = -1;
-    CUDA_TRY(cudaGetDevice(&dev));
-    if (dev != h->device)
-      return fail(MEM_ERR_INVALID_ARG, "handle was created on device %d, the current device is %d", h->device, dev);
-  }
-  if (h->event_offset + (uint64_t)n_events > 0x100000000ULL)
-    return fail(MEM_ERR_INVALID_ARG, "event index exceeds the 32-bit Philox counter word");
+  mem_status cs = check_device(h);
+  if (cs == MEM_OK) cs = check_counter(h, n_events);
+  if (cs != MEM_OK) return cs;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   switch (h->process) {
     case MEM_PROC_W_ENU: return integrate_impl<ProcWenu>(h, events, n_events, n_points, seed, out_p, out_err, st);
@@ -563,18 +616,22 @@ mem_status mem_integrate(mem_handle* h, const double* events, int64_t n_events, 
 }
 
 mem_status mem_integrate_host(mem_handle* h, const double* events_host, int64_t n_events, int64_t n_points,
-                              uint64_t seed, double* out_p_host, double* out_err_host) {
+                              uint64_t seed, double* out_p_host, double* out_err_host, void* cuda_stream) {
   if (!h) return fail(MEM_ERR_INVALID_ARG, "handle is NULL");
   if (n_events < 0) return fail(MEM_ERR_INVALID_ARG, "n_events < 0");
   if (n_points < 2) return fail(MEM_ERR_INVALID_ARG, "n_points < 2");
   if (n_events == 0) return MEM_OK;
   if (!events_host || !out_p_host || !out_err_host) return fail(MEM_ERR_INVALID_ARG, "a host buffer is NULL");
+  mem_status s = check_device(h);
+  if (s != MEM_OK) return s;
   const size_t in_bytes = (size_t)n_events * n_fields_of(h->process) * sizeof(double);
   const size_t out_bytes = (size_t)n_events * sizeof(double);
-  cudaStream_t st = 0;
-  mem_status s = ensure(h->stage_in, in_bytes, st);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  // the staging buffers belong to the workspace: order this call after the previous one before touching them
+  if (h->has_done) CUDA_TRY(cudaStreamWaitEvent(st, h->ev_done, 0));
+  s = ensure(h, h->stage_in, in_bytes, st);
   if (s != MEM_OK) return s;
-  s = ensure(h->stage_out, 2 * out_bytes, st);
+  s = ensure(h, h->stage_out, 2 * out_bytes, st);
   if (s != MEM_OK) return s;
   double* d_out = (double*)h->stage_out.p;
   CUDA_TRY(cudaMemcpyAsync(h->stage_in.p, events_host, in_bytes, cudaMemcpyHostToDevice, st));
@@ -582,6 +639,7 @@ mem_status mem_integrate_host(mem_handle* h, const double* events_host, int64_t 
   if (s != MEM_OK) return s;
   CUDA_TRY(cudaMemcpyAsync(out_p_host, d_out, out_bytes, cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaMemcpyAsync(out_err_host, d_out + n_events, out_bytes, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaEventRecord(h->ev_done, st));          // the copies out read the staging buffer too
   CUDA_TRY(cudaStreamSynchronize(st));
   return MEM_OK;
 }
@@ -599,6 +657,9 @@ mem_status mem_eval_points(mem_handle* h, const double* events, int64_t n_events
     return fail(MEM_ERR_INVALID_ARG, "device pointers must be 8-byte aligned");
   if (grid && (h->params.vegas_bins < 1 || h->params.vegas_bins > kMaxBins))
     return fail(MEM_ERR_INVALID_ARG, "vegas_bins outside 1..%d", kMaxBins);
+  mem_status cs = check_device(h);
+  if (cs == MEM_OK) cs = check_counter(h, n_events);
+  if (cs != MEM_OK) return cs;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   switch (h->process) {
     case MEM_PROC_W_ENU: return eval_impl<ProcWenu>(h, events, n_events, event, first_point, n, seed, iteration, grid, out_w, st);
@@ -616,6 +677,11 @@ mem_status mem_eval_points(mem_handle* h, const double* events, int64_t n_events
 mem_status mem_set_pdf_grid(mem_handle* h, const double* table, int32_t nx, int32_t nq, double lxmin, double lxmax,
                             double lqmin, double lqmax, double Q) {
   if (!h) return fail(MEM_ERR_INVALID_ARG, "handle is NULL");
+  mem_status cs = check_device(h);
+  if (cs != MEM_OK) return cs;
+  // kernels in flight on any stream (torch side streams do not synchronise with the legacy stream) may still read
+  // the table that is about to be replaced or dropped
+  CUDA_TRY(cudaDeviceSynchronize());
   if (!table) {                                             // back to the toy PDF
     h->dc.pdf_tab = nullptr;
     return MEM_OK;
@@ -639,7 +705,7 @@ mem_status mem_set_pdf_grid(mem_handle* h, const double* table, int32_t nx, int3
       row[(size_t)s * nx + ix] = (d0 * (c22q - lq) + d1 * (lq - c11q)) / dq;
     }
   cudaStream_t st = 0;
-  mem_status r = ensure(h->pdf_tab, (size_t)6 * nx * sizeof(double), st);
+  mem_status r = ensure(h, h->pdf_tab, (size_t)6 * nx * sizeof(double), st);
   cudaError_t e = cudaSuccess;
   if (r == MEM_OK) {
     e = cudaMemcpy(h->pdf_tab.p, row, (size_t)6 * nx * sizeof(double), cudaMemcpyHostToDevice);   // synchronous
@@ -663,6 +729,8 @@ mem_status mem_eval_parton(mem_handle* h, const double* momenta, int64_t n_event
   if (n_events == 0) return MEM_OK;
   if (!momenta || !out_w) return fail(MEM_ERR_INVALID_ARG, "momenta / out_w is NULL");
   if (!aligned8(momenta) || !aligned8(out_w)) return fail(MEM_ERR_INVALID_ARG, "device pointers must be 8-byte aligned");
+  mem_status cs = check_device(h);
+  if (cs != MEM_OK) return cs;
   const int threads = 128;
   const int64_t blocks = (n_events + threads - 1) / threads;
   if (blocks > 0x7fffffffLL) return fail(MEM_ERR_INVALID_ARG, "n_events exceeds the grid limit");
@@ -699,9 +767,15 @@ mem_status mem_get_grid(mem_handle* h, int64_t n_events, double* out_grid, void*
   if (!h || !out_grid) return fail(MEM_ERR_INVALID_ARG, "handle / out_grid is NULL");
   if (h->params.vegas_iters <= 0 || !h->grids.p || n_events != h->grid_events)
     return fail(MEM_ERR_INVALID_ARG, "no VEGAS grids for %lld events on this handle", (long long)n_events);
+  mem_status cs = check_device(h);
+  if (cs != MEM_OK) return cs;
   const size_t bytes = (size_t)n_events * n_dims_of(h->process) * (h->params.vegas_bins + 1) * sizeof(double);
-  CUDA_TRY(cudaMemcpyAsync(out_grid, h->grids.p, bytes, cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream));
-  return MEM_OK;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  bool capturing = false;
+  cs = begin_call(h, st, &capturing);
+  if (cs != MEM_OK) return cs;
+  CUDA_TRY(cudaMemcpyAsync(out_grid, h->grids.p, bytes, cudaMemcpyDeviceToDevice, st));
+  return end_call(h, st, capturing);
 }
 
 }  // extern "C"
