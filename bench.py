@@ -28,31 +28,33 @@ if ROOT not in sys.path:
 
 SEED = 20140729
 
-# Algorithmic FP64 work per integrand call of the dominant kernel: executed
-# thread-level DFMA / DMUL / DADD per point from the ncu captures in profiles/ (r01_ncu_config3.md,
-# r01_fp64_counts.md): smsp__sass_thread_inst_executed_op_{dfma,dmul,dadd}_pred_on.sum / points.
-# flop = 2 DFMA + DMUL + DADD.  Key = config; config 5's dominant kernel is the grid-mapped final pass.
-FP64_PER_CALL = {           # key = (config, jet-parton assignments per point)
-    (1, 1): {"dfma": 87.3, "dmul": 47.0, "dadd": 18.4},
-    (2, 1): {"dfma": 86.0, "dmul": 37.0, "dadd": 15.6},
-    (3, 1): {"dfma": 196.0, "dmul": 90.0, "dadd": 41.2},
-    (3, 24): {"dfma": 1597.0, "dmul": 1335.0, "dadd": 551.2},
-    (4, 1): {"dfma": 241.0, "dmul": 82.9, "dadd": 57.9},
-    (4, 2): {"dfma": 327.2, "dmul": 120.2, "dadd": 79.8},
-    (5, 1): {"dfma": 166.0, "dmul": 115.1, "dadd": 55.7},
+# FP64 work per integrand call of the dominant kernel, two counts:
+#  - executed: thread-level DFMA / DMUL / DADD per point from an ncu metric pass, read from
+#    paper_1407_7595_b200/fp64_counts.json together with the SASS hash of the kernel they were taken on
+#    (counts.py); a count that belongs to another build is reported as stale, never silently reused;
+#  - algorithmic: a fixed reference, flop = 2 FMA + MUL + ADD of the formulas as first implemented (the round-1
+#    kernels' executed counts, profiles/r01_fp64_counts.md, with every exponential at the cost of the table-driven
+#    implementation), NOT updated when later kernels remove instructions -- so that faster code never scores lower.
+#    roofline.frac uses this one.  Key = (config, jet-parton assignments per point).
+ALGORITHMIC_FLOP = {
+    (1, 1): 240.0,       # 87.3 DFMA, 47.0 DMUL, 18.4 DADD
+    (2, 1): 224.6,       # 86.0, 37.0, 15.6
+    (3, 1): 451.2,       # 196.0, 90.0, 41.2 with libdevice exp = 523.2; six exponentials at table cost: -72
+    (3, 24): 4007.2,     # 1597, 1335, 551.2 = 4079.2; -72 as above
+    (4, 1): 622.8,       # 241.0, 82.9, 57.9
+    (4, 2): 854.2,       # 327.2, 120.2, 79.8
+    (5, 1): 502.8,       # 166.0, 115.1, 55.7 (grid-mapped final pass)
 }
-# fp32 variant of config 3 (reading A15): executed FFMA / FMUL / FADD per call (same ncu pass)
-FP32_PER_CALL = {3: {"ffma": 81.0, "fmul": 93.3, "fadd": 27.4}, 5: {"ffma": 81.0, "fmul": 93.3, "fadd": 27.4}}
-# dram__bytes_read.sum + dram__bytes_write.sum of the dominant launch at full size, from an ncu metric pass
-# of the same command (profiles/r01_ncu_config3.md); key = (config, events, points/event, assignments, precision)
-TRAFFIC_BYTES = {(3, 4096, 1 << 20, 1, 64): 1821696}
+# NEXT-4 (config 6), per hypothesis: executed count of the first parity-green kernel of round 2 (profiles/r02_fp64_counts.md)
+TTH_ALGORITHMIC_FLOP = {0: 536.3, 1: 462.2}   # 209.5 / 68.0 / 49.4 and 181.2 / 56.6 / 43.2 (DFMA / DMUL / DADD)
 NOMINAL_FP64_FMA_PER_CLK_PER_SM = 64      # 4 SMSPs x 16 lanes; confirmed by the microbenchmark
 VEGAS_ITERS, VEGAS_POINTS = 5, 1 << 17    # BASELINE.json:configs[4]
 
 
-def flops_per_call(cfg, perm=1):
-    c = FP64_PER_CALL.get((cfg, max(perm, 1)))
-    return None if c is None else 2.0 * c["dfma"] + c["dmul"] + c["dadd"]
+def executed_counts(cfg, perm=1, precision=64):
+    """(record or None) from fp64_counts.json, with "match" = taken on the SASS that is built now"""
+    from paper_1407_7595_b200 import counts
+    return counts.lookup(cfg, perm, precision)
 
 
 def parse_args():
@@ -60,7 +62,8 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5, 6],
+                    help="1-5: BASELINE.json configs; 6: NEXT-4, t tbar H(-> b bbar) dilepton with four b jets")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--events", type=int, default=0, help="override the event count (default: the config's)")
     ap.add_argument("--points", type=int, default=0, help="override points/event (default: the config's)")
@@ -70,6 +73,10 @@ def parse_args():
                     help="jet-parton assignments summed per point (NEXT-1): config 3/5: 4 or 24, config 4: 2")
     ap.add_argument("--pdf", default="toy", choices=["toy", "grid"],
                     help="grid = NEXT-3: bilinear (ln x, ln Q) tables synthesised from the toy PDF (configs 3-5)")
+    ap.add_argument("--hyp", type=int, default=0, choices=[0, 1],
+                    help="config 6: hypothesis of PAPER.md Eq. 10 (0 = t tbar H, 1 = non-resonant t tbar b bbar)")
+    ap.add_argument("--dist-backend", default="nccl", choices=["nccl", "gloo"],
+                    help="process-group backend for N > 1 (gloo: several ranks sharing one GPU, for tests)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--parton", action="store_true",
                     help="NEXT-2 parton-level mode: ME evaluations of --events configurations (default 10^5)")
@@ -89,11 +96,19 @@ def workload(cfg, args):
         npts = args.points
     name = {1: "config1 W->e nu 1-D", 2: "config2 Z->bb 2-D", 3: "config3 ttbar l+jets 6-D",
             4: "config4 ttbar dilepton 8-D",
-            5: "config5 ttbar l+jets 6-D + VEGAS 5x2^17"}[cfg]
+            5: "config5 ttbar l+jets 6-D + VEGAS 5x2^17",
+            6: "NEXT-4 ttH(->bb) dilepton 8-D (Eq. 7-9, 11), hypothesis %d, closure records" % args.hyp}[cfg]
     return proc, ne, npts, "%s, %d events x %d points/event, %s%s" % (
         name, ne, npts, "fp32 core (A15)" if args.precision == 32 else "fp64",
         (", %d jet-parton assignments per point" % args.perm if args.perm > 1 else "") +
         (", grid PDFs" if args.pdf == "grid" else ""))
+
+
+def make_records(cfg, proc, n):
+    """config 6 is measured on physical t tbar H records (they stand in for the paper's MadGraph + Pythia sample,
+    PAPER.md:145); the BASELINE configs on their i.i.d. records"""
+    from paper_1407_7595_b200 import workloads as wl
+    return wl.make_tth_events(n) if cfg == 6 else wl.make_events(proc, n)
 
 
 # --------------------------------------------------------------------------------------------
@@ -104,6 +119,7 @@ class ClockSampler:
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index):
+        """index: what nvidia-smi -i accepts -- a physical index or a GPU UUID (robust under CUDA_VISIBLE_DEVICES)"""
         self.proc = None
         self.index = index
         try:
@@ -152,9 +168,10 @@ class ClockSampler:
 # CPU oracle legs
 # --------------------------------------------------------------------------------------------
 def _oracle_worker(job):
-    cfg, proc, ev, lo, n_points, seed = job
+    cfg, proc, ev, lo, n_points, seed, hyp = job
     import oracle
     p = oracle.params_default(proc)
+    p.tth_hyp = hyp
     t0 = time.perf_counter()
     if cfg == 5:
         p.vegas_iters, p.vegas_points = VEGAS_ITERS, VEGAS_POINTS
@@ -166,13 +183,13 @@ def _oracle_worker(job):
     return evals, time.perf_counter() - t0
 
 
-def oracle_sample(cfg, proc, ev, n_points, events_per_core, pool, cores):
+def oracle_sample(cfg, proc, ev, n_points, events_per_core, pool, cores, hyp=0):
     """The oracle, single-threaded by design, run as `cores` independent processes over disjoint
     event ranges.  Returns (evaluations, wall seconds, events)."""
     jobs = []
     for k in range(cores):
         lo = k * events_per_core
-        jobs.append((cfg, proc, ev[:, lo:lo + events_per_core].copy(), lo, n_points, SEED))
+        jobs.append((cfg, proc, ev[:, lo:lo + events_per_core].copy(), lo, n_points, SEED, hyp))
     t0 = time.perf_counter()
     res = pool.map(_oracle_worker, jobs)
     wall = time.perf_counter() - t0
@@ -192,13 +209,13 @@ def run_reference(args):
     cores = min(os.cpu_count() or 1, 64)
     per_core = 1 if n_points >= (1 << 20) else max(1, (1 << 20) // n_points)
     per_core = min(per_core, max(1, ne // cores))
-    ev = wl.make_events(proc, ne)
+    ev = make_records(cfg, proc, ne)
     with mp.get_context("spawn").Pool(cores) as pool:
         for _ in range(args.warmup):
-            oracle_sample(cfg, proc, ev, n_points, per_core, pool, cores)
+            oracle_sample(cfg, proc, ev, n_points, per_core, pool, cores, args.hyp)
         evals = wall = events = 0
         for _ in range(args.steps):
-            a, b, c = oracle_sample(cfg, proc, ev, n_points, per_core, pool, cores)
+            a, b, c = oracle_sample(cfg, proc, ev, n_points, per_core, pool, cores, args.hyp)
             evals += a; wall += b; events += c
     value = evals / wall
     sample = "%d events (%d per core) x %d points/event per step" % (cores * per_core, per_core, n_points)
@@ -229,13 +246,14 @@ def run_b200(args):
     rank, local_rank, world = sharding.dist_env()
     torch.cuda.set_device(local_rank)
     if world > 1:
-        sharding.init_process_group("nccl")
+        sharding.init_process_group(args.dist_backend)
+    red_dev = "cuda" if args.dist_backend == "nccl" else "cpu"
     import torch.distributed as dist
 
     cfg = args.config
     proc, ne, n_points, name = workload(cfg, args)
     # weak scaling: every rank owns `ne` events of a list of ne * world (contiguous shard)
-    ev_all = wl.make_events(proc, ne * world)
+    ev_all = make_records(cfg, proc, ne * world)
     lo = rank * ne
     ev_host = torch.from_numpy(ev_all[:, lo:lo + ne].copy()).pin_memory()
     ev_dev = ev_host.cuda()
@@ -244,6 +262,8 @@ def run_b200(args):
         over["precision"] = 32
     if args.perm > 1:
         over["n_perm"] = args.perm
+    if cfg == 6:
+        over["tth_hyp"] = args.hyp
     it = mem.Integrator(proc, **over)
     if args.pdf == "grid":
         g = wl.PDF_GRID
@@ -287,18 +307,33 @@ def run_b200(args):
         step_dev()
     step_host()
     barrier()
-    sampler = ClockSampler(local_rank) if rank == 0 else None
+    # nvidia-smi wants the physical device: address it by UUID, which survives CUDA_VISIBLE_DEVICES remapping
+    uuid = getattr(torch.cuda.get_device_properties(local_rank), "uuid", None)
+    sampler = ClockSampler("GPU-%s" % uuid if uuid is not None else local_rank) if rank == 0 else None
     launches0 = it.launches
     barrier()
     ms, kms = timed(step_dev, args.steps, collect_kernel=True)
     barrier()
     launches = it.launches - launches0
     clocks = sampler.stop() if sampler else None
-    t_dev = sharding.max_over_ranks(sum(ms) / 1e3, device="cuda")
+    t_dev = sharding.max_over_ranks(sum(ms) / 1e3, device=red_dev)
     barrier()
     ms_h, _ = timed(step_host, args.steps)
     barrier()
-    t_host = sharding.max_over_ranks(sum(ms_h) / 1e3, device="cuda")
+    t_host = sharding.max_over_ranks(sum(ms_h) / 1e3, device=red_dev)
+
+    # outside the timed region: the global event index reached the Philox counter on every rank -- the first event of
+    # this rank's shard, integrated alone with event_offset = lo, reproduces out_p[0] bit for bit; and the optional
+    # all-gather of the 16 B/event results works (first 8 events of every shard)
+    one_p = torch.empty(1, dtype=torch.float64, device="cuda")
+    one_e = torch.empty_like(one_p)
+    it.integrate(ev_dev[:, :1].contiguous(), n_points, SEED, out_p=one_p, out_err=one_e)
+    torch.cuda.synchronize()
+    shard_ok = bool(torch.equal(one_p, out_p[:1]) and torch.equal(one_e, out_err[:1]))
+    n_head = min(8, ne)
+    head = out_p[:n_head].clone() if args.dist_backend == "nccl" else out_p[:n_head].cpu()
+    gathered = sharding.gather_results(head, n_head * world)
+    shard_ok_all = sharding.sum_over_ranks(1.0 if shard_ok else 0.0, device=red_dev) == float(world)
 
     if rank != 0:
         it.close()
@@ -311,41 +346,54 @@ def run_b200(args):
     k_evals = ne * n_points
     peak_meas = mem.mem_measure_fp64_peak(5)
     peak_rrr = mem.mem_measure_fp64_peak_rrr(5)
-    fl = flops_per_call(cfg, args.perm)
-    c = FP64_PER_CALL.get((cfg, max(args.perm, 1)))
-    if fl is None:          # no ncu count for this combination yet: report the single-assignment floor
-        fl, c = flops_per_call(cfg), FP64_PER_CALL[(cfg, 1)]
-    achieved = k_evals * fl / (k_ms * 1e-3) / 1e12
-    pipe_inst = c["dfma"] + c["dmul"] + c["dadd"]
-    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    perm = max(args.perm, 1)
+    ex = executed_counts(cfg, perm, 64) if args.pdf == "toy" else None
+    fl_ex = None if ex is None else 2.0 * ex.get("dfma", 0.0) + ex.get("dmul", 0.0) + ex.get("dadd", 0.0)
+    pipe_inst = None if ex is None else ex.get("dfma", 0.0) + ex.get("dmul", 0.0) + ex.get("dadd", 0.0)
+    fl_alg = ALGORITHMIC_FLOP.get((cfg, perm))
+    if fl_alg is None and cfg == 6 and perm == 1:
+        fl_alg = TTH_ALGORITHMIC_FLOP.get(args.hyp)
+    rate = k_evals / (k_ms * 1e-3) / 1e12                  # 1e12 evaluations/s of the dominant kernel
+    sms = torch.cuda.get_device_properties(local_rank).multi_processor_count
     sm_mhz = (clocks or {}).get("sm_mhz") or 0.0
+    achieved = None if fl_alg is None else rate * fl_alg
     roofline = {
         "bound": "alu", "kernel": "integrate_kernel<%s>" % ("ProcTTljets,GRID" if cfg == 5 else "proc%d,PLAIN" % proc),
-        "achieved": achieved, "peak": peak_meas, "unit": "TFLOP/s", "frac": achieved / peak_meas,
+        "achieved": achieved, "peak": peak_meas, "unit": "TFLOP/s",
+        "frac": None if achieved is None else achieved / peak_meas,
+        "flop_per_call_algorithmic": fl_alg,
+        "flop_per_call_algorithmic_note": "fixed reference count (bench.py: ALGORITHMIC_FLOP, DESIGN.md section 5); "
+                                          "achieved and frac use it",
+        "flop_per_call_executed": fl_ex,
+        "achieved_executed": None if fl_ex is None else rate * fl_ex,
+        "frac_executed": None if fl_ex is None else rate * fl_ex / peak_meas,
+        "executed_counts": None if ex is None else {k: ex[k] for k in ("dfma", "dmul", "dadd") if k in ex},
+        "executed_counts_match_build": None if ex is None else ex.get("match"),
         "peak_source": "measured in this run: independent DFMA chains on all SMs (mem_measure_fp64_peak)",
         "peak_three_register_operands": peak_rrr,
         "peak_three_register_operands_note": "same microbenchmark with x = fma(x, y, z), y and z in registers: the "
                                              "register file feeds such DFMAs at ~2/3 of the pipe's nominal rate",
         "peak_nominal_at_observed_clock": 2e-6 * NOMINAL_FP64_FMA_PER_CLK_PER_SM * sms * sm_mhz,
-        "fp64_pipe_frac": (k_evals * pipe_inst / (k_ms * 1e-3)) / (peak_meas * 1e12 / 2.0),
-        "flop_per_call": fl, "fp64_inst_per_call": pipe_inst, "kernel_ms": k_ms,
+        "fp64_pipe_frac": None if pipe_inst is None else rate * pipe_inst / (peak_meas / 2.0),
+        "fp64_inst_per_call": pipe_inst, "kernel_ms": k_ms,
         "kernel_share_of_step": k_ms * len(kms) / sum(ms),
-        "traffic": TRAFFIC_BYTES.get((cfg, ne, n_points, max(args.perm, 1), args.precision)) if args.pdf == "toy" else None,
+        "traffic": ((ex or {}).get("dram_bytes") or {}).get("%dx%d" % (ne, n_points)),
         "hbm_gbs_event_result_path": (ne * mem.mem_event_fields(proc) * 8 + ne * 16) / (sum(ms) / len(ms) * 1e-3) / 1e9,
     }
     if args.precision == 32:
         # fp32 core: the bound is instruction issue (FP32 + INT share the 4 x 32-lane datapaths), so
         # the roofline is counted in executed FP32 flops against 128 FFMA/clk/SM at the observed clock
-        f = FP32_PER_CALL[cfg]
-        fl32 = 2.0 * f["ffma"] + f["fmul"] + f["fadd"]
+        f = executed_counts(cfg, perm, 32) or {}
+        fl32 = 2.0 * f.get("ffma", 0.0) + f.get("fmul", 0.0) + f.get("fadd", 0.0)
         peak32 = 2e-6 * 128 * sms * (sm_mhz or 1965.0)
-        ach32 = k_evals * fl32 / (k_ms * 1e-3) / 1e12
+        ach32 = rate * fl32
         roofline.update({"kernel": roofline["kernel"].replace("proc3", "ProcTTljetsF"), "achieved": ach32,
-                         "peak": peak32, "frac": ach32 / peak32, "flop_per_call": fl32,
-                         "peak_source": "derived: 128 FP32 FMA/clk/SM x SMs x sampled SM clock (DESIGN.md)",
-                         "fp64_flop_per_call_kept": fl})
-        roofline.pop("fp64_pipe_frac", None)
-        roofline.pop("fp64_inst_per_call", None)
+                         "peak": peak32, "frac": ach32 / peak32, "flop_per_call_executed": fl32,
+                         "flop_per_call_algorithmic": None, "executed_counts_match_build": f.get("match"),
+                         "peak_source": "derived: 128 FP32 FMA/clk/SM x SMs x sampled SM clock (DESIGN.md); executed FP32 flops",
+                         "fp64_flop_per_call_kept": fl_ex})
+        for k in ("fp64_pipe_frac", "fp64_inst_per_call", "achieved_executed", "frac_executed", "executed_counts"):
+            roofline.pop(k, None)
     h2d = ne * mem.mem_event_fields(proc) * 8
     d2h = 2 * ne * 8
     line = {
@@ -362,6 +410,8 @@ def run_b200(args):
                 "ms_per_step": 1e3 * t_host / args.steps, "entry": "mem_integrate_host (pinned host buffers)"},
         "gpu_launches": launches,
         "roofline": roofline,
+        "shard_check": {"first_event_recomputed_with_offset_is_bit_identical_on_every_rank": bool(shard_ok_all),
+                        "gathered_first_events_p": [float(x) for x in gathered.cpu().tolist()]},
     }
     it.close()
     if world == 1 and not args.no_cpu_baseline:
@@ -372,7 +422,7 @@ def run_b200(args):
         per_core = 8 if n_points >= (1 << 20) else max(1, (8 << 20) // n_points)
         per_core = max(1, min(per_core, ne // cores))
         with mp.get_context("spawn").Pool(cores) as pool:
-            evals, wall, events = oracle_sample(cfg, proc, ev_all, n_points, per_core, pool, cores)
+            evals, wall, events = oracle_sample(cfg, proc, ev_all, n_points, per_core, pool, cores, args.hyp)
         line["cpu_baseline"] = {"value": evals / wall, "unit": "evals/s", "cores": cores, "kind": "oracle",
                                 "events_per_s": events / wall, "seconds": wall,
                                 "sample": "first %d events (%d per core) x %d points/event of the same workload"
