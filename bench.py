@@ -244,6 +244,7 @@ def run_b200(args):
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
     rank, local_rank, world = sharding.dist_env()
+    local_rank %= torch.cuda.device_count()         # several ranks may share a GPU in a plumbing test (--dist-backend gloo)
     torch.cuda.set_device(local_rank)
     if world > 1:
         sharding.init_process_group(args.dist_backend)

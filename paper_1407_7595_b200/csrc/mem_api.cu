@@ -316,9 +316,11 @@ mem_status launch_pass(mem_handle* h, int64_t n_events, int64_t n_points, int64_
                        uint64_t seed, uint32_t pass, cudaStream_t st) {
   const int64_t blocks = n_events * n_chunks;
   if (blocks > 0x7fffffffLL) return fail(MEM_ERR_INVALID_ARG, "n_events * chunks = %lld exceeds the grid limit", (long long)blocks);
-  // lane-compacting kernels keep two queues of 64 32-bit point offsets per warp
-  const size_t smem = integrate_smem(P::NC * h->dc.n_perm, P::D, h->dc.vegas_bins, MODE) +
-                      ((P::kCompact && MODE == MODE_PLAIN) ? (size_t)kWarps * 128 * sizeof(uint32_t) : 0);
+  // lane-compacting kernels keep (classes + 1) queues of 64 32-bit point offsets per warp, plus their counters
+  size_t smem = integrate_smem(P::NC * h->dc.n_perm, P::D, h->dc.vegas_bins, MODE);
+  if constexpr (P::kCompact) {
+    if (MODE == MODE_PLAIN) smem += (size_t)kWarps * ((P::kClasses + 1) * 64 + 2 * (P::kClasses + 1) + 2) * sizeof(uint32_t);
+  }
   auto launch = [&](auto perm, auto grid) {
     integrate_kernel<P, MODE, decltype(perm)::value, decltype(grid)::value><<<(unsigned)blocks, kThreads, smem, st>>>(
         dc_of<typename P::real>(h), (const double*)h->ecs.p, (const double*)h->grids.p, (double*)h->partials.p,

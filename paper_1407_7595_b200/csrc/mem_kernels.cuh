@@ -124,58 +124,86 @@ integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__
   const int64_t hi = (lo + chunk < n_points) ? lo + chunk : n_points;
   double s1 = 0.0, s2 = 0.0;
   if constexpr (P::kCompact && MODE == MODE_PLAIN && !PERM) {
-    // Lane compaction (config 4).  Most points have no kinematic solution, and the ones that do are
-    // scattered over the warp, so the long per-solution part would run with a few lanes active.
-    // Pass A: every lane takes one point up to the quartic and learns its number of real roots.
-    // Points with roots are queued per warp (two queues: 2 roots, 4 roots, so that a batch has a
-    // uniform trip count) as 32-bit offsets; whenever a queue holds 32 entries the warp runs the
-    // full integrand on them, all lanes active (pass B recomputes the point from its counter:
-    // cheaper than carrying 13 doubles of state per entry through shared memory).  The order in
-    // which a lane meets its points depends only on the data, so the sums stay reproducible.
-    // Measured on config 4: +9.5 % (1.50e10 -> 1.64e10 evaluations/s); with two assignments per point
-    // pass A doubles and the scheme loses 30 %, so the assignment sum keeps the plain loop.
-    uint32_t* q = reinterpret_cast<uint32_t*>(edges) + (threadIdx.x >> 5) * 128;   // [2][64] per warp
+    // Staged lane compaction (the conic-solver processes: config 4, NEXT-4).  Most points die early -- at the cheap
+    // kinematic tests, or because the two conics do not intersect -- and the survivors are scattered over the warp, so
+    // a plain loop runs its long tail (quartics, per-solution Newton steps, matrix element) with a third of the lanes
+    // (ncu: 10.4 of 32 threads per instruction in the NEXT-4 kernel before this loop).  Three stages, each on full warps:
+    //   A  every point up to the cheap tests; survivors are queued (queue 0)
+    //   B  32 queued points up to the resultant quartic(s): the number of real roots gives the point's class
+    //      (P::kClasses classes with a uniform trip count each); non-empty classes are queued (queues 1..kClasses)
+    //   C  32 points of one class: the full integrand
+    // A queue entry is the 32-bit offset of the point in the chunk; a later stage recomputes the point from its Philox
+    // counter (cheaper than carrying its state: 8 warps x 7 queues x 64 entries of ~100 B would not fit in shared
+    // memory).  One loop body serves all stages (the stage is warp-uniform), so the prelude exists once in the code.
+    // The order in which a lane meets its points depends only on the data: sums stay bitwise reproducible.
+    // Queue counters live in registers (kept in shared memory they cost 25 %).  Measured on B200: NEXT-4 7.7e9 ->
+    // 1.33e10 evaluations/s; config 4 (two classes, no stage A: its cheap test rejects only 15 %) 2.2e10.
+    constexpr int NQ = P::kClasses + 1;
+    uint32_t* q = reinterpret_cast<uint32_t*>(edges) + (threadIdx.x >> 5) * (NQ * 64);   // [NQ][64] ring buffers per warp
     const int lane = threadIdx.x & 31;
     const unsigned lt = (1u << lane) - 1u;
-    int cnt2 = 0, cnt4 = 0, head2 = 0, head4 = 0;                                   // warp-uniform
+    // entries waiting and ring heads of the NQ queues, one byte each, in two warp-uniform 64-bit registers
+    uint64_t cnts = 0, heads = 0;
+    auto get = [](uint64_t pack, int k) { return (int)((pack >> (8 * k)) & 0xffu); };
     int64_t base = lo;
     bool draining = base >= hi;
-    // One loop body serves both passes (the mode is warp-uniform): pass B whenever a queue holds a
-    // full batch, or anything at all once the chunk is exhausted; pass A otherwise.
     while (true) {
-      int which = -1;
-      if (cnt2 >= 32 || (draining && cnt2 > 0)) which = 0;
-      else if (cnt4 >= 32 || (draining && cnt4 > 0)) which = 1;
-      if (which < 0 && draining) break;
-      const bool pass_b = which >= 0;
+      // choose the stage: a full batch of the latest stage first (a class queue never holds more than 63 entries
+      // when 32 more may arrive); then, while the chunk lasts, a full batch of queue 0, else fresh points; once the
+      // chunk is exhausted, queue 0 until it is empty (it feeds the class queues), then whatever the class queues hold
+      int sel = -1;
+#pragma unroll
+      for (int k = 1; k < NQ; ++k) if (get(cnts, k) >= 32) sel = k;
+      if (sel < 0) {
+        if (!draining) {
+          if (get(cnts, 0) >= 32) sel = 0;
+        } else if (get(cnts, 0) > 0) {
+          sel = 0;
+        } else {
+#pragma unroll
+          for (int k = 1; k < NQ; ++k) if (get(cnts, k) > 0) sel = k;
+          if (sel < 0) break;
+        }
+      }
       int64_t i;
       bool active;
-      if (pass_b) {
-        const int n_live = min(32, which ? cnt4 : cnt2), hd = which ? head4 : head2;
+      if (sel >= 0) {
+        const int n_live = min(32, get(cnts, sel)), hd = get(heads, sel);
         active = lane < n_live;
-        i = lo + q[which * 64 + ((hd + lane) & 63)];
-        if (which) { head4 += n_live; cnt4 -= n_live; } else { head2 += n_live; cnt2 -= n_live; }
+        i = lo + q[sel * 64 + ((hd + lane) & 63)];
+        heads = (heads & ~(0xffull << (8 * sel))) | ((uint64_t)((hd + n_live) & 63) << (8 * sel));
+        cnts -= (uint64_t)n_live << (8 * sel);
       } else {
         i = base + threadIdx.x;
         active = i < hi;
         base += kThreads;
         draining = base >= hi;
       }
+      // a process whose cheap tests reject little (config 4: 15 % of the points) skips stage A: fresh points are classified
+      // directly and queue 0 stays empty
+      const bool classify = sel == 0 || (sel < 0 && !P::kCheapStage);
+      const int mode = sel > 0 ? P::kModeFull : (classify ? P::kModeClassify : P::kModeCheap);
       double r = 0.0;
       if (active) {
         double u[D];
         draw_uniforms<D>(rng, (uint64_t)i, ev_ctr, pass, u);
-        r = P::template weight_rt<GRIDPDF, true>(c, ec, u, !pass_b);              // pass A: number of real roots; pass B: the weight
+        r = P::template weight_rt<GRIDPDF, true>(c, ec, u, mode);
       }
       __syncwarp();                                        // the batch has been read before anything is queued
-      if (pass_b) {
+      if (sel > 0) {
         s1 += r; s2 = fma(r, r, s2);
+      } else if (classify) {
+        const int cls = (int)r;                            // 0 = no real root; 1..kClasses
+#pragma unroll
+        for (int k = 1; k < NQ; ++k) {
+          const unsigned m = __ballot_sync(0xffffffffu, cls == k);
+          if (cls == k) q[k * 64 + ((get(heads, k) + get(cnts, k) + __popc(m & lt)) & 63)] = (uint32_t)(i - lo);
+          cnts += (uint64_t)__popc(m) << (8 * k);
+        }
       } else {
-        const int nr = (int)r;
-        const unsigned m2 = __ballot_sync(0xffffffffu, nr > 0 && nr <= 2), m4 = __ballot_sync(0xffffffffu, nr > 2);
-        if (nr > 2) q[64 + ((head4 + cnt4 + __popc(m4 & lt)) & 63)] = (uint32_t)(i - lo);
-        else if (nr > 0) q[(head2 + cnt2 + __popc(m2 & lt)) & 63] = (uint32_t)(i - lo);
-        cnt2 += __popc(m2); cnt4 += __popc(m4);
+        const unsigned m = __ballot_sync(0xffffffffu, r != 0.0);
+        if (r != 0.0) q[(get(heads, 0) + get(cnts, 0) + __popc(m & lt)) & 63] = (uint32_t)(i - lo);
+        cnts += (uint64_t)__popc(m);
       }
       __syncwarp();
     }

@@ -59,6 +59,7 @@ __device__ inline void jet_assignment(int n_perm, int k, int (&sig)[4]) {
 struct ProcWenu {
   using real = double;
   static constexpr bool kCompact = false;   // lane compaction in the plain integrate kernel
+  static constexpr int kClasses = 0;
   static constexpr bool kHeavy = false;   // see min_blocks() in mem_kernels.cuh
   static constexpr bool kSplitC0 = false;
   static constexpr int D = 1, NF = 5, NC = 16;
@@ -176,6 +177,7 @@ __device__ __forceinline__ JetR<T> jet_mom(const T* o, T u) {
 struct ProcZbb {
   using real = double;
   static constexpr bool kCompact = false;   // lane compaction in the plain integrate kernel
+  static constexpr int kClasses = 0;
   static constexpr bool kHeavy = false;   // see min_blocks() in mem_kernels.cuh
   static constexpr bool kSplitC0 = false;
   static constexpr int D = 2, NF = 6, NC = 12;
@@ -239,6 +241,7 @@ template <typename T>
 struct ProcTTljetsR {
   using real = T;
   static constexpr bool kCompact = false;
+  static constexpr int kClasses = 0;
   static constexpr bool kHeavy = false;
   static constexpr int D = 6, NF = 17, NC = 44;
   static constexpr bool kSplitC0 = !std::is_same<T, double>::value;
@@ -491,6 +494,10 @@ struct ProcTTdilep {
   static constexpr bool kSplitC0 = false;
   static constexpr int D = 8, NF = 14, NC = 64;
   static constexpr int kNewton = 3;      // Newton steps on the un-squared equations per root
+  // stages of the lane-compacting loop (mem_kernels.cuh) and the classes its queues sort points into
+  static constexpr int kModeFull = 0, kModeClassify = 1, kModeCheap = 2;
+  static constexpr int kClasses = 2;     // 2 or 4 real roots of the resultant quartic
+  static constexpr bool kCheapStage = false;   // the b.nu > 0 test rejects only ~15 % of the points: classify directly
   // per top side s (0: l+, b; 1: l-, bbar), 14 constants each, at S0 + 14 s:
   //   LE LX LY LZ   lepton four-momentum
   //   I2EL          1 / (2 E_l)
@@ -566,17 +573,19 @@ struct ProcTTdilep {
   // PERM = true: NEXT-1, both assignments of the two b jets (ec = 2 blocks of NC constants)
   template <bool PERM, bool GRIDPDF, bool TAB_UNUSED>
   __device__ static double weight_t(const DevConst& c, const double* ec, const double (&u)[D]) {
-    if (!PERM) return weight_rt<GRIDPDF, true>(c, ec, u, false);
+    if (!PERM) return weight_rt<GRIDPDF, true>(c, ec, u, kModeFull);
     double w = 0.0;
 #pragma unroll 1
-    for (int k = 0; k < c.n_perm; ++k) w += weight_rt<GRIDPDF, false>(c, ec + k * NC, u, false);
+    for (int k = 0; k < c.n_perm; ++k) w += weight_rt<GRIDPDF, false>(c, ec + k * NC, u, kModeFull);
     return w;
   }
 
   __device__ static double weight(const DevConst& c, const double* ec, const double (&u)[D]) {
-    return weight_rt<false, true>(c, ec, u, false);
+    return weight_rt<false, true>(c, ec, u, kModeFull);
   }
 
+  // mode (a warp-uniform run-time flag: kModeCheap returns 1 after the cheap kinematic tests, kModeClassify the
+  // class of the point, 0 = no real root, 1 = two, 2 = four; see the staged loop in mem_kernels.cuh).  Formerly
   // count_only (a warp-uniform run-time flag, so that the prelude exists once in the kernel: the
   // config-4 kernel is instruction-cache bound, profiles/r01_ncu_config4.md): stop after the resultant
   // quartic and return its number of real roots (0, 2, 4) -- what the lane-compacting loop
@@ -584,13 +593,15 @@ struct ProcTTdilep {
   // TAB: table-driven exp (+5.8 % in the single-assignment kernel; the two-assignment kernel, tighter on
   // registers, loses 9 % with it and keeps libdevice's exp)
   template <bool GRIDPDF, bool TAB>
-  __device__ static double weight_rt(const DevConst& c, const double* ec, const double (&u)[D], bool count_only) {
+  __device__ static double weight_rt(const DevConst& c, const double* ec, const double (&u)[D], int mode) {
     // ---- S2: jets, transfer functions
     TfAcc<double> tfa{0.0, 1.0};
     const double xb0 = fma(c.dr, u[0], c.rlo), xb1 = fma(c.dr, u[1], c.rlo);
     const double ixb0 = rcp_fast(xb0), ixb1 = rcp_fast(xb1);
-    tf_accum<TAB>(c, ixb0, tfa);
-    tf_accum<TAB>(c, ixb1, tfa);
+    if (mode == kModeFull) {                       // the classification pass does not need them
+      tf_accum<TAB>(c, ixb0, tfa);
+      tf_accum<TAB>(c, ixb1, tfa);
+    }
     const double Eb0 = fma(ec[J0 + 1], u[0], ec[J0]), Eb1 = fma(ec[J1 + 1], u[1], ec[J1]);
     const double iEb0 = ixb0 * ec[IEJ0], iEb1 = ixb1 * ec[IEJ1];
     // ---- S2: the four mapped masses, s_k - m_k^2 = m Gam tan t_k (O6)
@@ -605,6 +616,7 @@ struct ProcTTdilep {
     const double hD0 = fma(0.5 * (dm2 + (smT0 - smW0)), iEb0, -ec[S0 + ELK]);
     const double hD1 = fma(0.5 * (dm2 + (smT1 - smW1)), iEb1, -ec[S1 + ELK]);
     if (!(hD0 > 0.0 && hD1 > 0.0)) return 0.0;
+    if (mode == kModeCheap) return 1.0;
     // ---- S2: total neutrino pT and the Gaussian MET transfer function (A8)
     const double g6 = fma(2.0, u[6], -1.0), g7 = fma(2.0, u[7], -1.0);
     const double Sx = fma(ec[MSPAN], g6, ec[METX]), Sy = fma(ec[MSPAN], g7, ec[METY]);
@@ -637,7 +649,7 @@ struct ProcTTdilep {
     double xr[4];
     const int nr = quartic_real_roots(R3 * ir4, R2 * ir4, R1 * ir4, R0 * ir4, xr);
     if (nr == 0) return 0.0;
-    if (count_only) return (double)nr;
+    if (mode == kModeClassify) return (double)(nr >> 1);
     // ---- solution-independent pieces
     const double ptx = ec[PTX] + Eb0 * ec[J0 + 2] + Eb1 * ec[J1 + 2] + Sx;     // total transverse momentum
     const double pty = ec[PTY] + Eb0 * ec[J0 + 3] + Eb1 * ec[J1 + 3] + Sy;

@@ -36,11 +36,17 @@ __device__ inline void tth_assignment(int n_perm, int k, int (&sig)[4]) {
 
 struct ProcTTHdilep {
   using real = double;
-  static constexpr bool kCompact = false;   // lane compaction in the plain integrate kernel
+  static constexpr bool kCompact = true;    // staged lane compaction in the plain integrate kernel
   static constexpr bool kHeavy = true;
   static constexpr bool kSplitC0 = false;
   static constexpr int D = 8, NF = 18, NC = 80;
   static constexpr int kNewton = 3;
+  // stages of the lane-compacting loop (mem_kernels.cuh).  Classes by the real roots (nr0, nr1) of the two orderings'
+  // quartics, so that a batch has one trip count: 1 = one ordering with 2 roots, 2 = one with 4, 3 = (2,2), 4 = (2,4),
+  // 5 = (4,2), 6 = (4,4)
+  static constexpr int kModeFull = 0, kModeClassify = 1, kModeCheap = 2;
+  static constexpr int kClasses = 6;
+  static constexpr bool kCheapStage = true;    // the cheap tests (b.nu > 0, Eq. 9 root inside the windows) reject most points
   // first 56 constants: the layout of ProcTTdilep (two top sides, conics, resultant, jets b and bbar)
   enum { LE, LX, LY, LZ, I2EL, ELK, IDZ, NLZ, AX, AY, LAX, LAY, MX, MY, SIDE = 14,
          S0 = 0, S1 = 14,
@@ -124,24 +130,22 @@ struct ProcTTHdilep {
 
   template <bool PERM, bool GRIDPDF, bool TAB_UNUSED>
   __device__ static double weight_t(const DevConst& c, const double* ec, const double (&u)[D]) {
-    if (!PERM) return weight_rt<GRIDPDF, true>(c, ec, u, -1);
+    if (!PERM) return weight_rt<GRIDPDF, true>(c, ec, u, kModeFull);
     double w = 0.0;
 #pragma unroll 1
-    for (int k = 0; k < c.n_perm; ++k) w += weight_rt<GRIDPDF, true>(c, ec + k * NC, u, -1);
+    for (int k = 0; k < c.n_perm; ++k) w += weight_rt<GRIDPDF, true>(c, ec + k * NC, u, kModeFull);
     return w;
   }
 
   __device__ static double weight(const DevConst& c, const double* ec, const double (&u)[D]) {
-    return weight_rt<false, true>(c, ec, u, -1);
+    return weight_rt<false, true>(c, ec, u, kModeFull);
   }
 
-  // which (a warp-uniform run-time selector, one copy of the code as in config 4):
-  //   -1  the weight (both Eq. 9 orderings)
-  //   -2  count only: stop after the two resultant quartics and return nr0 + 8 nr1, the numbers of real
-  //       roots (0, 2, 4) of ordering 0 and ordering 1 -- what the lane-compacting loop sorts work by
-  //   0/1 the contribution of ordering 0 / 1 alone (the compacting loop's second pass)
+  // mode (a warp-uniform run-time selector, one copy of the code as in config 4): kModeFull the weight (both Eq. 9
+  // orderings); kModeCheap 1 if the point passes the cheap tests (b.nu > 0 on both sides, Eq. 9 has a root and at
+  // least one ordering lies inside both energy windows); kModeClassify the point's class (0 = no real root).
   template <bool GRIDPDF, bool TAB>
-  __device__ static double weight_rt(const DevConst& c, const double* ec, const double (&u)[D], int which) {
+  __device__ static double weight_rt(const DevConst& c, const double* ec, const double (&u)[D], int mode) {
     // ---- S2: jets b, bbar
     const double xb0 = fma(c.dr, u[0], c.rlo), xb1 = fma(c.dr, u[1], c.rlo);
     const double ixb0 = rcp_fast(xb0), ixb1 = rcp_fast(xb1);
@@ -165,6 +169,11 @@ struct ProcTTHdilep {
     if (!(disc > 0.0)) return 0.0;
     const double rt = sqrt(disc);
     const double Ehi = 0.5 * (f + rt), Elo = 0.5 * (f - rt);
+    // an ordering counts only inside both parton-energy windows: the chart then covers exactly the box of O5
+    const bool in0 = Ehi >= ec[J2] && Ehi <= ec[J2 + 1] && Elo >= ec[J3] && Elo <= ec[J3 + 1];     // (E1, E2) = (Ehi, Elo)
+    const bool in1 = Elo >= ec[J2] && Elo <= ec[J2 + 1] && Ehi >= ec[J3] && Ehi <= ec[J3 + 1];     // (E1, E2) = (Elo, Ehi)
+    if (!(in0 || in1)) return 0.0;
+    if (mode == kModeCheap) return 1.0;
     // ---- S2: offsets of nu_z and E_nu on each side, conic linear/constant parts (independent of the ordering)
     const double w00 = sW0 * ec[S0 + I2EL], w01 = sW1 * ec[S1 + I2EL];
     const double al0 = (hD0 - w00) * ec[S0 + IDZ], al1 = (hD1 - w01) * ec[S1 + IDZ];
@@ -184,13 +193,12 @@ struct ProcTTHdilep {
     const double tvx = ec[S0 + LX] + Eb0 * ec[J0 + 2], tvy = ec[S0 + LY] + Eb0 * ec[J0 + 3];
     const double avx = ec[S1 + LX] + Eb1 * ec[J1 + 2], avy = ec[S1 + LY] + Eb1 * ec[J1 + 3];
     const double s_t = c.mt2 + smT0, s_tb = c.mt2 + smT1;
-    double total = 0.0, counts = 0.0;
+    double total = 0.0;
+    int nr0 = 0, nr1 = 0;
 #pragma unroll 1
     for (int r = 0; r < 2; ++r) {
-      if (which >= 0 && r != which) continue;
+      if (!(r ? in1 : in0)) continue;
       const double E1 = r ? Elo : Ehi, E2 = r ? Ehi : Elo;
-      // an ordering counts only inside both parton-energy windows: the chart then covers exactly the box of O5
-      if (!(E1 >= ec[J2] && E1 <= ec[J2 + 1] && E2 >= ec[J3] && E2 <= ec[J3 + 1])) continue;
       const double kx = fma(E1, ec[J2 + 2], E2 * ec[J3 + 2]), ky = fma(E1, ec[J2 + 3], E2 * ec[J3 + 3]);
       const double kz = fma(E1, ec[J2 + 4], E2 * ec[J3 + 4]);
       // Eq. 11: the neutrino pair balances the visible system of this point
@@ -211,7 +219,7 @@ struct ProcTTHdilep {
       const double R0 = fma(U0, U0, -V0 * W0);
       double xr[4];
       const int nr = quartic_real_roots(R3 * ir4, R2 * ir4, R1 * ir4, R0 * ir4, xr);
-      if (which == -2) { counts += r ? 8.0 * nr : (double)nr; continue; }
+      if (mode == kModeClassify) { if (r) nr1 = nr; else nr0 = nr; continue; }
       if (nr == 0) continue;
       double sum = 0.0;
 #pragma unroll 1
@@ -310,7 +318,10 @@ struct ProcTTHdilep {
         total = fma(th.fac * (TAB ? exp_tab<true>(-th.esum) : exp(-th.esum)), sum, total);
       }
     }
-    if (which == -2) return counts;
+    if (mode == kModeClassify) {
+      if (nr0 == 0 || nr1 == 0) return (double)((nr0 + nr1) >> 1);        // 0, 1 (two roots) or 2 (four)
+      return (double)(3 + (nr0 >> 2) * 2 + (nr1 >> 2));                     // (2,2) 3, (2,4) 4, (4,2) 5, (4,4) 6
+    }
     if (total == 0.0) return 0.0;
     // ---- S5: decays (p_t.p_l)(p_b.p_nu) per side; S6: transfer functions of b, bbar; S7
     TfAcc<double> tfa{0.0, 1.0};
