@@ -666,10 +666,9 @@ struct ProcTTdilep {
       const double V = fma(vv1, x, V0);
       if (!(V != 0.0)) continue;
       double y = -fma(fma(uu2, x, U1), x, U0) * rcp_fast(V);
-      // Newton on g1 = |nu| - E_nu(x, y), g2 = |nubar| - E_nubar(Sx - x, Sy - y)
       double nz, nbz, xb, yb;
-#pragma unroll
-      for (int it = 0; it < kNewton; ++it) {
+      // one Newton step on g1 = |nu| - E_nu(x, y), g2 = |nubar| - E_nubar(Sx - x, Sy - y); returns |dx| + |dy|
+      auto newton = [&]() {
         nz = fma(ec[S0 + AX], x, fma(ec[S0 + AY], y, al0));
         xb = Sx - x; yb = Sy - y;
         nbz = fma(ec[S1 + AX], xb, fma(ec[S1 + AY], yb, al1));
@@ -682,17 +681,33 @@ struct ProcTTdilep {
         const double j21 = -fma(fma(nbz, ec[S1 + AX], xb), iEnb, -ec[S1 + LAX]);
         const double j22 = -fma(fma(nbz, ec[S1 + AY], yb), iEnb, -ec[S1 + LAY]);
         const double idet = rcp_fast(fma(j11, j22, -j12 * j21));
-        x -= fma(g1, j22, -g2 * j12) * idet;
-        y -= fma(j11, g2, -j21 * g1) * idet;
+        const double dxn = fma(g1, j22, -g2 * j12) * idet, dyn = fma(j11, g2, -j21 * g1) * idet;
+        x -= dxn; y -= dyn;
+        return fabs(dxn) + fabs(dyn);
+      };
+#pragma unroll
+      for (int it = 0; it < kNewton; ++it) newton();
+      double EnL, EnbL, En, Enb;
+      bool good = false;
+#pragma unroll 1
+      for (int attempt = 0; attempt < 2; ++attempt) {
+        nz = fma(ec[S0 + AX], x, fma(ec[S0 + AY], y, al0));
+        xb = Sx - x; yb = Sy - y;
+        nbz = fma(ec[S1 + AX], xb, fma(ec[S1 + AY], yb, al1));
+        EnL = fma(ec[S0 + LAX], x, fma(ec[S0 + LAY], y, la0));
+        EnbL = fma(ec[S1 + LAX], xb, fma(ec[S1 + LAY], yb, la1));
+        En = sqrt(fma(x, x, fma(y, y, nz * nz))); Enb = sqrt(fma(xb, xb, fma(yb, yb, nbz * nbz)));
+        good = fabs(En - EnL) <= 1e-9 * (En + EnL) && fabs(Enb - EnbL) <= 1e-9 * (Enb + EnbL);
+        if (good || attempt == 1) break;
+        // rare: the Ferrari root was a poor start (the resultant's coefficients lose 6-8 digits to cancellation next
+        // to a tangency of the conics); polish until the point stops moving, as the oracle does
+#pragma unroll 1
+        for (int it = kNewton; it < 12; ++it) {
+          const double mv = newton();
+          if (!(mv > 0x1p-49 * (fabs(x) + fabs(y)))) break;
+        }
       }
-      nz = fma(ec[S0 + AX], x, fma(ec[S0 + AY], y, al0));
-      xb = Sx - x; yb = Sy - y;
-      nbz = fma(ec[S1 + AX], xb, fma(ec[S1 + AY], yb, al1));
-      const double EnL = fma(ec[S0 + LAX], x, fma(ec[S0 + LAY], y, la0));
-      const double EnbL = fma(ec[S1 + LAX], xb, fma(ec[S1 + LAY], yb, la1));
-      if (!(EnL > 0.0 && EnbL > 0.0)) continue;
-      const double En = sqrt(fma(x, x, fma(y, y, nz * nz))), Enb = sqrt(fma(xb, xb, fma(yb, yb, nbz * nbz)));
-      if (!(fabs(En - EnL) <= 1e-9 * (En + EnL) && fabs(Enb - EnbL) <= 1e-9 * (Enb + EnbL))) continue;
+      if (!(good && EnL > 0.0 && EnbL > 0.0)) continue;
       // Jacobian: E_nu (A x B)/(4 E_l E_b) = nu x d + E_nu (n_l x n_b), x and y components
       const double px = fma(y, ec[DZ0], fma(-nz, ec[DY0], En * ec[S0 + MX]));
       const double py = fma(nz, ec[DX0], fma(-x, ec[DZ0], En * ec[S0 + MY]));
