@@ -81,7 +81,7 @@ struct mem_handle {
   uint64_t event_offset;
   int64_t launches;
   int64_t grid_events;      // events covered by the grids of the last VEGAS call
-  Buffer ecs, partials, grids, hist, stage_in, stage_out, pdf_tab;
+  Buffer ecs, partials, grids, hist, stage_in, stage_out, pdf_tab, tickets;
   cudaEvent_t ev_begin, ev_end;  // around the dominant kernel of the last mem_integrate
   cudaEvent_t ev_done;           // recorded after the last launch of every call that uses the workspace
   bool has_done;                 // ev_done has been recorded at least once
@@ -294,7 +294,10 @@ bool aligned8(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 7u) == 0
 size_t integrate_smem(int NC, int D, int B, int mode) {   // NC = constants per event (all assignments)
   size_t n = (size_t)NC + 2 * kWarps;
   if (mode != MODE_PLAIN) n += (size_t)D * (B + 1);
-  if (mode == MODE_ADAPT) n += (size_t)kWarps * D * B;
+  if (mode == MODE_ADAPT) {
+    const size_t wh = (size_t)kWarps * D * B, scratch = (size_t)D * (3 * kMaxBins + 2);   // the refinement reuses the histograms' space
+    n += wh > scratch ? wh : scratch;
+  }
   return n * sizeof(double);
 }
 
@@ -313,7 +316,7 @@ mem_status launch_prepare(mem_handle* h, const double* events, int64_t n_events,
 
 template <class P, int MODE>
 mem_status launch_pass(mem_handle* h, int64_t n_events, int64_t n_points, int64_t chunk, int n_chunks,
-                       uint64_t seed, uint32_t pass, cudaStream_t st) {
+                       uint64_t seed, uint32_t pass, cudaStream_t st, double* out_p = nullptr, double* out_err = nullptr) {
   const int64_t blocks = n_events * n_chunks;
   if (blocks > 0x7fffffffLL) return fail(MEM_ERR_INVALID_ARG, "n_events * chunks = %lld exceeds the grid limit", (long long)blocks);
   // lane-compacting kernels keep (classes + 1) queues of 64 32-bit point offsets per warp, plus their counters
@@ -323,8 +326,9 @@ mem_status launch_pass(mem_handle* h, int64_t n_events, int64_t n_points, int64_
   }
   auto launch = [&](auto perm, auto grid) {
     integrate_kernel<P, MODE, decltype(perm)::value, decltype(grid)::value><<<(unsigned)blocks, kThreads, smem, st>>>(
-        dc_of<typename P::real>(h), (const double*)h->ecs.p, (const double*)h->grids.p, (double*)h->partials.p,
-        (double*)h->hist.p, n_points, chunk, n_chunks, make_philox(seed), h->event_offset, pass);
+        dc_of<typename P::real>(h), (const double*)h->ecs.p, (double*)h->grids.p, (double*)h->partials.p,
+        (double*)h->hist.p, n_points, chunk, n_chunks, make_philox(seed), h->event_offset, pass,
+        (unsigned*)h->tickets.p, out_p, out_err);
   };
   const bool perm = h->dc.n_perm > 1, grid = h->dc.pdf_tab != nullptr;
   if (perm && grid) launch(std::true_type{}, std::true_type{});
@@ -352,10 +356,10 @@ int64_t chunk_for(int64_t n_points) {
 // the pass that produces the outputs, bracketed by the handle's events
 template <class P, int MODE>
 mem_status launch_timed_pass(mem_handle* h, int64_t n_events, int64_t n_points, int n_chunks, uint64_t seed,
-                             uint32_t pass, cudaStream_t st, bool capturing) {
+                             uint32_t pass, cudaStream_t st, bool capturing, double* out_p, double* out_err) {
   // no event records inside a stream capture: they would belong to the graph and mem_last_pass_ms could not read them
   if (!capturing) CUDA_TRY(cudaEventRecord(h->ev_begin, st));
-  mem_status s = launch_pass<P, MODE>(h, n_events, n_points, chunk_for(n_points), n_chunks, seed, pass, st);
+  mem_status s = launch_pass<P, MODE>(h, n_events, n_points, chunk_for(n_points), n_chunks, seed, pass, st, out_p, out_err);
   if (s != MEM_OK) return s;
   if (!capturing) CUDA_TRY(cudaEventRecord(h->ev_end, st));
   h->last_evals = capturing ? 0 : n_events * n_points;
@@ -374,6 +378,12 @@ mem_status integrate_impl(mem_handle* h, const double* events, int64_t n_events,
   const int n_chunks = (int)((n_points + chunk - 1) / chunk);
   s = ensure(h, h->partials, (size_t)n_events * n_chunks * 2 * sizeof(double), st);
   if (s != MEM_OK) return s;
+  // arrival counters of the "last block of an event finishes it" step: zero when allocated, reset by the last block
+  if ((size_t)n_events * sizeof(unsigned) > h->tickets.cap) {
+    s = ensure(h, h->tickets, (size_t)n_events * sizeof(unsigned), st);
+    if (s != MEM_OK) return s;
+    CUDA_TRY(cudaMemsetAsync(h->tickets.p, 0, h->tickets.cap, st));
+  }
   const mem_params& p = h->params;
   if (p.vegas_iters > 0) {
     const int D = P::D, B = p.vegas_bins;
@@ -390,28 +400,17 @@ mem_status integrate_impl(mem_handle* h, const double* events, int64_t n_events,
       s = ensure(h, h->partials, (size_t)n_events * a_chunks * 2 * sizeof(double), st);
       if (s != MEM_OK) return s;
     }
-    const int64_t ng = n_events * D * (B + 1);
-    grid_init_kernel<<<(unsigned)((ng + 255) / 256), 256, 0, st>>>((double*)h->grids.p, n_events, D, B);
-    ++h->launches;
-    CUDA_TRY(cudaGetLastError());
+    // each adaptation pass refines the grids itself (last block per event); the first starts from the uniform grid
     for (int it = 0; it < p.vegas_iters; ++it) {
       s = launch_pass<P, MODE_ADAPT>(h, n_events, p.vegas_points, a_chunk, a_chunks, seed, (uint32_t)it, st);
       if (s != MEM_OK) return s;
-      refine_kernel<<<(unsigned)n_events, dim3(64, D), 0, st>>>(h->dc, (const double*)h->hist.p, a_chunks,
-                                                                (double*)h->grids.p, D);
-      ++h->launches;
-      CUDA_TRY(cudaGetLastError());
     }
     h->grid_events = n_events;
-    s = launch_timed_pass<P, MODE_GRID>(h, n_events, n_points, n_chunks, seed, (uint32_t)p.vegas_iters, st, capturing);
+    s = launch_timed_pass<P, MODE_GRID>(h, n_events, n_points, n_chunks, seed, (uint32_t)p.vegas_iters, st, capturing, out_p, out_err);
   } else {
-    s = launch_timed_pass<P, MODE_PLAIN>(h, n_events, n_points, n_chunks, seed, 0u, st, capturing);
+    s = launch_timed_pass<P, MODE_PLAIN>(h, n_events, n_points, n_chunks, seed, 0u, st, capturing, out_p, out_err);
   }
   if (s != MEM_OK) return s;
-  finalize_kernel<<<(unsigned)((n_events + 127) / 128), 128, 0, st>>>((const double*)h->partials.p, n_chunks,
-                                                                      n_events, n_points, out_p, out_err);
-  ++h->launches;
-  CUDA_TRY(cudaGetLastError());
   return end_call(h, st, capturing);
 }
 
@@ -507,7 +506,7 @@ mem_status mem_destroy(mem_handle* h) {
   const bool have_cur = cudaGetDevice(&cur) == cudaSuccess;
   if (have_cur && cur != h->device) cudaSetDevice(h->device);
   cudaDeviceSynchronize();
-  Buffer* bs[] = {&h->ecs, &h->partials, &h->grids, &h->hist, &h->stage_in, &h->stage_out, &h->pdf_tab};
+  Buffer* bs[] = {&h->ecs, &h->partials, &h->grids, &h->hist, &h->stage_in, &h->stage_out, &h->pdf_tab, &h->tickets};
   for (Buffer* b : bs)
     if (b->p) cudaFree(b->p);
   cudaEventDestroy(h->ev_begin);

@@ -1,9 +1,9 @@
 // mem_kernels.cuh -- the kernels of the hot path, templated on the process.
 //
 //   prepare_kernel    S0  one thread per event: record -> per-event constants
-//   integrate_kernel  S1-S8 (+S1v, histogram of S9): one block per (event, chunk of points)
-//   finalize_kernel   S8  per event: chunk partials -> (p, err), Eq. 5-6
-//   grid_init_kernel / refine_kernel  S9: per-event VEGAS grid (reading A14)
+//   integrate_kernel  S1-S8 (+S1v, S9): one block per (event, chunk of points); the last block of an event to
+//                     arrive turns the chunk partials into (p, err), Eq. 5-6, or refines the
+//                     event's VEGAS grid from the chunk histograms (reading A14)
 //   eval_points_kernel  diagnostic: one thread per point, writes w
 #pragma once
 #include "mem_processes.cuh"
@@ -85,6 +85,104 @@ __device__ __forceinline__ void warp_hist_add(double* wh, int k, double v) {
 // sums go registers -> warp shuffle -> shared -> partials[event][chunk] in a fixed order.
 // MODE_GRID/ADAPT: grids = [n_events][D][B+1].  MODE_ADAPT also writes the block's histogram
 // of w^2 to hist[event][chunk][D][B].
+// O1 (PAPER.md:76 Eq. 5, :80 Eq. 6, reading A1): p = sum w / N, err = sqrt(max(0, <w^2> - p^2)/(N-1)); the chunk
+// partials are added in chunk order by one thread
+__device__ __forceinline__ void finalize_event(const double* partials_e, int n_chunks, int64_t n_points,
+                                               double* out_p, double* out_err) {
+  double s1 = 0.0, s2 = 0.0;
+  for (int ch = 0; ch < n_chunks; ++ch) {
+    s1 += __ldcg(partials_e + 2 * ch);
+    s2 += __ldcg(partials_e + 2 * ch + 1);
+  }
+  const double N = (double)n_points;
+  const double m = s1 / N;
+  double var = s2 / N - m * m;
+  if (var < 0.0) var = 0.0;
+  *out_p = m;
+  *out_err = sqrt(var / (N - 1.0));
+}
+
+// S9 for one event, by the kThreads threads of one block: sum the chunk histograms in chunk order, smooth (1,6,1)/8,
+// normalise, compress r <- ((1-r)/ln(1/r))^alpha, then re-bin to the j/B quantiles of the piecewise-constant density r
+// on the old bins (reading A14).  old_x: the grid this pass sampled through, [D][B+1] in shared memory; new_x: the
+// event's grid in global memory, always written (the old edges when a dimension's histogram is empty).
+// sm: scratch of D * (3 * kMaxBins + 2) doubles.  Ends with a block barrier.
+template <int D>
+__device__ void refine_event(double vegas_alpha, int B, const double* hist_e, int n_chunks, const double* old_x,
+                             double* new_x, double* sm) {
+  double* h = sm;                      // [D][kMaxBins] smoothed
+  double* r = h + D * kMaxBins;        // [D][kMaxBins] raw, then compressed
+  double* nx = r + D * kMaxBins;       // [D][kMaxBins + 1]
+  double* tot = nx + D * (kMaxBins + 1);   // [D]
+  for (int idx = threadIdx.x; idx < D * B; idx += kThreads) {
+    const int d = idx / B, k = idx - d * B;
+    double a = 0.0;
+    for (int ch = 0; ch < n_chunks; ++ch) a += __ldcg(hist_e + ((size_t)ch * D + d) * B + k);
+    r[d * kMaxBins + k] = a;
+  }
+  __syncthreads();
+  for (int idx = threadIdx.x; idx < D * B; idx += kThreads) {
+    const int d = idx / B, k = idx - d * B;
+    const double* rd = r + d * kMaxBins;
+    double sv;
+    if (B == 1) sv = rd[0];
+    else if (k == 0) sv = (7.0 * rd[0] + rd[1]) / 8.0;
+    else if (k == B - 1) sv = (rd[B - 2] + 7.0 * rd[B - 1]) / 8.0;
+    else sv = (rd[k - 1] + 6.0 * rd[k] + rd[k + 1]) / 8.0;
+    h[d * kMaxBins + k] = sv;
+  }
+  __syncthreads();
+  if (threadIdx.x < D) {
+    double t = 0.0;
+    for (int j = 0; j < B; ++j) t += h[threadIdx.x * kMaxBins + j];
+    tot[threadIdx.x] = t;
+  }
+  __syncthreads();
+  for (int idx = threadIdx.x; idx < D * B; idx += kThreads) {
+    const int d = idx / B, k = idx - d * B;
+    const double t = tot[d];
+    if ((t > 0.0) && isfinite(t)) {
+      const double rk = h[d * kMaxBins + k] / t;
+      double v;
+      if (rk <= 0.0) v = 0.0;
+      else if (rk >= 1.0) v = 1.0;
+      else v = pow((1.0 - rk) / log(1.0 / rk), vegas_alpha);
+      r[d * kMaxBins + k] = v;
+    }
+  }
+  __syncthreads();
+  if (threadIdx.x < D) {
+    const int d = threadIdx.x;
+    const double t = tot[d];
+    const double* x = old_x + d * (B + 1);
+    const double* rd = r + d * kMaxBins;
+    double* nd = nx + d * (kMaxBins + 1);
+    if ((t > 0.0) && isfinite(t)) {
+      double rsum = 0.0;
+      for (int j = 0; j < B; ++j) rsum += rd[j];
+      const double per = rsum / (double)B;
+      double acc = 0.0;
+      int kk = 0;
+      nd[0] = x[0]; nd[B] = x[B];
+      for (int j = 1; j < B; ++j) {
+        const double target = (double)j * per;
+        while (kk < B - 1 && acc + rd[kk] < target) { acc += rd[kk]; ++kk; }
+        double frac = (rd[kk] > 0.0) ? (target - acc) / rd[kk] : 0.0;
+        frac = frac < 0.0 ? 0.0 : (frac > 1.0 ? 1.0 : frac);
+        nd[j] = x[kk] + frac * (x[kk + 1] - x[kk]);
+      }
+    } else {
+      for (int j = 0; j <= B; ++j) nd[j] = x[j];        // leave the grid
+    }
+  }
+  __syncthreads();
+  for (int idx = threadIdx.x; idx < D * (B + 1); idx += kThreads) {
+    const int d = idx / (B + 1), j = idx - d * (B + 1);
+    new_x[idx] = nx[d * (kMaxBins + 1) + j];
+  }
+  __syncthreads();
+}
+
 // Resident blocks per SM the register allocation aims at (measured on B200): 3 blocks of 256
 // threads = 80 registers for every integrate kernel.  The plain config-1/2/3 kernels fit without spills (uncapped
 // the config-3 kernel takes 100 registers, 2 blocks/SM, and is 1.6 % slower; 4 blocks at 64 registers change nothing);
@@ -96,9 +194,10 @@ constexpr int min_blocks() { return 3; }
 // then n_perm blocks of NC.  GRIDPDF: the flavour sum may use interpolated tables (NEXT-3).
 template <class P, int MODE, bool PERM, bool GRIDPDF>
 __global__ void __launch_bounds__(kThreads, min_blocks<P, MODE>())
-integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__ ecs, const double* __restrict__ grids,
-                 double* __restrict__ partials, double* __restrict__ hist, int64_t n_points,
-                 int64_t chunk, int n_chunks, const Philox rng, uint64_t event_offset, uint32_t pass) {
+integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__ ecs, double* grids,
+                 double* partials, double* hist, int64_t n_points,
+                 int64_t chunk, int n_chunks, const Philox rng, uint64_t event_offset, uint32_t pass,
+                 unsigned* __restrict__ tickets, double* __restrict__ out_p, double* __restrict__ out_err) {
   constexpr int D = P::D;
   using T = typename P::real;                         // fp64, or fp32 for the A15 variant
   extern __shared__ double smem[];
@@ -113,8 +212,13 @@ integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__
   const int ch = (int)(blockIdx.x - e * n_chunks);
   for (int k = threadIdx.x; k < NCP; k += kThreads) ec[k] = (T)ecs[e * NCP + k];
   const double c0 = P::kSplitC0 ? ecs[e * NCP + P::C0] : 1.0;     // fp32 core x fp64 per-event constant
-  if (MODE != MODE_PLAIN)
-    for (int k = threadIdx.x; k < D * (B + 1); k += kThreads) edges[k] = grids[e * D * (B + 1) + k];
+  if (MODE != MODE_PLAIN) {
+    // the first adaptation pass starts from the uniform grid x[d][j] = j / B without reading it from memory
+    if (MODE == MODE_ADAPT && pass == 0)
+      for (int k = threadIdx.x; k < D * (B + 1); k += kThreads) edges[k] = (double)(k % (B + 1)) / (double)B;
+    else
+      for (int k = threadIdx.x; k < D * (B + 1); k += kThreads) edges[k] = grids[e * D * (B + 1) + k];
+  }
   if (MODE == MODE_ADAPT)
     for (int k = threadIdx.x; k < kWarps * D * B; k += kThreads) whist[k] = 0.0;
   __syncthreads();
@@ -253,93 +357,27 @@ integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__
       hist[(size_t)blockIdx.x * D * B + k] = a;
     }
   }
-}
-
-// O1 (PAPER.md:76 Eq. 5, :80 Eq. 6, reading A1): p = sum w / N, err = sqrt(max(0, <w^2> - p^2)/(N-1))
-__global__ void finalize_kernel(const double* __restrict__ partials, int n_chunks, int64_t n_events,
-                                int64_t n_points, double* __restrict__ out_p, double* __restrict__ out_err) {
-  const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (e >= n_events) return;
-  double s1 = 0.0, s2 = 0.0;
-  for (int ch = 0; ch < n_chunks; ++ch) {
-    s1 += partials[2 * ((size_t)e * n_chunks + ch)];
-    s2 += partials[2 * ((size_t)e * n_chunks + ch) + 1];
-  }
-  const double N = (double)n_points;
-  const double m = s1 / N;
-  double var = s2 / N - m * m;
-  if (var < 0.0) var = 0.0;
-  out_p[e] = m;
-  out_err[e] = sqrt(var / (N - 1.0));
-}
-
-__global__ void grid_init_kernel(double* __restrict__ grids, int64_t n_events, int D, int B) {
-  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n_events * D * (B + 1)) return;
-  const int j = (int)(i % (B + 1));
-  grids[i] = (double)j / (double)B;
-}
-
-// S9, one block per event, blockDim = (64, D): thread (k, d).  Sum the chunk histograms in chunk
-// order, smooth (1,6,1)/8, normalise, compress r <- ((1-r)/ln(1/r))^alpha, then re-bin to the
-// j/B quantiles of the piecewise-constant density r on the old bins (reading A14).
-__global__ void refine_kernel(const DevConst c, const double* __restrict__ hist, int n_chunks,
-                              double* __restrict__ grids, int D) {
-  const int B = c.vegas_bins;
-  __shared__ double h[kMaxDims][kMaxBins], r[kMaxDims][kMaxBins], tot[kMaxDims], nx[kMaxDims][kMaxBins + 1];
-  const int k = threadIdx.x, d = threadIdx.y;
-  const int64_t e = blockIdx.x;
-  double* x = grids + (e * D + d) * (B + 1);
-  if (k < B) {
-    double a = 0.0;
-    for (int ch = 0; ch < n_chunks; ++ch) a += hist[(((size_t)e * n_chunks + ch) * D + d) * B + k];
-    r[d][k] = a;                                      // raw histogram
+  // The last block of an event to arrive finishes the event: Eq. 5-6 from the chunk partials (the pass that produces
+  // the outputs) or the grid refinement from the chunk histograms (an adaptation pass), both in chunk order, so the
+  // result does not depend on which block comes last.  One launch fewer per pass; no finalize / refine / grid-init kernels.
+  __shared__ int s_last;
+  __threadfence();                                         // this block's partials / histogram are visible device-wide
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    const unsigned t = atomicAdd(tickets + e, 1u);
+    s_last = (t == (unsigned)n_chunks - 1u);
+    if (s_last) tickets[e] = 0u;                           // ready for the next pass
   }
   __syncthreads();
-  if (k < B) {
-    double s;
-    if (B == 1) s = r[d][0];
-    else if (k == 0) s = (7.0 * r[d][0] + r[d][1]) / 8.0;
-    else if (k == B - 1) s = (r[d][B - 2] + 7.0 * r[d][B - 1]) / 8.0;
-    else s = (r[d][k - 1] + 6.0 * r[d][k] + r[d][k + 1]) / 8.0;
-    h[d][k] = s;
-  }
-  __syncthreads();
-  if (k == 0) {
-    double t = 0.0;
-    for (int j = 0; j < B; ++j) t += h[d][j];
-    tot[d] = t;
-  }
-  __syncthreads();
-  const double t = tot[d];
-  const bool ok = (t > 0.0) && isfinite(t);           // otherwise leave the grid
-  if (k < B && ok) {
-    const double rk = h[d][k] / t;
-    double v;
-    if (rk <= 0.0) v = 0.0;
-    else if (rk >= 1.0) v = 1.0;
-    else v = pow((1.0 - rk) / log(1.0 / rk), c.vegas_alpha);
-    r[d][k] = v;
-  }
-  __syncthreads();
-  if (k == 0 && ok) {
-    double rsum = 0.0;
-    for (int j = 0; j < B; ++j) rsum += r[d][j];
-    const double per = rsum / (double)B;
-    double acc = 0.0;
-    int kk = 0;
-    nx[d][0] = x[0]; nx[d][B] = x[B];
-    for (int j = 1; j < B; ++j) {
-      const double target = (double)j * per;
-      while (kk < B - 1 && acc + r[d][kk] < target) { acc += r[d][kk]; ++kk; }
-      double frac = (r[d][kk] > 0.0) ? (target - acc) / r[d][kk] : 0.0;
-      frac = frac < 0.0 ? 0.0 : (frac > 1.0 ? 1.0 : frac);
-      nx[d][j] = x[kk] + frac * (x[kk + 1] - x[kk]);
+  if (s_last) {
+    __threadfence();
+    if (MODE == MODE_ADAPT) {
+      refine_event<D>((double)c.vegas_alpha, B, hist + (size_t)e * n_chunks * D * B, n_chunks, edges,
+                      grids + e * D * (B + 1), whist);
+    } else if (threadIdx.x == 0) {
+      finalize_event(partials + 2 * (size_t)e * n_chunks, n_chunks, n_points, out_p + e, out_err + e);
     }
   }
-  __syncthreads();
-  if (ok)
-    for (int j = k; j <= B; j += blockDim.x) x[j] = nx[d][j];
 }
 
 // diagnostic: weights of points [first, first + n) of one event
