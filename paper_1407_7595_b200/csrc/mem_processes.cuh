@@ -423,7 +423,10 @@ using ProcTTljetsF = ProcTTljetsR<float>;   // reading A15
 // decay factors do not depend on the solution.
 // =========================================================================================
 
-// largest real root of z^3 + c2 z^2 + c1 z + c0: Cardano / trigonometric form, two Newton steps
+// largest real root of z^3 + c2 z^2 + c1 z + c0: Cardano / trigonometric form as a single-precision START (cube
+// root through cbrtf; cos(acos(c)/3) = T(s), s = sqrt((1 + c)/2), as a degree-6 polynomial: both ~1e-6), then three
+// Newton steps on the cubic in fp64, which converge to the root to rounding.  The closed forms in fp64 (libdevice
+// cbrt, acos) cost ~130 instructions with both branches of a diverged warp and 8 KB of code; this is ~50.
 __device__ __forceinline__ double cubic_largest_root(double c2, double c1, double c0) {
   const double sh = c2 * (1.0 / 3.0);
   const double P3 = fma(-c2, sh, c1) * (1.0 / 3.0);                  // P/3, P = c1 - c2^2/3
@@ -432,7 +435,11 @@ __device__ __forceinline__ double cubic_largest_root(double c2, double c1, doubl
   double w;
   if (disc > 0.0) {
     const double sq = sqrt(disc);
-    const double A = (Qh > 0.0) ? -cbrt(Qh + sq) : cbrt(sq - Qh);
+    const double a3 = (Qh > 0.0) ? -(Qh + sq) : (sq - Qh);           // A^3
+    const double aa = fabs(a3);
+    double A;
+    if (aa > 1e-30 && aa < 1e30) A = (double)cbrtf((float)a3);
+    else A = cbrt(a3);                                               // outside the comfortable float range: rare
     w = (A != 0.0) ? fma(-P3, rcp_fast(A), A) : 0.0;
   } else {
     const double m2 = -P3, m = sqrt(m2);
@@ -441,12 +448,21 @@ __device__ __forceinline__ double cubic_largest_root(double c2, double c1, doubl
     } else {
       double c = -Qh * rcp_fast(m2 * m);
       c = fmin(1.0, fmax(-1.0, c));
-      w = 2.0 * m * cos_third(acos(c) * (1.0 / 3.0));
+      // T(s) = cos((2/3) acos(s)) on [0, 1] (own Chebyshev fit, 4e-7)
+      const float sf = sqrtf(0.5f * (1.0f + (float)c));
+      float T = -0.002122052712365985f;
+      T = fmaf(T, sf, 0.010519994422793388f);
+      T = fmaf(T, sf, -0.026367755606770515f);
+      T = fmaf(T, sf, 0.05142129212617874f);
+      T = fmaf(T, sf, -0.11077950149774551f);
+      T = fmaf(T, sf, 0.5773273706436157f);
+      T = fmaf(T, sf, 0.5000004172325134f);
+      w = 2.0 * m * (double)T;
     }
   }
   double z = w - sh;
 #pragma unroll
-  for (int it = 0; it < 2; ++it) {
+  for (int it = 0; it < 3; ++it) {
     const double f = fma(fma(z + c2, z, c1), z, c0);
     const double fp = fma(fma(3.0, z, 2.0 * c2), z, c1);
     const double zn = fma(-f, rcp_fast(fp), z);
