@@ -188,7 +188,7 @@ __device__ void refine_event(double vegas_alpha, int B, const double* hist_e, in
 // the config-3 kernel takes 100 registers, 2 blocks/SM, and is 1.6 % slower; 4 blocks at 64 registers change nothing);
 // the divergent conic-solver kernels and the VEGAS passes (shuffle/match latency) gain 43 % / 7 % from 3 blocks.
 template <class P, int MODE>
-constexpr int min_blocks() { return P::kClasses > 2 ? 2 : 3; }
+constexpr int min_blocks() { return 3; }
 
 // PERM: sum over c.n_perm jet-parton assignments per point (NEXT-1); the per-event constants are
 // then n_perm blocks of NC.  GRIDPDF: the flavour sum may use interpolated tables (NEXT-3).

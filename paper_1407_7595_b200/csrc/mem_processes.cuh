@@ -610,14 +610,9 @@ struct ProcTTdilep {
   // registers, loses 9 % with it and keeps libdevice's exp)
   template <bool GRIDPDF, bool TAB>
   __device__ static double weight_rt(const DevConst& c, const double* ec, const double (&u)[D], int mode) {
-    // ---- S2: jets, transfer functions
-    TfAcc<double> tfa{0.0, 1.0};
+    // ---- S2: jets
     const double xb0 = fma(c.dr, u[0], c.rlo), xb1 = fma(c.dr, u[1], c.rlo);
     const double ixb0 = rcp_fast(xb0), ixb1 = rcp_fast(xb1);
-    if (mode == kModeFull) {                       // the classification pass does not need them
-      tf_accum<TAB>(c, ixb0, tfa);
-      tf_accum<TAB>(c, ixb1, tfa);
-    }
     const double Eb0 = fma(ec[J0 + 1], u[0], ec[J0]), Eb1 = fma(ec[J1 + 1], u[1], ec[J1]);
     const double iEb0 = ixb0 * ec[IEJ0], iEb1 = ixb1 * ec[IEJ1];
     // ---- S2: the four mapped masses, s_k - m_k^2 = m Gam tan t_k (O6)
@@ -636,6 +631,19 @@ struct ProcTTdilep {
     // ---- S2: total neutrino pT and the Gaussian MET transfer function (A8)
     const double g6 = fma(2.0, u[6], -1.0), g7 = fma(2.0, u[7], -1.0);
     const double Sx = fma(ec[MSPAN], g6, ec[METX]), Sy = fma(ec[MSPAN], g7, ec[METY]);
+    // ---- everything of the point that does not depend on the solution, folded into one factor now (the full pass
+    // only), so that it need not stay live -- or be spilled -- across the solution loop: S5 decays (p_t.p_l)(p_b.p_nu)
+    // per side, S6 jet transfer functions and the MET Gaussian (one shared exponential), 1/(E_b E_bbar) of the Jacobian
+    double pre = 0.0;
+    if (mode == kModeFull) {
+      TfAcc<double> tfa{0.0, 1.0};
+      tf_accum<TAB>(c, ixb0, tfa);
+      tf_accum<TAB>(c, ixb1, tfa);
+      const double targ = fma(ec[MEXP], fma(g6, g6, g7 * g7), -tfa.esum);
+      const double tf_tmet = tfa.fac * (TAB ? exp_tab<true>(targ) : exp(targ));
+      const double dec = fma(Eb0, ec[S0 + ELK], 0.5 * sW0) * (Eb0 * hD0) * fma(Eb1, ec[S1 + ELK], 0.5 * sW1) * (Eb1 * hD1);
+      pre = ec[C0] * tf_tmet * dec * (iEb0 * iEb1);
+    }
     // ---- S2: offsets of nu_z and E_nu on each side, conic linear/constant parts
     const double w00 = sW0 * ec[S0 + I2EL], w01 = sW1 * ec[S1 + I2EL];
     const double al0 = (hD0 - w00) * ec[S0 + IDZ], al1 = (hD1 - w01) * ec[S1 + IDZ];
@@ -667,13 +675,8 @@ struct ProcTTdilep {
     if (nr == 0) return 0.0;
     if (mode == kModeClassify) return (double)(nr >> 1);
     // ---- solution-independent pieces
-    const double ptx = ec[PTX] + Eb0 * ec[J0 + 2] + Eb1 * ec[J1 + 2] + Sx;     // total transverse momentum
-    const double pty = ec[PTY] + Eb0 * ec[J0 + 3] + Eb1 * ec[J1 + 3] + Sy;
-    const double visE = ec[S0 + LE] + ec[S1 + LE] + Eb0 + Eb1;
-    const double tvz = ec[S0 + LZ] + Eb0 * ec[J0 + 4], avz = ec[S1 + LZ] + Eb1 * ec[J1 + 4];   // visible p_z per top
-    const double tvE = ec[S0 + LE] + Eb0, avE = ec[S1 + LE] + Eb1;
-    const double tvx = ec[S0 + LX] + Eb0 * ec[J0 + 2], tvy = ec[S0 + LY] + Eb0 * ec[J0 + 3];
-    const double avx = ec[S1 + LX] + Eb1 * ec[J1 + 2], avy = ec[S1 + LY] + Eb1 * ec[J1 + 3];
+    // (the visible momenta of the two tops are rebuilt from E_b, E_bbar inside the solution loop: eight values fewer to
+    // keep live across it)
     double sum = 0.0;
     // one copy of the per-solution code (the roots stay in registers: selected, not indexed)
 #pragma unroll 1
@@ -731,11 +734,13 @@ struct ProcTTdilep {
       const double qy = fma(nbz, ec[DX1], fma(-xb, ec[DZ1], Enb * ec[S1 + MY]));
       const double xz = fabs(fma(px, qy, -py * qx));
       // ---- S3: transverse boost O7 of the two tops
-      const double tE = tvE + En, tz = tvz + nz, aE = avE + Enb, az = avz + nbz;
-      const double tx = tvx + x, ty = tvy + y, ax = avx + xb, ay = avy + yb;
-      const double PE = visE + En + Enb, Pz = tz + az;
+      const double tE = ec[S0 + LE] + Eb0 + En, tz = fma(Eb0, ec[J0 + 4], ec[S0 + LZ]) + nz;
+      const double aE = ec[S1 + LE] + Eb1 + Enb, az = fma(Eb1, ec[J1 + 4], ec[S1 + LZ]) + nbz;
+      const double tx = fma(Eb0, ec[J0 + 2], ec[S0 + LX]) + x, ty = fma(Eb0, ec[J0 + 3], ec[S0 + LY]) + y;
+      const double ax = fma(Eb1, ec[J1 + 2], ec[S1 + LX]) + xb, ay = fma(Eb1, ec[J1 + 3], ec[S1 + LY]) + yb;
+      const double PE = tE + aE, Pz = tz + az;
       const double iPE = rcp_fast(PE);
-      const double bx = ptx * iPE, by = pty * iPE;
+      const double bx = (tx + ax) * iPE, by = (ty + ay) * iPE;           // total transverse momentum / P_E
       const double omb = 1.0 - fma(bx, bx, by * by);
       if (!(omb > 0.0)) continue;
       const double gam = rsqrt(omb);
@@ -759,12 +764,7 @@ struct ProcTTdilep {
       const double ws = fma(lum.gg, Mgg, lum.qq * Mqq) * ish * rcp_fast(xz);  // flavour sum incl. the PDFs
       if (isfinite(ws)) sum += ws;
     }
-    // ---- S5: decays (p_t.p_l)(p_b.p_nu) per side; S6: MET TF; S7
-    const double dec = fma(Eb0, ec[S0 + ELK], 0.5 * sW0) * (Eb0 * hD0) * fma(Eb1, ec[S1 + ELK], 0.5 * sW1) * (Eb1 * hD1);
-    // jets' Gaussians and the MET Gaussian share one exponential
-    const double targ = fma(ec[MEXP], fma(g6, g6, g7 * g7), -tfa.esum);
-    const double tf_tmet = tfa.fac * (TAB ? exp_tab<true>(targ) : exp(targ));
-    const double w = ec[C0] * tf_tmet * dec * (iEb0 * iEb1) * sum;
+    const double w = pre * sum;
     return isfinite(w) ? w : 0.0;
   }
 };

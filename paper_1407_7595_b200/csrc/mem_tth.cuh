@@ -174,6 +174,19 @@ struct ProcTTHdilep {
     const bool in1 = Elo >= ec[J2] && Elo <= ec[J2 + 1] && Ehi >= ec[J3] && Ehi <= ec[J3 + 1];     // (E1, E2) = (Elo, Ehi)
     if (!(in0 || in1)) return 0.0;
     if (mode == kModeCheap) return 1.0;
+    // ---- everything of the point that does not depend on the ordering or the solution, folded into one factor now
+    // (the full pass only: its points have real roots), so that a dozen values need not stay live -- or be spilled --
+    // across the two loops: S5 decays (p_t.p_l)(p_b.p_nu) per side, S6 transfer functions of b and bbar, 1/(E_b E_bbar)
+    // of the Jacobian, Eq. 9's 1/|E1 - E2|, and k^2 of sum |M(H -> b bbar)|^2 (hypothesis 1: (1/k^4) k^2 (dk^2/du ~ k^2) = const)
+    double pre = 0.0;
+    if (mode == kModeFull) {
+      TfAcc<double> tfa{0.0, 1.0};
+      tf_accum<TAB>(c, ixb0, tfa);
+      tf_accum<TAB>(c, ixb1, tfa);
+      const double tf = tfa.fac * (TAB ? exp_tab<true>(-tfa.esum) : exp(-tfa.esum));
+      const double dec = fma(Eb0, ec[S0 + ELK], 0.5 * sW0) * (Eb0 * hD0) * fma(Eb1, ec[S1 + ELK], 0.5 * sW1) * (Eb1 * hD1);
+      pre = ec[C0] * tf * dec * (iEb0 * iEb1) * (c.tth_hyp ? 1.0 : sH) * rcp_fast(rt);
+    }
     // ---- S2: offsets of nu_z and E_nu on each side, conic linear/constant parts (independent of the ordering)
     const double w00 = sW0 * ec[S0 + I2EL], w01 = sW1 * ec[S1 + I2EL];
     const double al0 = (hD0 - w00) * ec[S0 + IDZ], al1 = (hD1 - w01) * ec[S1 + IDZ];
@@ -188,10 +201,8 @@ struct ProcTTHdilep {
     const double uu2 = ec[U2], vv1 = ec[V1], ir4 = ec[IR4];
     // visible momentum without the Higgs candidates
     const double vx0 = ec[PTX] + Eb0 * ec[J0 + 2] + Eb1 * ec[J1 + 2], vy0 = ec[PTY] + Eb0 * ec[J0 + 3] + Eb1 * ec[J1 + 3];
-    const double tvz = ec[S0 + LZ] + Eb0 * ec[J0 + 4], avz = ec[S1 + LZ] + Eb1 * ec[J1 + 4];
-    const double tvE = ec[S0 + LE] + Eb0, avE = ec[S1 + LE] + Eb1;
-    const double tvx = ec[S0 + LX] + Eb0 * ec[J0 + 2], tvy = ec[S0 + LY] + Eb0 * ec[J0 + 3];
-    const double avx = ec[S1 + LX] + Eb1 * ec[J1 + 2], avy = ec[S1 + LY] + Eb1 * ec[J1 + 3];
+    // (the visible momenta of the two tops are rebuilt from E_b, E_bbar inside the solution loop: eight values fewer to
+    // keep live across the loops)
     const double s_t = c.mt2 + smT0, s_tb = c.mt2 + smT1;
     double total = 0.0;
     int nr0 = 0, nr1 = 0;
@@ -221,6 +232,11 @@ struct ProcTTHdilep {
       const int nr = quartic_real_roots(R3 * ir4, R2 * ir4, R1 * ir4, R0 * ir4, xr);
       if (mode == kModeClassify) { if (r) nr1 = nr; else nr0 = nr; continue; }
       if (nr == 0) continue;
+      // S6: transfer functions of the two Higgs candidates for this ordering
+      TfAcc<double> th{0.0, 1.0};
+      tf_accum<TAB>(c, rcp_fast(E1 * ec[IEJ2]), th);
+      tf_accum<TAB>(c, rcp_fast(E2 * ec[IEJ3]), th);
+      const double tf12 = th.fac * (TAB ? exp_tab<true>(-th.esum) : exp(-th.esum));
       double sum = 0.0;
 #pragma unroll 1
       for (int k = 0; k < nr; ++k) {
@@ -277,8 +293,10 @@ struct ProcTTHdilep {
         const double qy = fma(nbz, ec[DX1], fma(-xb, ec[DZ1], Enb * ec[S1 + MY]));
         const double xz = fabs(fma(px, qy, -py * qx));
         // ---- S3: the two tops; P_T = 0 by Eq. 11, so x1, x2 come straight from P_E, P_z
-        const double tE = tvE + En, tz = tvz + nz, aE = avE + Enb, az = avz + nbz;
-        const double tx = tvx + x, ty = tvy + y, ax = avx + xb, ay = avy + yb;
+        const double tE = ec[S0 + LE] + Eb0 + En, tz = fma(Eb0, ec[J0 + 4], ec[S0 + LZ]) + nz;
+        const double aE = ec[S1 + LE] + Eb1 + Enb, az = fma(Eb1, ec[J1 + 4], ec[S1 + LZ]) + nbz;
+        const double tx = fma(Eb0, ec[J0 + 2], ec[S0 + LX]) + x, ty = fma(Eb0, ec[J0 + 3], ec[S0 + LY]) + y;
+        const double ax = fma(Eb1, ec[J1 + 2], ec[S1 + LX]) + xb, ay = fma(Eb1, ec[J1 + 3], ec[S1 + LY]) + yb;
         const double PE = (tE + aE) + f, Pz = (tz + az) + kz;
         const double x1 = (PE + Pz) * c.inv_sqrt_s, x2 = (PE - Pz) * c.inv_sqrt_s;
         if (!(x1 > 0.0 && x1 < 1.0 && x2 > 0.0 && x2 < 1.0)) continue;
@@ -310,28 +328,13 @@ struct ProcTTHdilep {
         const double ws = fma(lum.gg, Mgg, lum.qq * Mqq) * rad * rcp_fast(x1 * x2 * xz);
         if (isfinite(ws)) sum += ws;
       }
-      if (sum != 0.0) {
-        // ---- S6: transfer functions of the two Higgs candidates for this ordering
-        TfAcc<double> th{0.0, 1.0};
-        tf_accum<TAB>(c, rcp_fast(E1 * ec[IEJ2]), th);
-        tf_accum<TAB>(c, rcp_fast(E2 * ec[IEJ3]), th);
-        total = fma(th.fac * (TAB ? exp_tab<true>(-th.esum) : exp(-th.esum)), sum, total);
-      }
+      total = fma(tf12, sum, total);
     }
     if (mode == kModeClassify) {
       if (nr0 == 0 || nr1 == 0) return (double)((nr0 + nr1) >> 1);        // 0, 1 (two roots) or 2 (four)
       return (double)(3 + (nr0 >> 2) * 2 + (nr1 >> 2));                     // (2,2) 3, (2,4) 4, (4,2) 5, (4,4) 6
     }
-    if (total == 0.0) return 0.0;
-    // ---- S5: decays (p_t.p_l)(p_b.p_nu) per side; S6: transfer functions of b, bbar; S7
-    TfAcc<double> tfa{0.0, 1.0};
-    tf_accum<TAB>(c, ixb0, tfa);
-    tf_accum<TAB>(c, ixb1, tfa);
-    const double tf = tfa.fac * (TAB ? exp_tab<true>(-tfa.esum) : exp(-tfa.esum));
-    const double dec = fma(Eb0, ec[S0 + ELK], 0.5 * sW0) * (Eb0 * hD0) * fma(Eb1, ec[S1 + ELK], 0.5 * sW1) * (Eb1 * hD1);
-    // hypothesis 0: sum |M(H -> b bbar)|^2 carries k^2; hypothesis 1: (1/k^4)(k^2)(dk^2/du ~ k^2) is constant
-    const double hfac = c.tth_hyp ? 1.0 : sH;
-    const double w = ec[C0] * tf * dec * (iEb0 * iEb1) * hfac * rcp_fast(rt) * total;
+    const double w = pre * total;
     return isfinite(w) ? w : 0.0;
   }
 };
