@@ -51,10 +51,10 @@ NOMINAL_FP64_FMA_PER_CLK_PER_SM = 64      # 4 SMSPs x 16 lanes; confirmed by the
 VEGAS_ITERS, VEGAS_POINTS = 5, 1 << 17    # BASELINE.json:configs[4]
 
 
-def executed_counts(cfg, perm=1, precision=64):
+def executed_counts(cfg, perm=1, precision=64, variant=""):
     """(record or None) from fp64_counts.json, with "match" = taken on the SASS that is built now"""
     from paper_1407_7595_b200 import counts
-    return counts.lookup(cfg, perm, precision)
+    return counts.lookup(cfg, perm, precision, variant=variant)
 
 
 def parse_args():
@@ -348,7 +348,7 @@ def run_b200(args):
     peak_meas = mem.mem_measure_fp64_peak(5)
     peak_rrr = mem.mem_measure_fp64_peak_rrr(5)
     perm = max(args.perm, 1)
-    ex = executed_counts(cfg, perm, 64) if args.pdf == "toy" else None
+    ex = executed_counts(cfg, perm, 64, "h1" if (cfg == 6 and args.hyp == 1) else "") if args.pdf == "toy" else None
     fl_ex = None if ex is None else 2.0 * ex.get("dfma", 0.0) + ex.get("dmul", 0.0) + ex.get("dadd", 0.0)
     pipe_inst = None if ex is None else ex.get("dfma", 0.0) + ex.get("dmul", 0.0) + ex.get("dadd", 0.0)
     fl_alg = ALGORITHMIC_FLOP.get((cfg, perm))

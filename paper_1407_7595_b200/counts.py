@@ -45,6 +45,7 @@ KERNELS = {
     "5,1,64": "integrate_kernelINS_12ProcTTljetsRIdEELi1ELb0ELb0E",
     "5,1,32": "integrate_kernelINS_12ProcTTljetsRIfEELi1ELb0ELb0E",
     "6,1,64": "integrate_kernelINS_12ProcTTHdilepELi0ELb0ELb0E",
+    "6,1,64,h1": "integrate_kernelINS_12ProcTTHdilepELi0ELb0ELb0E",      # same kernel, hypothesis 1 (run-time switch)
     "6,12,64": "integrate_kernelINS_12ProcTTHdilepELi0ELb1ELb0E",
 }
 METRICS = {"dfma": "op_dfma_pred_on", "dmul": "op_dmul_pred_on", "dadd": "op_dadd_pred_on",
@@ -95,9 +96,9 @@ def load():
         return json.load(f)
 
 
-def lookup(config: int, perm: int = 1, precision: int = 64, check_build: bool = True):
+def lookup(config: int, perm: int = 1, precision: int = 64, check_build: bool = True, variant: str = ""):
     """counts of one kernel + "match": whether they were taken on the SASS that is built now (None = unknown)"""
-    key = "%d,%d,%d" % (config, max(perm, 1), precision)
+    key = "%d,%d,%d" % (config, max(perm, 1), precision) + ("," + variant if variant else "")
     rec = load().get(key)
     if rec is None:
         return None
@@ -113,7 +114,7 @@ def update(csv_path: str, key: str, points: int, note: str = ""):
     rows = list(csv.reader(l for l in open(csv_path) if l.startswith('"')))
     hdr = rows[0]
     i_name, i_metric, i_val, i_id = hdr.index("Kernel Name"), hdr.index("Metric Name"), hdr.index("Metric Value"), hdr.index("ID")
-    cfg, perm, prec = (int(x) for x in key.split(","))
+    cfg, perm, prec = (int(x) for x in key.split(",")[:3])
     proc = {1: "ProcWenu", 2: "ProcZbb", 3: "ProcTTljetsR", 4: "ProcTTdilep", 5: "ProcTTljetsR", 6: "ProcTTHdilep"}[cfg]
     if proc == "ProcTTljetsR":
         proc += "<double>" if prec == 64 else "<float>"
@@ -155,6 +156,6 @@ if __name__ == "__main__":
         print(json.dumps(update(a.update, a.key, a.points, a.note)))
     if a.check:
         for k in sorted(load()):
-            c, p, pr = (int(x) for x in k.split(","))
-            print(k, lookup(c, p, pr))
+            f = k.split(",")
+            print(k, lookup(int(f[0]), int(f[1]), int(f[2]), variant=f[3] if len(f) > 3 else ""))
     sys.exit(0)

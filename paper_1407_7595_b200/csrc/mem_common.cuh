@@ -213,6 +213,22 @@ __device__ __forceinline__ double cos_third(double x) {
   return fma(-2.0 * sn, sn, 1.0);
 }
 
+// sin(x) and cos(x) for 0 <= x < pi (config 1's Breit-Wigner complement angle and its window fraction): the
+// polynomials of tan_bw_n at x/4 <= pi/4, then two angle doublings.  No range reduction, no large-argument path.
+// cos(x/2) = 1 - 2 sin^2(x/4) cancels only next to x = pi, which the callers' windows exclude by >= 0.026
+// (the transverse-mass edge cannot lie more than 38 widths below the W pole): relative error <= 1e-14 there, ~2 ulp elsewhere.
+__device__ __forceinline__ void sincos_0pi(double x, double* sn, double* cs) {
+  const double r = 0.25 * x, z = r * r;
+  double ps = kTanS[5], pc = kTanC[5];
+#pragma unroll
+  for (int i = 4; i >= 0; --i) { ps = fma(ps, z, kTanS[i]); pc = fma(pc, z, kTanC[i]); }
+  const double s1 = fma(r * z, ps, r);                                // sin(x/4)
+  const double c1 = fma(z * z, pc, fma(-0.5, z, 1.0));                // cos(x/4)
+  const double s2 = 2.0 * s1 * c1, c2 = fma(-2.0 * s1, s1, 1.0);      // x/2
+  *sn = 2.0 * s2 * c2;
+  *cs = fma(-2.0 * s2, s2, 1.0);
+}
+
 __device__ __forceinline__ double tan_bw(double t) {
   const double a[1] = {t};
   double o[1];
@@ -316,7 +332,7 @@ __device__ __forceinline__ double exp_tab(double x) {
 // toy PDF shape product f(x1) f(x2) / A^2 = (x1 x2)^pow_x ((1-x1)(1-x2))^pow_1mx (O4)
 __device__ __forceinline__ double pdf_pair(const DevConst& c, double x1, double x2) {
   const double xx = x1 * x2, yy = (1.0 - x1) * (1.0 - x2);
-  if (c.pdf_fast) return rsqrt(xx) * (yy * yy * yy);
+  if (c.pdf_fast) return rsqrt_fast(xx) * (yy * yy * yy);
   return pow(xx, c.pdf_pow_x) * pow(yy, c.pdf_pow_1mx);
 }
 

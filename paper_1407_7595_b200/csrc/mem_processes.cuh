@@ -63,7 +63,7 @@ struct ProcWenu {
   static constexpr bool kHeavy = false;   // see min_blocks() in mem_kernels.cuh
   static constexpr bool kSplitC0 = false;
   static constexpr int D = 1, NF = 5, NC = 16;
-  enum { LM, LP, LE, LZ, PT, NT2, A, CLO, CHI, DT, SCLO, DSM, PTNT, IPT2, C0, _N };
+  enum { LM, LP, LE, LZ, PT, NT2, A, CLO, CHI, DT, ISCLO, DSM, PTNT, IPT2, C0, _N };
 
   __device__ static void prepare(const DevConst& c, const double* ev, int64_t n, int64_t e, int k, double* ec) {
     const double pT = ev[0 * n + e], eta = ev[1 * n + e], phi = ev[2 * n + e];
@@ -86,7 +86,7 @@ struct ProcWenu {
     ec[LM] = pT * exp(-eta);            // E_l - l_z
     ec[LP] = pT * exp(eta);             // E_l + l_z
     ec[LE] = lE; ec[LZ] = lz; ec[PT] = pT; ec[NT2] = nT2; ec[A] = a;
-    ec[CLO] = c_lo; ec[CHI] = c_hi; ec[DT] = dt; ec[SCLO] = sin(c_lo);   // sin(c_lo) = cos(t_lo)
+    ec[CLO] = c_lo; ec[CHI] = c_hi; ec[DT] = dt; ec[ISCLO] = 1.0 / sin(c_lo);   // sin(c_lo) = cos(t_lo)
     // s_min - s* without cancellation: E_l E_nu - l_z nu_z = pT nT cosh(eta - y_nu), so at the
     // boundary nu_z = +-P (y_P = +-asinh(P / nT)):  s(+-P) - s* = 4 pT nT sinh^2((eta - y_P) / 2)
     {
@@ -108,17 +108,20 @@ struct ProcWenu {
     // pi/2 - t = c_lo (1 - u) + c_hi u: positive terms only (1 - u is exact)
     const double cc_t = fma(ec[CLO], 1.0 - u[0], ec[CHI] * u[0]);
     double sc, cs;
-    sincos(cc_t, &sc, &cs);
-    const double smm = c.mWGW * (cs / sc);            // m Gam tan t = m Gam cot(pi/2 - t)
+    sincos_0pi(cc_t, &sc, &cs);
+    const double isc = rcp_fast(sc);                  // sc = sin(pi/2 - t) = cos t > 0 inside the window
+    const double smm = c.mWGW * (cs * isc);           // m Gam tan t = m Gam cot(pi/2 - t)
     const double sW = c.mW2 + smm;
     // s_W - s_min = m Gam (tan t - tan t_lo) = m Gam sin(dt u) / (cos t cos t_lo): no cancellation
     // at the transverse-mass edge
-    const double ds = c.mWGW * sin(ec[DT] * u[0]) / (sc * ec[SCLO]);
+    double sdt, cdt;
+    sincos_0pi(ec[DT] * u[0], &sdt, &cdt);
+    const double ds = c.mWGW * sdt * (isc * ec[ISCLO]);
     const double half = 0.5 * (ds + ec[DSM]);
     const double cc = 0.5 * sW + ec[A];
     const double disc = half * (cc + ec[PTNT]);
     if (!(disc > 0.0)) return 0.0;
-    const double rt = sqrt(disc);
+    const double irt = rsqrt_fast(disc), rt = disc * irt;
     double sum = 0.0;
 #pragma unroll
     for (int sgn = -1; sgn <= 1; sgn += 2) {
@@ -130,9 +133,16 @@ struct ProcWenu {
       if (!(x1 > 0.0 && x1 < 1.0 && x2 > 0.0 && x2 < 1.0)) continue;
       // both beam orderings: u^2 + t^2 = S (x1^2 (E_l - l_z)^2 + x2^2 (E_l + l_z)^2)
       const double a1 = x1 * ec[LM], a2 = x2 * ec[LP];
-      sum += pdf_pair(c, x1, x2) / (x1 * x2) * (a1 * a1 + a2 * a2);
+      const double me = fma(a1, a1, a2 * a2);
+      if (c.pdf_fast) {
+        // f f / (x1 x2) = (x1 x2)^(-3/2) ((1 - x1)(1 - x2))^3 = (r yy)^3 with r = (x1 x2)^(-1/2): no division
+        const double r = rsqrt_fast(x1 * x2), ry = r * ((1.0 - x1) * (1.0 - x2));
+        sum = fma(ry * ry * ry, me, sum);
+      } else {
+        sum += pdf_pair(c, x1, x2) / (x1 * x2) * me;
+      }
     }
-    const double w = ec[C0] * sum / rt;
+    const double w = ec[C0] * sum * irt;
     return isfinite(w) ? w : 0.0;
   }
 };
@@ -214,11 +224,11 @@ struct ProcZbb {
     //   s-hat  = 2 E1 E2 (1 - n1.n2) = (P_E' + P_z)(P_E' - P_z)
     const double e12 = p1.E * p2.E, ekt = e12 * ec[KT];
     const double Pz = p1.z + p2.z;
-    const double PEb = sqrt(fma(p1.z, p1.z, fma(p2.z, p2.z, 2.0 * ekt)));
-    const double iPEb = rcp_fast(PEb);
+    const double PEb2 = fma(p1.z, p1.z, fma(p2.z, p2.z, 2.0 * ekt));
+    const double iPEb = rsqrt_fast(PEb2), PEb = PEb2 * iPEb;
     const double E1 = fma(p1.z, p1.z, ekt) * iPEb, E2 = fma(p2.z, p2.z, ekt) * iPEb;
     const double shat = 2.0 * e12 * ec[J0 + 3];
-    const double Xb = PEb + fabs(Pz), Xs = shat / Xb;
+    const double Xb = PEb + fabs(Pz), Xs = shat * rcp_fast(Xb);
     const double x1 = (Pz >= 0.0 ? Xb : Xs) * c.inv_sqrt_s, x2 = (Pz >= 0.0 ? Xs : Xb) * c.inv_sqrt_s;
     if (!(x1 > 0.0 && x1 < 1.0 && x2 > 0.0 && x2 < 1.0)) return 0.0;
     // u = -2 qa.p2', t = -2 qa.p1' for qa = q1 and qa = q2 (both beam orderings), in units of -2h
@@ -226,7 +236,7 @@ struct ProcZbb {
     const double u2 = x2 * (E2 + p2.z), t2 = x2 * (E1 + p1.z);
     const double me = c.z_cu * (u1 * u1 + u2 * u2) + c.z_ct * (t1 * t1 + t2 * t2);
     const double dz = shat - c.mZ2;
-    const double w = ec[C0] * tf * pdf_pair(c, x1, x2) * me / (shat * (dz * dz + c.mZGZ2));
+    const double w = ec[C0] * tf * pdf_pair(c, x1, x2) * me * rcp_fast(shat * fma(dz, dz, c.mZGZ2));
     return isfinite(w) ? w : 0.0;
   }
 };
