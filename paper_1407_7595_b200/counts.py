@@ -136,6 +136,9 @@ def update(csv_path: str, key: str, points: int, note: str = ""):
     if note:
         rec["note"] = note
     data = load()
+    for keep in ("dram_bytes", "dram_bytes_source"):          # full-size traffic figures survive a count refresh
+        if keep in data.get(key, {}):
+            rec[keep] = data[key][keep]
     data[key] = rec
     with open(PATH, "w") as f:
         json.dump(data, f, indent=1, sort_keys=True)
