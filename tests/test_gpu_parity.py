@@ -305,3 +305,25 @@ def test_cuda_graph_capture_and_replay(mem):
         g.replay()
         torch.cuda.synchronize()
         assert torch.equal(out_p, ref_p) and torch.equal(out_e, ref_e)
+
+
+@pytest.mark.parametrize("proc,over", [(3, {}), (2, {}), (4, {}), (5, {}), (3, dict(vegas_iters=2, vegas_points=4096))])
+def test_diagnostic_weights_are_the_summed_weights(mem, proc, over):
+    """mem_eval_points evaluates with the same code (same exp, same grid map) as the pass that produces the outputs:
+    the mean of the per-point weights it reports is the integral mem_integrate returns"""
+    import torch
+    ne, n_points = 3, 8192 + 77
+    ev = wl.make_tth_events(ne, seed=3) if proc == 5 else wl.make_events(proc, 64, seed=9)
+    if proc == 4:            # keep events that have live points
+        po, _ = oracle.integrate(proc, oracle.params_default(proc), ev, 1500, SEED)
+        ev = np.ascontiguousarray(ev[:, po > 0])
+    ev = np.ascontiguousarray(ev[:, :ne])
+    dev = _dev(ev)
+    with mem.Integrator(proc, **over) as it:
+        p, _ = it.integrate(dev, n_points, SEED)
+        grid = it.grid(ne) if over else None
+        for e in range(ne):
+            w = it.eval_points(dev, e, 0, n_points, SEED, iteration=over.get("vegas_iters", 0),
+                               grid=None if grid is None else grid[e].contiguous())
+            assert abs(w.sum().item() / n_points - p[e].item()) <= 1e-12 * abs(p[e].item())
+    assert float(p.max()) > 0
