@@ -322,7 +322,7 @@ mem_status launch_pass(mem_handle* h, int64_t n_events, int64_t n_points, int64_
   // lane-compacting kernels keep (classes + 1) queues of 64 32-bit point offsets per warp, plus their counters
   size_t smem = integrate_smem(P::NC * h->dc.n_perm, P::D, h->dc.vegas_bins, MODE);
   if constexpr (P::kCompact) {
-    if (MODE == MODE_PLAIN) smem += (size_t)kWarps * ((P::kClasses + 1) * 64 + 2 * (P::kClasses + 1) + 2) * sizeof(uint32_t);
+    if (MODE == MODE_PLAIN) smem += (size_t)kWarps * (P::kClasses + P::kPreStages) * 64 * sizeof(uint32_t);
   }
   auto launch = [&](auto perm, auto grid) {
     integrate_kernel<P, MODE, decltype(perm)::value, decltype(grid)::value><<<(unsigned)blocks, kThreads, smem, st>>>(
@@ -346,7 +346,14 @@ mem_status launch_pass(mem_handle* h, int64_t n_events, int64_t n_points, int64_
 // with it every bit of the result, is the same however the event list is sharded.
 // (Measured and dropped: persistent blocks walking the items round-robin -- 7 to 15 % slower on every config, the
 // hardware block scheduler balances better; 32 chunks for every size -- config 4 loses 1.7 %.)
-int64_t chunk_for(int64_t n_points) {
+// compact = the staged lane-compacting loop of the conic-solver processes: every queue ends a chunk with a partial
+// batch, so a warp should see many points (2^16 per block, at least 4 chunks per event).
+int64_t chunk_for(int64_t n_points, bool compact = false) {
+  if (compact) {
+    int64_t c = 4 * kChunk;
+    while (c > 1024 && c * 4 > n_points) c >>= 1;
+    return c;
+  }
   int64_t c = kChunk;
   const int64_t min_chunks = n_points < (1 << 18) ? 32 : 16;
   while (c > 1024 && c * min_chunks > n_points) c >>= 1;
@@ -359,7 +366,7 @@ mem_status launch_timed_pass(mem_handle* h, int64_t n_events, int64_t n_points, 
                              uint32_t pass, cudaStream_t st, bool capturing, double* out_p, double* out_err) {
   // no event records inside a stream capture: they would belong to the graph and mem_last_pass_ms could not read them
   if (!capturing) CUDA_TRY(cudaEventRecord(h->ev_begin, st));
-  mem_status s = launch_pass<P, MODE>(h, n_events, n_points, chunk_for(n_points), n_chunks, seed, pass, st, out_p, out_err);
+  mem_status s = launch_pass<P, MODE>(h, n_events, n_points, chunk_for(n_points, P::kCompact && MODE == MODE_PLAIN && h->dc.n_perm <= 1), n_chunks, seed, pass, st, out_p, out_err);
   if (s != MEM_OK) return s;
   if (!capturing) CUDA_TRY(cudaEventRecord(h->ev_end, st));
   h->last_evals = capturing ? 0 : n_events * n_points;
@@ -374,7 +381,7 @@ mem_status integrate_impl(mem_handle* h, const double* events, int64_t n_events,
   if (s != MEM_OK) return s;
   s = launch_prepare<P>(h, events, n_events, st);
   if (s != MEM_OK) return s;
-  const int64_t chunk = chunk_for(n_points);
+  const int64_t chunk = chunk_for(n_points, P::kCompact && h->params.vegas_iters == 0 && h->dc.n_perm <= 1);
   const int n_chunks = (int)((n_points + chunk - 1) / chunk);
   s = ensure(h, h->partials, (size_t)n_events * n_chunks * 2 * sizeof(double), st);
   if (s != MEM_OK) return s;

@@ -232,7 +232,8 @@ integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__
     // kinematic tests, or because the two conics do not intersect -- and the survivors are scattered over the warp, so
     // a plain loop runs its long tail (quartics, per-solution Newton steps, matrix element) with a third of the lanes
     // (ncu: 10.4 of 32 threads per instruction in the NEXT-4 kernel before this loop).  Three stages, each on full warps:
-    //   A  every point up to the cheap tests; survivors are queued (queue 0)
+    //   A  (P::kPreStages = 0, 1 or 2 of them) every point through the process's cheap tests; the first needs one
+    //      Philox word block only, the second evaluates the prelude; survivors are queued
     //   B  32 queued points up to the resultant quartic(s): the number of real roots gives the point's class
     //      (P::kClasses classes with a uniform trip count each); non-empty classes are queued (queues 1..kClasses)
     //   C  32 points of one class: the full integrand
@@ -242,7 +243,9 @@ integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__
     // The order in which a lane meets its points depends only on the data: sums stay bitwise reproducible.
     // Queue counters live in registers (kept in shared memory they cost 25 %).  Measured on B200: NEXT-4 7.7e9 ->
     // 1.33e10 evaluations/s; config 4 (two classes, no stage A: its cheap test rejects only 15 %) 2.2e10.
-    constexpr int NQ = P::kClasses + 1;
+    constexpr int NP = P::kPreStages;                  // cheap-test stages before the classification (0, 1 or 2)
+    constexpr int NQ = P::kClasses + NP;               // queues 0..NP-1: survivors of the cheap tests; NP..NQ-1: classes
+    static_assert(NQ <= 8, "queue counters are packed one byte each into 64 bits");
     uint32_t* q = reinterpret_cast<uint32_t*>(edges) + (threadIdx.x >> 5) * (NQ * 64);   // [NQ][64] ring buffers per warp
     const int lane = threadIdx.x & 31;
     const unsigned lt = (1u << lane) - 1u;
@@ -252,22 +255,18 @@ integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__
     int64_t base = lo;
     bool draining = base >= hi;
     while (true) {
-      // choose the stage: a full batch of the latest stage first (a class queue never holds more than 63 entries
-      // when 32 more may arrive); then, while the chunk lasts, a full batch of queue 0, else fresh points; once the
-      // chunk is exhausted, queue 0 until it is empty (it feeds the class queues), then whatever the class queues hold
+      // choose what to run: a full batch of the latest stage first (so a queue never holds more than 63 entries when
+      // 32 more may arrive); while the chunk lasts, fresh points otherwise; once it is exhausted, the earliest
+      // non-empty cheap-test queue (it feeds the later ones), then whatever the class queues hold
       int sel = -1;
 #pragma unroll
-      for (int k = 1; k < NQ; ++k) if (get(cnts, k) >= 32) sel = k;
-      if (sel < 0) {
-        if (!draining) {
-          if (get(cnts, 0) >= 32) sel = 0;
-        } else if (get(cnts, 0) > 0) {
-          sel = 0;
-        } else {
+      for (int k = 0; k < NQ; ++k) if (get(cnts, k) >= 32) sel = k;
+      if (sel < 0 && draining) {
 #pragma unroll
-          for (int k = 1; k < NQ; ++k) if (get(cnts, k) > 0) sel = k;
-          if (sel < 0) break;
-        }
+        for (int k = NQ - 1; k >= NP; --k) if (get(cnts, k) > 0) sel = k;
+#pragma unroll
+        for (int k = NP - 1; k >= 0; --k) if (get(cnts, k) > 0) sel = k;
+        if (sel < 0) break;
       }
       int64_t i;
       bool active;
@@ -283,31 +282,41 @@ integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__
         base += kThreads;
         draining = base >= hi;
       }
-      // a process whose cheap tests reject little (config 4: 15 % of the points) skips stage A: fresh points are classified
-      // directly and queue 0 stays empty
-      const bool classify = sel == 0 || (sel < 0 && !P::kCheapStage);
-      const int mode = sel > 0 ? P::kModeFull : (classify ? P::kModeClassify : P::kModeCheap);
+      // the stage these points are in: 0..NP-1 a cheap test, NP the classification, NP+1 the full integrand
+      const int stage = sel < 0 ? 0 : (sel < NP ? sel + 1 : NP + 1);
       double r = 0.0;
       if (active) {
-        double u[D];
-        draw_uniforms<D>(rng, (uint64_t)i, ev_ctr, pass, u);
-        r = P::template weight_rt<GRIDPDF, true>(c, ec, u, mode);
+        if (NP > 0 && stage == 0 && P::kCheapBlock >= 0) {
+          // the first cheap test needs the two dimensions of one Philox word block only (NEXT-4: Eq. 9's k^2 and f)
+          uint32_t w4[4];
+          rng((uint32_t)i, (uint32_t)((uint64_t)i >> 32), ev_ctr, pass * 256u + (uint32_t)P::kCheapBlock, w4);
+          r = P::cheap_test(c, ec, u52(w4[0], w4[1]), u52(w4[2], w4[3]));
+        } else {
+          double u[D];
+          draw_uniforms<D>(rng, (uint64_t)i, ev_ctr, pass, u);
+          r = P::template weight_rt<GRIDPDF, true>(c, ec, u, stage > NP ? P::kModeFull : (stage == NP ? P::kModeClassify : P::kModeCheap));
+        }
       }
       __syncwarp();                                        // the batch has been read before anything is queued
-      if (sel > 0) {
+      if (stage > NP) {
         s1 += r; s2 = fma(r, r, s2);
-      } else if (classify) {
+      } else if (stage == NP) {
         const int cls = (int)r;                            // 0 = no real root; 1..kClasses
 #pragma unroll
-        for (int k = 1; k < NQ; ++k) {
-          const unsigned m = __ballot_sync(0xffffffffu, cls == k);
-          if (cls == k) q[k * 64 + ((get(heads, k) + get(cnts, k) + __popc(m & lt)) & 63)] = (uint32_t)(i - lo);
+        for (int k = NP; k < NQ; ++k) {
+          const unsigned m = __ballot_sync(0xffffffffu, cls == k - NP + 1);
+          if (cls == k - NP + 1) q[k * 64 + ((get(heads, k) + get(cnts, k) + __popc(m & lt)) & 63)] = (uint32_t)(i - lo);
           cnts += (uint64_t)__popc(m) << (8 * k);
         }
       } else {
+        // survivors of cheap test `stage` go to queue `stage`
         const unsigned m = __ballot_sync(0xffffffffu, r != 0.0);
-        if (r != 0.0) q[(get(heads, 0) + get(cnts, 0) + __popc(m & lt)) & 63] = (uint32_t)(i - lo);
-        cnts += (uint64_t)__popc(m);
+#pragma unroll
+        for (int k = 0; k < NP; ++k)
+          if (k == stage) {
+            if (r != 0.0) q[k * 64 + ((get(heads, k) + get(cnts, k) + __popc(m & lt)) & 63)] = (uint32_t)(i - lo);
+            cnts += (uint64_t)__popc(m) << (8 * k);
+          }
       }
       __syncwarp();
     }

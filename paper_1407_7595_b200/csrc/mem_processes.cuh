@@ -59,7 +59,7 @@ __device__ inline void jet_assignment(int n_perm, int k, int (&sig)[4]) {
 struct ProcWenu {
   using real = double;
   static constexpr bool kCompact = false;   // lane compaction in the plain integrate kernel
-  static constexpr int kClasses = 0;
+  static constexpr int kClasses = 0, kPreStages = 0;
   static constexpr bool kHeavy = false;   // see min_blocks() in mem_kernels.cuh
   static constexpr bool kSplitC0 = false;
   static constexpr int D = 1, NF = 5, NC = 16;
@@ -187,7 +187,7 @@ __device__ __forceinline__ JetR<T> jet_mom(const T* o, T u) {
 struct ProcZbb {
   using real = double;
   static constexpr bool kCompact = false;   // lane compaction in the plain integrate kernel
-  static constexpr int kClasses = 0;
+  static constexpr int kClasses = 0, kPreStages = 0;
   static constexpr bool kHeavy = false;   // see min_blocks() in mem_kernels.cuh
   static constexpr bool kSplitC0 = false;
   static constexpr int D = 2, NF = 6, NC = 12;
@@ -251,7 +251,7 @@ template <typename T>
 struct ProcTTljetsR {
   using real = T;
   static constexpr bool kCompact = false;
-  static constexpr int kClasses = 0;
+  static constexpr int kClasses = 0, kPreStages = 0;
   static constexpr bool kHeavy = false;
   static constexpr int D = 6, NF = 17, NC = 44;
   static constexpr bool kSplitC0 = !std::is_same<T, double>::value;
@@ -523,7 +523,9 @@ struct ProcTTdilep {
   // stages of the lane-compacting loop (mem_kernels.cuh) and the classes its queues sort points into
   static constexpr int kModeFull = 0, kModeClassify = 1, kModeCheap = 2;
   static constexpr int kClasses = 2;     // 2 or 4 real roots of the resultant quartic
-  static constexpr bool kCheapStage = false;   // the b.nu > 0 test rejects only ~15 % of the points: classify directly
+  static constexpr int kPreStages = 0;         // the b.nu > 0 test rejects only ~15 % of the points: classify directly
+  static constexpr int kCheapBlock = 0;
+  __device__ static double cheap_test(const DevConst&, const double*, double, double) { return 1.0; }
   // per top side s (0: l+, b; 1: l-, bbar), 14 constants each, at S0 + 14 s:
   //   LE LX LY LZ   lepton four-momentum
   //   I2EL          1 / (2 E_l)
@@ -714,7 +716,7 @@ struct ProcTTdilep {
         x -= dxn; y -= dyn;
         return fabs(dxn) + fabs(dyn);
       };
-#pragma unroll
+#pragma unroll 1
       for (int it = 0; it < kNewton; ++it) newton();
       double EnL, EnbL, En, Enb;
       bool good = false;
