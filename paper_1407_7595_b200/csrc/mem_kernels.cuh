@@ -143,8 +143,7 @@ __device__ void refine_event(double vegas_alpha, int B, const double* hist_e, in
                              double* new_x, double* sm) {
   double* h = sm;                      // [D][kMaxBins] smoothed
   double* r = h + D * kMaxBins;        // [D][kMaxBins] raw, then compressed
-  double* nx = r + D * kMaxBins;       // [D][kMaxBins + 1]
-  double* tot = nx + D * (kMaxBins + 1);   // [D]
+  double* tot = r + D * kMaxBins;      // [D]
   for (int idx = threadIdx.x; idx < D * B; idx += kThreads) {
     const int d = idx / B, k = idx - d * B;
     double a = 0.0;
@@ -182,34 +181,41 @@ __device__ void refine_event(double vegas_alpha, int B, const double* hist_e, in
     }
   }
   __syncthreads();
+  // running totals of the compressed density in bin order, cum[k] = r[0] + ... + r[k]: what the sequential re-binning
+  // loop (while acc + r[kk] < target: acc += r[kk], ++kk) holds in acc + r[kk] when it stands at bin kk
+  double* cum = h;                     // the smoothed histogram is no longer needed
   if (threadIdx.x < D) {
     const int d = threadIdx.x;
-    const double t = tot[d];
-    const double* x = old_x + d * (B + 1);
-    const double* rd = r + d * kMaxBins;
-    double* nd = nx + d * (kMaxBins + 1);
-    if ((t > 0.0) && isfinite(t)) {
-      double rsum = 0.0;
-      for (int j = 0; j < B; ++j) rsum += rd[j];
-      const double per = rsum / (double)B;
-      double acc = 0.0;
-      int kk = 0;
-      nd[0] = x[0]; nd[B] = x[B];
-      for (int j = 1; j < B; ++j) {
-        const double target = (double)j * per;
-        while (kk < B - 1 && acc + rd[kk] < target) { acc += rd[kk]; ++kk; }
-        double frac = (rd[kk] > 0.0) ? (target - acc) / rd[kk] : 0.0;
-        frac = frac < 0.0 ? 0.0 : (frac > 1.0 ? 1.0 : frac);
-        nd[j] = x[kk] + frac * (x[kk + 1] - x[kk]);
-      }
-    } else {
-      for (int j = 0; j <= B; ++j) nd[j] = x[j];        // leave the grid
-    }
+    double a = 0.0;
+    for (int j = 0; j < B; ++j) { a += r[d * kMaxBins + j]; cum[d * kMaxBins + j] = a; }
   }
   __syncthreads();
+  // every new edge on its own: the loop's kk at edge j is the number of bins k <= B - 2 with cum[k] < target_j (cum
+  // is non-decreasing, so that set is a prefix and a binary search finds the bin the loop stops at); same acc,
+  // same frac, same bits as the loop, without its 50-step serial chain of adds and divisions (14 us of a 33 us
+  // adaptation pass at 512 points per event)
   for (int idx = threadIdx.x; idx < D * (B + 1); idx += kThreads) {
     const int d = idx / (B + 1), j = idx - d * (B + 1);
-    new_x[idx] = nx[d * (kMaxBins + 1) + j];
+    const double t = tot[d];
+    const double* x = old_x + d * (B + 1);
+    double v = x[j];                                       // end points; the whole grid when the histogram is empty
+    if ((t > 0.0) && isfinite(t) && j > 0 && j < B) {
+      const double* cd = cum + d * kMaxBins;
+      const double* rd = r + d * kMaxBins;
+      const double per = cd[B - 1] / (double)B;
+      const double target = (double)j * per;
+      int lo = 0, hi = B - 1;
+      while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (cd[mid] < target) lo = mid + 1; else hi = mid;
+      }
+      const int kk = lo;
+      const double acc = kk ? cd[kk - 1] : 0.0;
+      double frac = (rd[kk] > 0.0) ? (target - acc) / rd[kk] : 0.0;
+      frac = frac < 0.0 ? 0.0 : (frac > 1.0 ? 1.0 : frac);
+      v = x[kk] + frac * (x[kk + 1] - x[kk]);
+    }
+    new_x[idx] = v;
   }
   __syncthreads();
 }
