@@ -186,6 +186,33 @@ def test_vegas_bin_counts(mem, bins):
     assert np.all(np.abs(pg.cpu().numpy() - po) <= TOL_EVENT * np.abs(po))
 
 
+def test_vegas_grid_reproducible_ragged_and_empty_histogram(mem):
+    """S9 edge cases: fewer adaptation points than one block takes per sweep (ragged warps in the histogram rounds), an
+    event whose weights all vanish (its grid must stay the uniform one), and bitwise identical grids on a second run"""
+    import torch
+    proc, ne = 2, 5
+    ev = wl.make_events(proc, ne, seed=21)
+    ev[0, 2] = ev[3, 2] = 1e5                      # jet energies beyond the beam energy: every point is cut
+    p = oracle.params_default(proc)
+    p.vegas_iters, p.vegas_points = 3, 301
+    po, eo, go = oracle.vegas_integrate(proc, p, ev, 777, SEED, return_grid=True)
+    assert po[2] == 0.0 and np.count_nonzero(po) == ne - 1
+    with mem.Integrator(proc, vegas_iters=3, vegas_points=301) as it:
+        dev = _dev(ev)
+        pg, eg = it.integrate(dev, 777, SEED)
+        g1 = it.grid(ne).clone()
+        pg2, _ = it.integrate(dev, 777, SEED)
+        g2 = it.grid(ne)
+        assert torch.equal(g1, g2) and torch.equal(pg, pg2)
+    gg = g1.cpu().numpy()
+    assert np.max(np.abs(gg - go)) <= 1e-11
+    B = gg.shape[2] - 1
+    assert np.array_equal(gg[2], np.broadcast_to(np.arange(B + 1) / B, gg[2].shape))
+    assert pg.cpu().numpy()[2] == 0.0
+    live = po > 0
+    assert np.all(np.abs(pg.cpu().numpy()[live] - po[live]) <= TOL_EVENT * po[live])
+
+
 def test_edge_cases_and_errors(mem):
     import torch
     proc = 1
