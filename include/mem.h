@@ -148,6 +148,44 @@ mem_status mem_integrate_host(mem_handle* h, const double* events_host, int64_t 
                               int64_t n_points, uint64_t seed,
                               double* out_p_host, double* out_err_host, void* cuda_stream);
 
+/* mem_integrate for callers that must not allocate device memory.
+ *
+ * mem_integrate keeps its intermediate arrays (per-event constants, per-block partial sums, block arrival counters)
+ * in a workspace it obtains with cudaMalloc and regrows with cudaFree + cudaMalloc whenever a call is larger than
+ * any before it.  Some hosts cannot live with that: an online event filter or another real-time loop whose device
+ * memory was divided up once at start-up and where a later driver allocation may fail or stall; a host application
+ * whose own memory pool has already claimed the whole GPU; any loop in which the device-wide synchronisation that
+ * cudaFree / cudaMalloc imply would stall work queued on other streams.  For them this entry point computes the same
+ * plain Monte Carlo estimate (Eq. 5-6; same kernels, same launch geometry, same Philox counters, hence
+ * the same bits in out_p and out_err as mem_integrate) with the intermediate arrays laid out in ONE array of
+ * MEM_NOALLOC_SCRATCH_BYTES bytes that is part of the library image: every GPU on which the library gets loaded
+ * holds those bytes from then until the process exits, whether or not this function is ever called.  The call makes
+ * no cudaMalloc, cudaFree or other allocating call; the caller passes inputs and outputs exactly as to mem_integrate.
+ *
+ * Limits and rules:
+ *  - plain Monte Carlo only: a handle created with vegas_iters > 0 gets MEM_ERR_UNSUPPORTED (the VEGAS grids and
+ *    histograms are not part of the fixed array);
+ *  - the call needs  r256(4 n_events) + r256(8 K n_perm n_events) + 16 n_events n_chunks  bytes, r256 = rounded up
+ *    to 256, K = 16 / 12 / 44 / 64 / 80 constants per event for processes 1..5, n_perm = max(1, params.n_perm),
+ *    n_chunks = blocks per event (64 at 2^20 points, 16 to 32 below 2^18).  More than MEM_NOALLOC_SCRATCH_BYTES is
+ *    MEM_ERR_INVALID_ARG, with both numbers in mem_last_error(), before anything is launched: split the event list
+ *    (with mem_set_event_offset the pieces reproduce the whole list bit for bit).  The headline workload, 4096
+ *    t tbar l+jets events x 2^20 points, needs 5.4 MiB;
+ *  - the first call on each device looks up the array's device address (cudaGetSymbolAddress, with that device
+ *    current) and keeps it for the life of the process.  Make that first call during set-up, outside any CUDA
+ *    stream capture;
+ *  - every call on a device, from every handle, stream and host thread, uses the same array, which still holds what
+ *    the previous call left there: each call zeroes the arrival counters on `cuda_stream` before its kernels and
+ *    overwrites the rest before reading it.  Two such calls that overlap on the GPU (different streams with no
+ *    dependency between them) corrupt each other's results; keeping them ordered is up to the caller.  Calls of
+ *    mem_integrate are not affected: they never touch this array;
+ *  - mem_last_pass_ms does not see these calls.
+ * Arguments, error codes, asynchrony on cuda_stream and the n_events == 0 case are those of mem_integrate. */
+#define MEM_NOALLOC_SCRATCH_BYTES (8u << 20)
+mem_status mem_integrate_noalloc(mem_handle* h, const double* events, int64_t n_events,
+                                 int64_t n_points, uint64_t seed,
+                                 double* out_p, double* out_err, void* cuda_stream);
+
 /* Diagnostic for the parity tests: the individual weights w_i of one event,
  * i in [first_point, first_point + n), for Philox pass `iteration`.
  * grid (device, may be NULL): VEGAS edges [D][vegas_bins + 1] of THIS event;

@@ -18,7 +18,7 @@ MEM_OK, MEM_ERR_INVALID_ARG, MEM_ERR_UNSUPPORTED, MEM_ERR_CUDA, MEM_ERR_NOMEM = 
 MEM_PROC_W_ENU, MEM_PROC_Z_BB, MEM_PROC_TT_LJETS, MEM_PROC_TT_DILEP, MEM_PROC_TTH_DILEP = 1, 2, 3, 4, 5
 
 EXPORTS = ("mem_params_default", "mem_event_fields", "mem_n_dims", "mem_create", "mem_destroy",
-           "mem_set_event_offset", "mem_integrate", "mem_integrate_host", "mem_eval_points",
+           "mem_set_event_offset", "mem_integrate", "mem_integrate_noalloc", "mem_integrate_host", "mem_eval_points",
            "mem_eval_parton", "mem_set_pdf_grid", "mem_get_grid", "mem_launch_count", "mem_last_error", "mem_last_pass_ms", "mem_measure_fp64_peak",
            "mem_measure_fp64_peak_rrr", "mem_measure_fp64_rate", "mem_normalisation", "mem_discriminant")
 
@@ -66,6 +66,7 @@ def lib():
         L.mem_set_event_offset.argtypes = [vp, u64]
         L.mem_integrate.argtypes = [vp, dp, i64, i64, u64, dp, dp, vp]
         L.mem_integrate_host.argtypes = [vp, dp, i64, i64, u64, dp, dp, vp]
+        L.mem_integrate_noalloc.argtypes = [vp, dp, i64, i64, u64, dp, dp, vp]
         L.mem_eval_points.argtypes = [vp, dp, i64, i64, i64, i64, u64, C.c_int32, dp, dp, vp]
         L.mem_eval_parton.argtypes = [vp, dp, i64, dp, vp]
         L.mem_set_pdf_grid.argtypes = [vp, dp, C.c_int32, C.c_int32] + [C.c_double] * 5
@@ -209,6 +210,28 @@ def mem_integrate(handle, events, n_points: int, seed: int, out_p=None, out_err=
     return out_p, out_err
 
 
+MEM_NOALLOC_SCRATCH_BYTES = 8 << 20
+
+
+def mem_integrate_noalloc(handle, events, n_points: int, seed: int, out_p, out_err, stream=None):
+    """mem_integrate for hosts that must not allocate device memory (a real-time loop with a fixed memory plan, an
+    application whose own pool owns the GPU): plain Monte Carlo only, intermediate arrays in the library's fixed
+    MEM_NOALLOC_SCRATCH_BYTES array, same bits as mem_integrate.  The caller brings `out_p` and `out_err`
+    (float64 CUDA tensors [n_events]) -- nothing is allocated here either.  A call that needs more scratch than the
+    array has raises MemError (MEM_ERR_INVALID_ARG).  All calls on a device share the array: do not let two of
+    them overlap on the GPU.  See include/mem.h for the size formula and the first-call rule."""
+    if events.dim() != 2:
+        raise ValueError("events must be [n_fields, n_events]")
+    _check_tensor(handle, events, "events", mem_event_fields(handle.process) if getattr(handle, "process", 0) else None)
+    n_events = int(events.shape[1])
+    _check_tensor(handle, out_p, "out_p")
+    _check_tensor(handle, out_err, "out_err")
+    _check(lib().mem_integrate_noalloc(handle, _dev_f64(events, "events"), n_events, int(n_points), int(seed),
+                                       _dev_f64(out_p, "out_p", (n_events,)), _dev_f64(out_err, "out_err", (n_events,)),
+                                       _stream_ptr(stream)))
+    return out_p, out_err
+
+
 def mem_integrate_host(handle, events, n_points: int, seed: int, out_p=None, out_err=None, stream=None):
     """events: float64 CPU tensor or numpy array [n_fields, n_events].  Copies in, integrates, copies the
     results back into float64 CPU tensors, all on `stream` (default: torch's current stream), and synchronises it."""
@@ -318,6 +341,9 @@ class Integrator:
 
     def integrate(self, events, n_points, seed, **kw):
         return mem_integrate(self.handle, events, n_points, seed, **kw)
+
+    def integrate_noalloc(self, events, n_points, seed, out_p, out_err, **kw):
+        return mem_integrate_noalloc(self.handle, events, n_points, seed, out_p, out_err, **kw)
 
     def integrate_host(self, events, n_points, seed, **kw):
         return mem_integrate_host(self.handle, events, n_points, seed, **kw)

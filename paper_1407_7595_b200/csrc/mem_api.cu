@@ -6,6 +6,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <type_traits>
 
@@ -441,6 +442,95 @@ mem_status eval_impl(mem_handle* h, const double* events, int64_t n_events, int6
 
 }  // namespace
 
+// ---- mem_integrate_noalloc (include/mem.h): the plain Monte Carlo path with its intermediate arrays in a fixed array ----
+//
+// For hosts that cannot let a library allocate device memory after start-up (a real-time event filter with a fixed
+// memory plan, an application whose own pool owns the GPU, a loop that cannot afford the device-wide stall of
+// cudaFree / cudaMalloc).  The array below is part of the library's device image: each GPU that loads the library
+// holds MEM_NOALLOC_SCRATCH_BYTES for it until the process ends.
+//
+// In host code the name `g_noalloc_scratch` is only a host-side handle for the symbol -- not an address a kernel can
+// use -- so the device address is asked for once per device (cudaGetSymbolAddress with that device current) and it
+// is that address, never the name, that is handed to the kernels.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[MEM_NOALLOC_SCRATCH_BYTES];
+
+namespace {
+
+constexpr int kNoallocMaxDevices = 64;
+std::mutex g_noalloc_mu;
+unsigned char* g_noalloc_addr[kNoallocMaxDevices] = {};
+
+// Device address of the array on device `dev`, which must be the current device (the callers have run check_device).
+mem_status noalloc_scratch(int dev, unsigned char** out) {
+  if (dev < 0 || dev >= kNoallocMaxDevices)
+    return fail(MEM_ERR_UNSUPPORTED, "mem_integrate_noalloc: device %d is outside the %d devices it keeps an address for", dev, kNoallocMaxDevices);
+  std::lock_guard<std::mutex> lock(g_noalloc_mu);
+  if (!g_noalloc_addr[dev]) {
+    void* p = nullptr;
+    CUDA_TRY(cudaGetSymbolAddress(&p, g_noalloc_scratch));
+    if (!p || (reinterpret_cast<uintptr_t>(p) & 255u) != 0)
+      return fail(MEM_ERR_CUDA, "cudaGetSymbolAddress(g_noalloc_scratch) returned %p", p);
+    g_noalloc_addr[dev] = static_cast<unsigned char*>(p);
+  }
+  *out = g_noalloc_addr[dev];
+  return MEM_OK;
+}
+
+size_t round256(size_t b) { return (b + 255u) & ~(size_t)255u; }
+
+// prepare_kernel + the plain-MC integrate_kernel of mem_integrate, same geometry, workspace = slices of the fixed array:
+//   [ tickets: n_events x u32 | ecs: n_events x n_perm x NC f64 | partials: n_events x n_chunks x 2 f64 ]
+template <class P>
+mem_status integrate_noalloc_impl(mem_handle* h, const double* events, int64_t n_events, int64_t n_points,
+                                  uint64_t seed, double* out_p, double* out_err, cudaStream_t st) {
+  const int n_perm = h->dc.n_perm;
+  const int64_t chunk = chunk_for(n_points, P::kCompact && n_perm <= 1);
+  const int64_t n_chunks = (n_points + chunk - 1) / chunk;
+  // sizes first, in floating point so that no product can wrap, then the exact integers
+  if ((double)n_events * (double)n_chunks > (double)0x7fffffffLL)
+    return fail(MEM_ERR_INVALID_ARG, "n_events * chunks exceeds the grid limit");
+  const int64_t blocks = n_events * n_chunks;
+  const size_t b_tickets = round256((size_t)n_events * sizeof(unsigned));
+  const size_t b_ecs = round256((size_t)n_events * (size_t)n_perm * P::NC * sizeof(double));
+  const size_t b_partials = (size_t)blocks * 2 * sizeof(double);
+  const size_t need = b_tickets + b_ecs + b_partials;
+  if (need > (size_t)MEM_NOALLOC_SCRATCH_BYTES)
+    return fail(MEM_ERR_INVALID_ARG,
+                "mem_integrate_noalloc: %lld events x %lld points need %zu bytes of scratch, the fixed array has %zu; "
+                "split the event list (mem_set_event_offset keeps the pieces bit-identical to the whole)",
+                (long long)n_events, (long long)n_points, need, (size_t)MEM_NOALLOC_SCRATCH_BYTES);
+  unsigned char* base = nullptr;
+  mem_status s = noalloc_scratch(h->device, &base);
+  if (s != MEM_OK) return s;
+  unsigned* tickets = reinterpret_cast<unsigned*>(base);
+  double* ecs = reinterpret_cast<double*>(base + b_tickets);
+  double* partials = reinterpret_cast<double*>(base + b_tickets + b_ecs);
+  // the array keeps whatever the last call (or a failed one) left: the arrival counters must start at zero; the
+  // constants and partial sums are written by this call's kernels before they are read
+  CUDA_TRY(cudaMemsetAsync(tickets, 0, b_tickets, st));
+  const int64_t n_rec = n_events * n_perm;
+  prepare_kernel<P><<<(unsigned)((n_rec + 127) / 128), 128, 0, st>>>(h->dc, events, n_events, ecs);
+  ++h->launches;
+  CUDA_TRY(cudaGetLastError());
+  size_t smem = integrate_smem(P::NC * n_perm, P::D, h->dc.vegas_bins, MODE_PLAIN);
+  if constexpr (P::kCompact) smem += (size_t)kWarps * (P::kClasses + P::kPreStages) * 64 * sizeof(uint32_t);
+  auto launch = [&](auto perm, auto grid) {
+    integrate_kernel<P, MODE_PLAIN, decltype(perm)::value, decltype(grid)::value><<<(unsigned)blocks, kThreads, smem, st>>>(
+        dc_of<typename P::real>(h), ecs, nullptr, partials, nullptr, n_points, chunk, (int)n_chunks,
+        make_philox(seed), h->event_offset, 0u, tickets, out_p, out_err);
+  };
+  const bool perm = n_perm > 1, grid = h->dc.pdf_tab != nullptr;
+  if (perm && grid) launch(std::true_type{}, std::true_type{});
+  else if (perm) launch(std::true_type{}, std::false_type{});
+  else if (grid) launch(std::false_type{}, std::true_type{});
+  else launch(std::false_type{}, std::false_type{});
+  ++h->launches;
+  CUDA_TRY(cudaGetLastError());
+  return MEM_OK;
+}
+
+}  // namespace
+
 extern "C" {
 
 const char* mem_last_error(void) { return g_err; }
@@ -622,6 +712,34 @@ mem_status mem_integrate(mem_handle* h, const double* events, int64_t n_events, 
       return integrate_impl<ProcTTljets>(h, events, n_events, n_points, seed, out_p, out_err, st);
     case MEM_PROC_TT_DILEP: return integrate_impl<ProcTTdilep>(h, events, n_events, n_points, seed, out_p, out_err, st);
     case MEM_PROC_TTH_DILEP: return integrate_impl<ProcTTHdilep>(h, events, n_events, n_points, seed, out_p, out_err, st);
+  }
+  return fail(MEM_ERR_UNSUPPORTED, "process %d is not implemented", h->process);
+}
+
+mem_status mem_integrate_noalloc(mem_handle* h, const double* events, int64_t n_events, int64_t n_points, uint64_t seed,
+                                 double* out_p, double* out_err, void* cuda_stream) {
+  if (!h) return fail(MEM_ERR_INVALID_ARG, "handle is NULL");
+  if (n_events < 0) return fail(MEM_ERR_INVALID_ARG, "n_events < 0");
+  if (n_points < 2) return fail(MEM_ERR_INVALID_ARG, "n_points < 2");
+  if (h->params.vegas_iters > 0)
+    return fail(MEM_ERR_UNSUPPORTED, "mem_integrate_noalloc is plain Monte Carlo only (this handle has vegas_iters = %d)", h->params.vegas_iters);
+  if (n_events == 0) return MEM_OK;
+  if (!events || !out_p || !out_err) return fail(MEM_ERR_INVALID_ARG, "events / out_p / out_err is NULL");
+  if (!aligned8(events) || !aligned8(out_p) || !aligned8(out_err))
+    return fail(MEM_ERR_INVALID_ARG, "device pointers must be 8-byte aligned");
+  mem_status cs = check_device(h);
+  if (cs == MEM_OK) cs = check_counter(h, n_events);
+  if (cs != MEM_OK) return cs;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  switch (h->process) {
+    case MEM_PROC_W_ENU: return integrate_noalloc_impl<ProcWenu>(h, events, n_events, n_points, seed, out_p, out_err, st);
+    case MEM_PROC_Z_BB: return integrate_noalloc_impl<ProcZbb>(h, events, n_events, n_points, seed, out_p, out_err, st);
+    case MEM_PROC_TT_LJETS:
+      if (h->params.precision == 32)
+        return integrate_noalloc_impl<ProcTTljetsF>(h, events, n_events, n_points, seed, out_p, out_err, st);
+      return integrate_noalloc_impl<ProcTTljets>(h, events, n_events, n_points, seed, out_p, out_err, st);
+    case MEM_PROC_TT_DILEP: return integrate_noalloc_impl<ProcTTdilep>(h, events, n_events, n_points, seed, out_p, out_err, st);
+    case MEM_PROC_TTH_DILEP: return integrate_noalloc_impl<ProcTTHdilep>(h, events, n_events, n_points, seed, out_p, out_err, st);
   }
   return fail(MEM_ERR_UNSUPPORTED, "process %d is not implemented", h->process);
 }
