@@ -59,11 +59,12 @@ def _cuobjdump():
     return "cuobjdump"
 
 
-def kernel_name(key: str):
+def kernel_name(key: str, lib: str | None = None):
     """full mangled name of the kernel of `key` in the built library (None if it cannot be listed)"""
+    lib = lib or _build.LIB
     try:
-        out = subprocess.run([_cuobjdump(), "-elf", "-lelf", _build.LIB], capture_output=True, text=True, timeout=60).stdout
-        out += subprocess.run([_cuobjdump(), "-symbols", _build.LIB], capture_output=True, text=True, timeout=60).stdout
+        out = subprocess.run([_cuobjdump(), "-elf", "-lelf", lib], capture_output=True, text=True, timeout=60).stdout
+        out += subprocess.run([_cuobjdump(), "-symbols", lib], capture_output=True, text=True, timeout=60).stdout
     except (OSError, subprocess.SubprocessError):
         return None
     pat = KERNELS[key]
@@ -73,17 +74,27 @@ def kernel_name(key: str):
     return None
 
 
-def sass_sha256(key: str):
-    """SHA-256 of the SASS listing (instructions and encodings) of the kernel of `key`; None if unavailable"""
-    name = kernel_name(key)
+def _instruction(line: str) -> str:
+    """one SASS listing line reduced to what the kernel executes: address, opcode, operands.  The encoding comment is
+    dropped and the slot of constant bank 4 (where the linker keeps the addresses of the library's global arrays) is
+    masked: that slot moves whenever a global is added anywhere in the library (the fixed array of
+    mem_integrate_noalloc moved kExpTab's from 0x0 to 0x8) without changing a single instruction."""
+    line = re.sub(r"/\*\s*0x[0-9a-f]+\s*\*/\s*$", "", line.strip()).rstrip()
+    return re.sub(r"c\[0x4\]\[[^\]]*\]", "c[0x4][*]", line)
+
+
+def sass_sha256(key: str, lib: str | None = None):
+    """SHA-256 of the SASS listing (addresses, opcodes, operands; see _instruction) of the kernel of `key`; None if unavailable"""
+    lib = lib or _build.LIB
+    name = kernel_name(key, lib)
     if name is None:
         return None
     try:
-        out = subprocess.run([_cuobjdump(), "-sass", "-fun", name, _build.LIB], capture_output=True, text=True,
+        out = subprocess.run([_cuobjdump(), "-sass", "-fun", name, lib], capture_output=True, text=True,
                              timeout=120).stdout
     except (OSError, subprocess.SubprocessError):
         return None
-    lines = [l.strip() for l in out.splitlines() if re.match(r"\s+/\*[0-9a-f]{4,}\*/", l)]
+    lines = [_instruction(l) for l in out.splitlines() if re.match(r"\s+/\*[0-9a-f]{4,}\*/", l)]
     if not lines:
         return None
     return hashlib.sha256("\n".join(lines).encode()).hexdigest()
