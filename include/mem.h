@@ -134,6 +134,9 @@ mem_status mem_set_event_offset(mem_handle* h, uint64_t first_event);
  *   replayed (mem_last_pass_ms does not see captured calls).
  * n_events == 0 is MEM_OK with no launch; n_points < 2 is MEM_ERR_INVALID_ARG; so is a call made while
  * another CUDA device than the handle's is current.
+ * A call that fails after it has started launching (MEM_ERR_NOMEM or MEM_ERR_CUDA between two passes) leaves
+ * out_p / out_err undefined but the handle usable: the next call on it first resets the workspace's block arrival
+ * counters on its stream.  After a sticky CUDA error (every later CUDA call fails too) destroy the handle.
  * Kinematically forbidden or non-finite points contribute w = 0 and still count in N. */
 mem_status mem_integrate(mem_handle* h, const double* events, int64_t n_events,
                          int64_t n_points, uint64_t seed,
@@ -254,19 +257,6 @@ mem_status mem_last_pass_ms(mem_handle* h, double* ms, int64_t* evals);
  * *tflops (host, out) = 2 * fused multiply-adds / second / 1e12, best of `repeats` launches.
  * The denominator of the "alu" roofline (MEASURED_PEAKS.json has no FP64 figure). */
 mem_status mem_measure_fp64_peak(int32_t repeats, double* tflops, void* cuda_stream);
-
-/* The same measurement with three distinct 64-bit register operands per DFMA (x = fma(x, y, z), y and z in
- * registers): what the register file sustains for generic fused multiply-adds, about 2/3 of the figure
- * above on B200.  Reported beside the roofline as the ceiling of register-operand code. */
-mem_status mem_measure_fp64_peak_rrr(int32_t repeats, double* tflops, void* cuda_stream);
-
-/* The family of FP64 issue microbenchmarks behind the roofline discussion.  Every kind runs
- * 8 independent FP64 instruction chains per thread; *tflops = 2 * FP64 instructions / second / 1e12 (i.e. an FMA
- * counts 2 in every kind, so the figures compare instruction rates).  kind 0: DFMA with two uniform operands (=
- * mem_measure_fp64_peak); 1: DFMA with three register operands (= ..._rrr); 2: 5 DFMA : 2 DMUL : 1 DADD with
- * shuffled register operands; 3 / 4: kind 0 plus 8 / 16 independent integer instructions per 8 DFMAs; 5: DMUL and
- * 6: DADD with two register operands. */
-mem_status mem_measure_fp64_rate(int32_t kind, int32_t repeats, double* tflops, void* cuda_stream);
 
 /* Thread-local description of the last error on this thread ("" if none). */
 const char* mem_last_error(void);

@@ -169,7 +169,7 @@ def mem_measure_fp64_peak_rrr(repeats: int = 5, stream=None) -> float:
 
 
 def mem_measure_fp64_rate(kind: int, repeats: int = 5, stream=None) -> float:
-    """FP64 issue microbenchmarks (include/mem.h): 2 x FP64 instructions/s/1e12 for instruction mix `kind`."""
+    """FP64 issue microbenchmarks (include/mem_bench.h): 2 x FP64 instructions/s/1e12 for instruction mix `kind`."""
     t = C.c_double()
     _check(lib().mem_measure_fp64_rate(int(kind), int(repeats), C.byref(t), _stream_ptr(stream)))
     return t.value

@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmem_b200.so")
 SOURCES = [os.path.join(CSRC, "mem_api.cu")]
 HEADERS = [os.path.join(CSRC, f) for f in ("mem_common.cuh", "mem_processes.cuh", "mem_kernels.cuh", "mem_parton.cuh", "mem_tth.cuh")] + [
-    os.path.join(ROOT, "include", "mem.h")]
+    os.path.join(ROOT, "include", "mem.h"), os.path.join(ROOT, "include", "mem_bench.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]

@@ -1,6 +1,7 @@
 // mem_api.cu -- the C ABI of include/mem.h: argument checks, workspace, kernel launches.
 // No arithmetic of the method lives here beyond turning mem_params into DevConst.
 #include "../../include/mem.h"
+#include "../../include/mem_bench.h"
 
 #include <cmath>
 #include <cstdarg>
@@ -86,6 +87,7 @@ struct mem_handle {
   cudaEvent_t ev_begin, ev_end;  // around the dominant kernel of the last mem_integrate
   cudaEvent_t ev_done;           // recorded after the last launch of every call that uses the workspace
   bool has_done;                 // ev_done has been recorded at least once
+  bool tickets_dirty;            // a mem_integrate on this handle returned an error after it had started launching
   int64_t last_evals;            // integrand evaluations of that kernel; 0 = none yet
 };
 
@@ -236,6 +238,7 @@ mem_status check_params(int process, const mem_params& p) {
   if (p.struct_size != sizeof(mem_params))
     return fail(MEM_ERR_INVALID_ARG, "mem_params.struct_size = %u, expected %zu", p.struct_size, sizeof(mem_params));
   if (p.precision != 64 && p.precision != 32) return fail(MEM_ERR_INVALID_ARG, "precision must be 64 or 32");
+  if (p.reserved0 != 0) return fail(MEM_ERR_INVALID_ARG, "mem_params.reserved0 must be 0");
   if (p.precision == 32 && process != MEM_PROC_TT_LJETS)
     return fail(MEM_ERR_UNSUPPORTED, "precision 32 is implemented for MEM_PROC_TT_LJETS only (reading A15)");
   const bool pos = p.sqrt_s > 0 && p.G_F > 0 && p.m_W > 0 && p.Gam_W > 0 && p.m_Z > 0 && p.Gam_Z > 0 && p.m_t > 0 &&
@@ -374,13 +377,11 @@ mem_status launch_timed_pass(mem_handle* h, int64_t n_events, int64_t n_points, 
   return MEM_OK;
 }
 
+// the launches of one mem_integrate, between begin_call and end_call
 template <class P>
-mem_status integrate_impl(mem_handle* h, const double* events, int64_t n_events, int64_t n_points, uint64_t seed,
-                          double* out_p, double* out_err, cudaStream_t st) {
-  bool capturing = false;
-  mem_status s = begin_call(h, st, &capturing);
-  if (s != MEM_OK) return s;
-  s = launch_prepare<P>(h, events, n_events, st);
+mem_status integrate_launches(mem_handle* h, const double* events, int64_t n_events, int64_t n_points, uint64_t seed,
+                              double* out_p, double* out_err, cudaStream_t st, bool capturing) {
+  mem_status s = launch_prepare<P>(h, events, n_events, st);
   if (s != MEM_OK) return s;
   const int64_t chunk = chunk_for(n_points, P::kCompact && h->params.vegas_iters == 0 && h->dc.n_perm <= 1);
   const int n_chunks = (int)((n_points + chunk - 1) / chunk);
@@ -418,7 +419,32 @@ mem_status integrate_impl(mem_handle* h, const double* events, int64_t n_events,
   } else {
     s = launch_timed_pass<P, MODE_PLAIN>(h, n_events, n_points, n_chunks, seed, 0u, st, capturing, out_p, out_err);
   }
+  return s;
+}
+
+// The arrival counters are zero between calls only because every pass runs to its end (the last block of an event
+// resets its counter).  A call that returns an error part-way (an allocation or a launch refused between two VEGAS
+// passes, a launch failure) may leave some of them counting, and a later pass would then finish events early from
+// partial sums not yet written, or never.  So a failed call marks the handle; the next call zeroes the counters on its
+// stream before it launches anything.  A failed call also leaves its event behind, so that the next call is still
+// ordered after whatever did get launched.  (After a sticky CUDA error nothing helps: destroy the handle.)
+template <class P>
+mem_status integrate_impl(mem_handle* h, const double* events, int64_t n_events, int64_t n_points, uint64_t seed,
+                          double* out_p, double* out_err, cudaStream_t st) {
+  bool capturing = false;
+  mem_status s = begin_call(h, st, &capturing);
   if (s != MEM_OK) return s;
+  if (h->tickets_dirty && h->tickets.p) CUDA_TRY(cudaMemsetAsync(h->tickets.p, 0, h->tickets.cap, st));
+  h->tickets_dirty = true;
+  s = integrate_launches<P>(h, events, n_events, n_points, seed, out_p, out_err, st, capturing);
+  if (s != MEM_OK) {
+    char keep[sizeof(g_err)];
+    std::memcpy(keep, g_err, sizeof(keep));            // end_call may overwrite the message of the real failure
+    (void)end_call(h, st, capturing);
+    std::memcpy(g_err, keep, sizeof(keep));
+    return s;
+  }
+  h->tickets_dirty = false;
   return end_call(h, st, capturing);
 }
 
@@ -584,7 +610,7 @@ mem_status mem_create(mem_process process, const mem_params* params, mem_handle*
   mem_handle* h = new (std::nothrow) mem_handle();
   if (!h) return fail(MEM_ERR_NOMEM, "out of host memory");
   h->process = (int)process; h->device = dev; h->params = p; h->dc = make_dev_const(p); h->dcf = to_float(h->dc);
-  h->event_offset = 0; h->launches = 0; h->grid_events = 0; h->last_evals = 0; h->has_done = false;
+  h->event_offset = 0; h->launches = 0; h->grid_events = 0; h->last_evals = 0; h->has_done = false; h->tickets_dirty = false;
   cudaError_t ce = cudaEventCreate(&h->ev_begin);
   if (ce == cudaSuccess) ce = cudaEventCreate(&h->ev_end);
   if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&h->ev_done, cudaEventDisableTiming);

@@ -76,6 +76,7 @@ __device__ __forceinline__ double vegas_map(const double* edges, int B, double (
 // instructions per 32 points at D = 6 and a serial chain of match, votes and shuffles per dimension.)
 template <int D>
 __device__ __forceinline__ void warp_hist_add(double* wh, int B, const int (&k)[D], bool live, double v) {
+  static_assert(kMaxBins <= 64, "the peer masks below compare six bits of the bin index");
   const unsigned full = 0xffffffffu;
   const int lane = threadIdx.x & 31;
   const unsigned lt = (1u << lane) - 1u;
@@ -408,6 +409,9 @@ integrate_kernel(const DevConstR<typename P::real> c, const double* __restrict__
   __threadfence();                                         // this block's partials / histogram are visible device-wide
   __syncthreads();
   if (threadIdx.x == 0) {
+    // the barrier has ordered the other threads' stores before this point; this second fence makes the ticket
+    // increment release them too (fence, barrier, fence, atomic: cumulative by the PTX memory model, not just in practice)
+    __threadfence();
     const unsigned t = atomicAdd(tickets + e, 1u);
     s_last = (t == (unsigned)n_chunks - 1u);
     if (s_last) tickets[e] = 0u;                           // ready for the next pass

@@ -13,9 +13,20 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def _declared_symbols():
+    """every function declared by a header under include/ (mem.h: the integrator; mem_bench.h: microbenchmarks)"""
+    names = set()
+    inc = os.path.join(ROOT, "include")
+    for f in sorted(os.listdir(inc)):
+        if f.endswith(".h"):
+            text = re.sub(r"/\*.*?\*/", "", open(os.path.join(inc, f)).read(), flags=re.S)
+            names |= set(re.findall(r"\b(mem_[a-z0-9_]+)\s*\(", text))
+    return sorted(names)
+
+
+def test_microbenchmarks_are_not_in_the_integrator_header():
     text = open(os.path.join(ROOT, "include", "mem.h")).read()
-    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(mem_[a-z0-9_]+)\s*\(", text)))
+    assert "mem_measure_fp64_rate" not in text and "mem_measure_fp64_peak_rrr" not in text
+    assert "mem_measure_fp64_peak(" in text                       # the roofline denominator stays
 
 
 def test_library_builds_and_exports_every_declared_symbol():
@@ -52,6 +63,15 @@ def test_every_python_field_is_in_the_header_in_order():
         if m:
             names += [n.strip() for n in m.group(1).split(",")]
     assert names == [f[0] for f in mem.mem_params._fields_]
+
+
+def test_reserved_field_must_be_zero():
+    # include/mem.h: "reserved0 must be 0"; rejected by the parameter check, before any CUDA call
+    p = mem.mem_params_default(mem.MEM_PROC_TT_LJETS)
+    p.reserved0 = 1
+    with pytest.raises(mem.MemError) as ei:
+        mem.mem_create(mem.MEM_PROC_TT_LJETS, p)
+    assert ei.value.status == mem.MEM_ERR_INVALID_ARG and "reserved0" in str(ei.value)
 
 
 def test_no_cpu_fallback_without_a_device():
