@@ -6,26 +6,27 @@ FMUL / FADD) instructions per sample point from an ncu metric pass, together wit
 figures and recomputes the hash of the kernel it is about to time: a count taken on another build is reported as
 stale instead of being silently reused (measurement item 8).
 
-Refresh after a kernel change (on the GPU box; writes the JSON in place):
+How a record is made (after a kernel change, on the GPU box): one ncu metric pass over a short bench.py run,
 
     ncu --metrics smsp__sass_thread_inst_executed_op_dfma_pred_on.sum,smsp__sass_thread_inst_executed_op_dmul_pred_on.sum,\
 smsp__sass_thread_inst_executed_op_dadd_pred_on.sum,smsp__sass_thread_inst_executed_op_ffma_pred_on.sum,\
 smsp__sass_thread_inst_executed_op_fmul_pred_on.sum,smsp__sass_thread_inst_executed_op_fadd_pred_on.sum \
         --clock-control none -k regex:integrate_kernel --csv --log-file gpurun_out/counts_c3.csv \
-        python bench.py --config 3 --events 592 --points 65536 --steps 1 --warmup 3 --no-cpu-baseline
-    python -m paper_1407_7595_b200.counts --update gpurun_out/counts_c3.csv --key 3,1,64 --points 38797312
+        python bench.py --config 3 --events 37 --steps 1 --warmup 3 --no-cpu-baseline
+
+then, for the launch of KERNELS[key] with the most FP instructions, each metric divided by the sample points of that
+launch (events x points), rounded to 0.01, stored with sass_sha256(key) of the library that ran
+(profiles/r03_fp64_counts.md lists the runs of this round).  This module only reads the file.
 
 No arithmetic of the method lives here.
 """
 from __future__ import annotations
 
-import csv
 import hashlib
 import json
 import os
 import re
 import subprocess
-import sys
 
 from . import build as _build
 
@@ -118,58 +119,3 @@ def lookup(config: int, perm: int = 1, precision: int = 64, check_build: bool = 
         h = sass_sha256(key)
         rec["match"] = None if h is None else (h == rec.get("sass_sha256"))
     return rec
-
-
-def update(csv_path: str, key: str, points: int, note: str = ""):
-    """parse an ncu --csv metric log, take the launch of KERNELS[key] with the most FP instructions, store per-point counts"""
-    rows = list(csv.reader(l for l in open(csv_path) if l.startswith('"')))
-    hdr = rows[0]
-    i_name, i_metric, i_val, i_id = hdr.index("Kernel Name"), hdr.index("Metric Name"), hdr.index("Metric Value"), hdr.index("ID")
-    cfg, perm, prec = (int(x) for x in key.split(",")[:3])
-    proc = {1: "ProcWenu", 2: "ProcZbb", 3: "ProcTTljetsR", 4: "ProcTTdilep", 5: "ProcTTljetsR", 6: "ProcTTHdilep"}[cfg]
-    if proc == "ProcTTljetsR":
-        proc += "<double>" if prec == 64 else "<float>"
-    # ncu's CSV prints the short demangled form: integrate_kernel<ProcTTljetsR<double>, 1, 0, 0>
-    want = re.compile(r"integrate_kernel<(memb200::)?%s, (\(int\))?%d, (\(bool\))?%d, (\(bool\))?0>" % (re.escape(proc), 1 if cfg == 5 else 0, 1 if perm > 1 else 0))
-    demangled = want.pattern
-    per_launch = {}
-    for r in rows[1:]:
-        if not want.search(r[i_name]):
-            continue
-        for short, m in METRICS.items():
-            if m in r[i_metric]:
-                per_launch.setdefault(r[i_id], {})[short] = float(r[i_val].replace(",", ""))
-    if not per_launch:
-        raise SystemExit("no integrate_kernel<%s> launch in %s" % (demangled, csv_path))
-    best = max(per_launch.values(), key=lambda d: sum(d.values()))
-    rec = {k: round(v / points, 2) for k, v in best.items() if v > 0}
-    rec.update(kernel=KERNELS[key], sass_sha256=sass_sha256(key), points_per_launch=points, source=os.path.basename(csv_path))
-    if note:
-        rec["note"] = note
-    data = load()
-    for keep in ("dram_bytes", "dram_bytes_source"):          # full-size traffic figures survive a count refresh
-        if keep in data.get(key, {}):
-            rec[keep] = data[key][keep]
-    data[key] = rec
-    with open(PATH, "w") as f:
-        json.dump(data, f, indent=1, sort_keys=True)
-        f.write("\n")
-    return rec
-
-
-if __name__ == "__main__":
-    import argparse
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--update", help="ncu --csv metric log")
-    ap.add_argument("--key", help="config,assignments,precision")
-    ap.add_argument("--points", type=int, help="sample points of the measured launch")
-    ap.add_argument("--note", default="")
-    ap.add_argument("--check", action="store_true", help="print every stored key with its build match")
-    a = ap.parse_args()
-    if a.update:
-        print(json.dumps(update(a.update, a.key, a.points, a.note)))
-    if a.check:
-        for k in sorted(load()):
-            f = k.split(",")
-            print(k, lookup(int(f[0]), int(f[1]), int(f[2]), variant=f[3] if len(f) > 3 else ""))
-    sys.exit(0)

@@ -420,9 +420,9 @@ template <bool TAB> __device__ __forceinline__ float x_exp(float x) { return m_e
 template <bool TAB> __device__ __forceinline__ double b_exp(double x) { return TAB ? exp_tab<false>(x) : exp(x); }
 template <bool TAB> __device__ __forceinline__ float b_exp(float x) { return m_exp(x); }
 
-// TAB: exp_tab instead of libdevice's exp (fp64 only).  Measured: configs 2 and 4 gain 5.7 % and 5.8 %;
-// config 3's time does not move (its plain kernel sits on the mixed-operand FP64 ceiling either way) while
-// its executed flop count, hence the reported roofline fraction, would drop: it keeps libdevice's exp.
+// TAB: exp_tab instead of libdevice's exp (fp64 only).  Every integrate kernel is instantiated with TAB = true
+// (mem_kernels.cuh); TAB = false is passed only at the fp32 variant's call sites, where the flag has no effect.
+// Measured when it went in: configs 2 and 4 gain 5.7 % and 5.8 %, the VEGAS passes 3 %.
 template <bool TAB = false, typename T>
 __device__ __forceinline__ void tf_accum(const DevConstR<T>& c, T inv_x, TfAcc<T>& acc) {
   // fp64: z1^2 - z2^2 as a quadratic in inv_x (coefficients tf_q2, tf_q1, tf_q0 from the host): four FP64

@@ -60,7 +60,6 @@ struct ProcWenu {
   using real = double;
   static constexpr bool kCompact = false;   // lane compaction in the plain integrate kernel
   static constexpr int kClasses = 0, kPreStages = 0;
-  static constexpr bool kHeavy = false;   // see min_blocks() in mem_kernels.cuh
   static constexpr bool kSplitC0 = false;
   static constexpr int D = 1, NF = 5, NC = 16;
   enum { LM, LP, LE, LZ, PT, NT2, A, CLO, CHI, DT, ISCLO, DSM, PTNT, IPT2, C0, _N };
@@ -188,7 +187,6 @@ struct ProcZbb {
   using real = double;
   static constexpr bool kCompact = false;   // lane compaction in the plain integrate kernel
   static constexpr int kClasses = 0, kPreStages = 0;
-  static constexpr bool kHeavy = false;   // see min_blocks() in mem_kernels.cuh
   static constexpr bool kSplitC0 = false;
   static constexpr int D = 2, NF = 6, NC = 12;
   enum { J0 = 0, J1 = 5, C0 = 10, KT = 11 };
@@ -252,7 +250,6 @@ struct ProcTTljetsR {
   using real = T;
   static constexpr bool kCompact = false;
   static constexpr int kClasses = 0, kPreStages = 0;
-  static constexpr bool kHeavy = false;
   static constexpr int D = 6, NF = 17, NC = 44;
   static constexpr bool kSplitC0 = !std::is_same<T, double>::value;
   enum { LE, LX, LY, LZ, ELI, EL, LPT2, OMC, CPN, SPN,   // lepton, neutrino azimuth
@@ -313,8 +310,7 @@ struct ProcTTljetsR {
   // blocks.  Everything that depends only on the point -- energy fractions, transfer functions
   // (functions of E / E_jet alone), the neutrino -- is computed once; only the jet momenta, the
   // invariants, the boost and the matrix element are repeated per assignment.
-  // TAB: table-driven exp (fp64).  The plain kernel does not gain from it and keeps
-  // libdevice's exp; the VEGAS passes gain 3 %.
+  // TAB: table-driven exp (fp64); true in every integrate kernel (mem_kernels.cuh).
   template <bool PERM, bool GRIDPDF, bool TAB>
   __device__ static T weight_t(const DevConstR<T>& c, const T* ec0, const T (&u)[D]) {
     const T* ec = ec0;
@@ -516,7 +512,6 @@ __device__ __forceinline__ int quartic_real_roots(double a3, double a2, double a
 struct ProcTTdilep {
   using real = double;
   static constexpr bool kCompact = true;   // lane compaction in the plain integrate kernel
-  static constexpr bool kHeavy = true;   // see min_blocks() in mem_kernels.cuh
   static constexpr bool kSplitC0 = false;
   static constexpr int D = 8, NF = 14, NC = 64;
   static constexpr int kNewton = 3;      // Newton steps on the un-squared equations per root

@@ -37,7 +37,6 @@ __device__ inline void tth_assignment(int n_perm, int k, int (&sig)[4]) {
 struct ProcTTHdilep {
   using real = double;
   static constexpr bool kCompact = true;    // staged lane compaction in the plain integrate kernel
-  static constexpr bool kHeavy = true;
   static constexpr bool kSplitC0 = false;
   static constexpr int D = 8, NF = 18, NC = 80;
   static constexpr int kNewton = 3;
