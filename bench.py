@@ -34,8 +34,9 @@ SEED = 20140729
 #    (counts.py); a count that belongs to another build is reported as stale, never silently reused;
 #  - algorithmic: a fixed reference, flop = 2 FMA + MUL + ADD of the formulas as first implemented (the round-1
 #    kernels' executed counts, profiles/r01_fp64_counts.md, with every exponential at the cost of the table-driven
-#    implementation), NOT updated when later kernels remove instructions -- so that faster code never scores lower.
-#    roofline.frac uses this one.  Key = (config, jet-parton assignments per point).
+#    implementation), NOT updated when later kernels remove instructions; reported as frac_fixed_reference.
+#    roofline.frac uses the executed count; the fixed one only where no executed count exists.
+#    Key = (config, jet-parton assignments per point).
 ALGORITHMIC_FLOP = {
     (1, 1): 240.0,       # 87.3 DFMA, 47.0 DMUL, 18.4 DADD
     (2, 1): 224.6,       # 86.0, 37.0, 15.6
@@ -357,17 +358,31 @@ def run_b200(args):
     rate = k_evals / (k_ms * 1e-3) / 1e12                  # 1e12 evaluations/s of the dominant kernel
     sms = torch.cuda.get_device_properties(local_rank).multi_processor_count
     sm_mhz = (clocks or {}).get("sm_mhz") or 0.0
-    achieved = None if fl_alg is None else rate * fl_alg
+    # Headline: the FP64 flops the timed kernel executes (thread-level DFMA x 2 + DMUL + DADD per call from
+    # fp64_counts.json, tied to this build by its SASS hash), so that achieved / frac can be reproduced from profiles/.
+    # The fixed round-1 count stays beside it as "useful work per call as first implemented"; it is the fallback only
+    # for variants without an executed count (grid PDFs), and the line says which basis it used.
+    stale = ex is not None and ex.get("match") is False
+    if fl_ex is not None:
+        achieved, basis = rate * fl_ex, "executed" + (" (STALE: the counts were taken on another build of this kernel)" if stale else "")
+    elif fl_alg is not None:
+        achieved, basis = rate * fl_alg, "fixed_reference (no executed count for this variant)"
+    else:
+        achieved, basis = None, None
+    fixed = None if fl_alg is None else rate * fl_alg
     roofline = {
         "bound": "alu", "kernel": "integrate_kernel<%s>" % ("ProcTTljets,GRID" if cfg == 5 else "proc%d,PLAIN" % proc),
         "achieved": achieved, "peak": peak_meas, "unit": "TFLOP/s",
         "frac": None if achieved is None else achieved / peak_meas,
-        "flop_per_call_algorithmic": fl_alg,
-        "flop_per_call_algorithmic_note": "fixed reference count (bench.py: ALGORITHMIC_FLOP, DESIGN.md section 5); "
-                                          "achieved and frac use it",
+        "frac_basis": basis,
         "flop_per_call_executed": fl_ex,
         "achieved_executed": None if fl_ex is None else rate * fl_ex,
         "frac_executed": None if fl_ex is None else rate * fl_ex / peak_meas,
+        "flop_per_call_algorithmic": fl_alg,
+        "flop_per_call_algorithmic_note": "fixed reference count (bench.py: ALGORITHMIC_FLOP, DESIGN.md section 5), "
+                                          "not updated when kernels shed instructions",
+        "achieved_fixed_reference": fixed,
+        "frac_fixed_reference": None if fixed is None else fixed / peak_meas,
         "executed_counts": None if ex is None else {k: ex[k] for k in ("dfma", "dmul", "dadd") if k in ex},
         "executed_counts_match_build": None if ex is None else ex.get("match"),
         "peak_source": "measured in this run: independent DFMA chains on all SMs (mem_measure_fp64_peak)",
