@@ -5,22 +5,21 @@ for the neutrino momenta; next to a tangency of the conics the solution and its 
 ill-conditioned in fp64 on either side ("double precision is required due to
 cancellation of large coefficients"), so the fp64 oracle itself departs from its long-double
 referee by more than 1e-12 at ~0.3 % of the live points.  The bar is therefore:
-  A  identical zero pattern (same points have no solution / fail the cuts), except at isolated near-tangent
-     points (at most 2e-4 of the live ones) where the root count is decided by rounding; there one of the two
-     fp64 evaluations must side with the long-double referee (tests/helpers.py: check_points_conic)
+  A  identical zero pattern (same points have no solution / fail the cuts)
   B  |w_gpu - w_ref| <= 1e-12 |w_ref| at >= 99 % of the live points
   C  at every live point |w_gpu - w_ref| <= 1e-12 |w_ref| + 4 |w_orc - w_ref|, except at most 0.1 % of
-     them, and never beyond 1e-8
+     them, and never beyond 1e-10
   D  the 99.9th percentile of the GPU's error is not larger than twice the fp64 oracle's
-Per-event bar: |p_gpu - p_orc| <= 1e-9 |p_orc|, same for the standard error; an event that misses it is
-taken apart point by point (check_events_conic): the miss must come from <= 2e-4 of its live points, each
-adjudicated by the referee, must stay below 2 % of the statistical error, and the rest must sum to 1e-9.
+Per-event bar: |p_gpu - p_orc| <= 1e-9 |p_orc| on every event, same for the standard error -- no allowance
+(tests/helpers.py: check_points_conic, check_events_conic with max_miss = 0).  These are round 1's bars; the round-2
+relaxations (zero-pattern flips, 15 % of the events) are gone: measured on this round's kernel, no config-4 test
+needs them (profiles/r03_conic_parity.md).
 """
 import numpy as np
 import pytest
 
 import oracle
-from helpers import check_events_conic, check_points_conic, conic_ill_conditioned
+from helpers import check_events_conic, check_points_conic
 from paper_1407_7595_b200 import workloads as wl
 
 pytestmark = pytest.mark.gpu
@@ -103,7 +102,7 @@ def test_per_event_parity(mem, ne, n_points):
     with mem.Integrator(PROC) as it:
         pg, eg = it.integrate(_dev(ev), n_points, SEED)
         pg, eg = pg.cpu().numpy(), eg.cpu().numpy()
-    check_events_conic(pg, eg, po, eo, _drill(mem, ev, n_points), n_points, ill=conic_ill_conditioned(ev))
+    check_events_conic(pg, eg, po, eo, _drill(mem, ev, n_points), n_points)
     if n_points > 1000:
         assert (po > 0).sum() >= ne // 4
 
@@ -161,5 +160,4 @@ def test_full_size_sampled_outputs(mem):
     for e in list(rng.choice(live, 3, replace=False)) + list(rng.choice(dead, 1)):
         one = np.ascontiguousarray(ev[:, e:e + 1])
         po, eo = oracle.integrate(proc, p, one, n_points, SEED, event_offset=int(e))
-        check_events_conic(pg[e:e + 1], eg[e:e + 1], po, eo, _drill(mem, one, n_points, offset=int(e)), n_points,
-                           ill=conic_ill_conditioned(one, n_jets=2))
+        check_events_conic(pg[e:e + 1], eg[e:e + 1], po, eo, _drill(mem, one, n_points, offset=int(e)), n_points)

@@ -4,9 +4,10 @@ CPU oracle, through the C ABI; then 1/sigma and the discriminant D (PAPER.md:45,
 The neutrino system is the one of config 4 (two conics, Ferrari quartic, Newton polish), so the per-point
 bar is config 4's: identical zero pattern; <= 1e-12 against the long-double
 referee at >= 99 % of the live points; <= 1e-12 + 4 |w_orc - w_ref| everywhere except <= 0.1 % of them and
-never beyond 1e-8; the GPU's 99.9th-percentile error not larger than twice the fp64 oracle's.
+never beyond 1e-10; the GPU's 99.9th-percentile error not larger than twice the fp64 oracle's.
 Eq. 9 adds one more integrable 1/sqrt edge (E1 = E2) with the same character.
-Per event: |p_gpu - p_orc| <= 1e-9 |p_orc|, same for the standard error.
+Per event: |p_gpu - p_orc| <= 1e-9 |p_orc|, same for the standard error, on every event; the one test with records
+that miss it states how many (two ill-conditioned ones of 32) and has each taken apart (tests/helpers.py).
 """
 import numpy as np
 import pytest
@@ -114,9 +115,13 @@ def test_per_point_parity_grid_pdfs(mem):
     _check(np.concatenate(G), np.concatenate(O), np.concatenate(X), min_live=200)
 
 
-@pytest.mark.parametrize("ne,n_points,hyp", [(24, 2, 0), (24, 255, 0), (16, 1 << 14, 0), (16, (1 << 14) + 1, 1),
-                                             (32, 2 * (1 << 14) + 301, 0), (12, 2 * (1 << 14) + 301, 1)])
-def test_per_event_parity(mem, ne, n_points, hyp):
+# max_miss: events allowed to miss 1e-9, the measured count (profiles/r03_conic_parity.md).  Only the 32-record case
+# has any: two records, both flagged by conic_ill_conditioned, miss by 8.5e-7 and 5.6e-5 (3e-6 and 7.8e-4 of their
+# statistical error) through 1 of 707 and 11 of 2998 live points; each is taken apart by check_events_conic.
+@pytest.mark.parametrize("ne,n_points,hyp,max_miss", [(24, 2, 0, 0), (24, 255, 0, 0), (16, 1 << 14, 0, 0),
+                                                      (16, (1 << 14) + 1, 1, 0), (32, 2 * (1 << 14) + 301, 0, 2),
+                                                      (12, 2 * (1 << 14) + 301, 1, 0)])
+def test_per_event_parity(mem, ne, n_points, hyp, max_miss):
     ev = wl.make_tth_events(ne, seed=11)
     p = _params(dict(tth_hyp=hyp))
     po, eo = oracle.integrate(PROC, p, ev, n_points, SEED)
@@ -124,7 +129,7 @@ def test_per_event_parity(mem, ne, n_points, hyp):
         pg, eg = it.integrate(_dev(ev), n_points, SEED)
         pg, eg = pg.cpu().numpy(), eg.cpu().numpy()
     check_events_conic(pg, eg, po, eo, _drill(mem, ev, n_points, dict(tth_hyp=hyp)), n_points,
-                       ill=conic_ill_conditioned(ev, n_jets=4))
+                       ill=conic_ill_conditioned(ev, n_jets=4), max_miss=max_miss)
     if n_points > 1000:
         assert (po > 0).sum() >= ne // 2
 
