@@ -408,7 +408,9 @@ def run_b200(args):
                          "flop_per_call_algorithmic": None, "executed_counts_match_build": f.get("match"),
                          "peak_source": "derived: 128 FP32 FMA/clk/SM x SMs x sampled SM clock (DESIGN.md); executed FP32 flops",
                          "fp64_flop_per_call_kept": fl_ex})
-        for k in ("fp64_pipe_frac", "fp64_inst_per_call", "achieved_executed", "frac_executed", "executed_counts"):
+        roofline["frac_basis"] = "executed FP32 flops" + (" (STALE: counts from another build)" if f.get("match") is False else "")
+        for k in ("fp64_pipe_frac", "fp64_inst_per_call", "achieved_executed", "frac_executed", "executed_counts",
+                  "achieved_fixed_reference", "frac_fixed_reference", "flop_per_call_algorithmic_note"):
             roofline.pop(k, None)
     h2d = ne * mem.mem_event_fields(proc) * 8
     d2h = 2 * ne * 8
